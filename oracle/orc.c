@@ -1,0 +1,514 @@
+/* oracle/orc.c -- CPU ORACLE, TEST INFRASTRUCTURE ONLY (see orc.h).
+ *
+ * Plain nested loops over cells, nodes and edges, in the paper's order and notation; fp64 by
+ * default.  No blocking, fusion or layout tricks; OpenMP over z-planes / nodes only.
+ * Every function cites the passage of /root/reference/PAPER.md it follows ("L" = line number)
+ * or the SURVEY.md section 8(c) reading ("O-n", "G-n") taken where the paper is silent/garbled.
+ *
+ * PARITY UNPINNED (conventions fixed in DESIGN.md, not by the paper): which velocity is
+ * interpolated (G11, reading A), the wall density rho_w = 1 (G9), dropped stencil cells at a
+ * wall (G15), the corner rule for links leaving through two wall faces at once.
+ */
+#include "orc.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef ORC_REAL_FLOAT
+typedef float real;
+#else
+typedef double real;
+#endif
+
+#define Q 19
+/* internal storage: the 19 values of a lattice site side by side (L181 "19 values f_i(x,t) are
+ * stored at each lattice site"); the interface (orc.h) is SoA f[i*cells + q] */
+#define FI(i, q) ((size_t)(q) * Q + (size_t)(i))
+static const double PI = 3.14159265358979323846264338327950288;
+
+/* D3Q19 vectors in the paper's numbering (1-based i -> row i-1).  The paper shows them only in
+ * Fig. 4 (L434); the order is fixed uniquely by the boundary equations Eq. 23-30 (L217-238):
+ * {i : c_z=+1} = {5,9,13,15,17}, opposites 5/6, 9/14, 13/10, 15/18, 17/16, +x set {1,7,8},
+ * -x set {2,11,12}, +y set {3,7,11}, -y set {4,8,12}; rest population is i = 19 (Eq. 21).   */
+static const int C[Q][3] = {
+    {+1, 0, 0}, {-1, 0, 0}, {0, +1, 0}, {0, -1, 0}, {0, 0, +1}, {0, 0, -1},      /* 1..6   */
+    {+1, +1, 0}, {+1, -1, 0}, {+1, 0, +1}, {+1, 0, -1},                           /* 7..10  */
+    {-1, +1, 0}, {-1, -1, 0}, {-1, 0, +1}, {-1, 0, -1},                           /* 11..14 */
+    {0, +1, +1}, {0, +1, -1}, {0, -1, +1}, {0, -1, -1},                           /* 15..18 */
+    {0, 0, 0}};                                                                   /* 19     */
+
+/* Eq. 21 (L208): 2/36 for i=1..6, 1/36 for i=7..18, 12/36 for i=19 */
+static double weight(int i0) { return i0 < 6 ? 2.0 / 36.0 : (i0 < 18 ? 1.0 / 36.0 : 12.0 / 36.0); }
+
+static int opposite(int i0) {
+    for (int j = 0; j < Q; ++j)
+        if (C[j][0] == -C[i0][0] && C[j][1] == -C[i0][1] && C[j][2] == -C[i0][2]) return j;
+    return -1;
+}
+static int OPP[Q];   /* OPP[i] = opposite(i), filled by orc_create */
+
+struct orc_ctx {
+    int n[3];
+    long cells;
+    real tau;
+    int kind[3];
+    real u_lo[3][3], u_hi[3][3];
+    real *f, *fstar, *g_last;          /* f[FI(i,q)]; g_last[d*cells+q] */
+    /* meshes, concatenated in orc_add_mesh order */
+    int n_nodes, n_edges, n_meshes, cap_nodes, cap_edges;
+    real *X, *F, *U;                   /* AoS 3 per node */
+    int *edge;                         /* global node index pairs */
+    real *rest, *kspring;              /* per edge */
+    int forces_valid;
+};
+
+void orc_lattice(int* c_out, double* w_out) {
+    for (int i = 0; i < Q; ++i) {
+        for (int d = 0; d < 3; ++d) c_out[3 * i + d] = C[i][d];
+        w_out[i] = weight(i);
+    }
+}
+int orc_real_bytes(void) { return (int)sizeof(real); }
+
+/* ---- Eq. 36 (L273), with the second case read as |r| >= 2 (G6) -------------------------- */
+double orc_phi(double r) {
+    double a = fabs(r);
+    if (a >= 2.0) return 0.0;
+    return 0.25 * (1.0 + cos(PI * r / 2.0));
+}
+static real phi(real r) { return (real)orc_phi((double)r); }
+
+/* ---- Eq. 20 (L203): f_eq = w rho [1 + c.v/cs^2 + (c.v)^2/(2 cs^4) - v^2/(2 cs^2)], cs^2 = 1/3 */
+static real feq(int i, real rho, const real v[3]) {
+    real cv = C[i][0] * v[0] + C[i][1] * v[1] + C[i][2] * v[2];
+    real vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    return (real)weight(i) * rho * ((real)1 + (real)3 * cv + (real)4.5 * cv * cv - (real)1.5 * vv);
+}
+double orc_feq(int i0, double rho, const double v[3]) {
+    real vr[3] = {(real)v[0], (real)v[1], (real)v[2]};
+    return (double)feq(i0, (real)rho, vr);
+}
+
+/* ---- O-8: Philox4x32-10 (Salmon et al., SC'11): 10 rounds of
+ *   (c0,c1,c2,c3) <- (hi(M1 c2)^c1^k0, lo(M1 c2), hi(M0 c0)^c3^k1, lo(M0 c0)),
+ * key bumped by the Weyl constants (W0, W1) between rounds.                                */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) { k0 += W0; k1 += W1; }
+        uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+/* xi = ((r >> 8) + 0.5) 2^-24: exact in fp32, never 0 or 1 */
+double orc_uniform01(uint32_t r) { return ((double)(r >> 8) + 0.5) * (1.0 / 16777216.0); }
+
+static void noise_words(uint64_t seed, uint64_t index, uint32_t step, uint32_t tag, uint32_t r[4]) {
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    uint32_t ctr[4] = {(uint32_t)index, (uint32_t)(index >> 32), step, tag};
+    orc_philox4x32_10(ctr, key, r);
+}
+void orc_noise_uniform(uint64_t seed, uint64_t index, uint32_t step, uint32_t tag, double xi[4]) {
+    uint32_t r[4];
+    noise_words(seed, index, step, tag, r);
+    for (int j = 0; j < 4; ++j) xi[j] = orc_uniform01(r[j]);
+}
+/* Box-Muller: z0 = sqrt(-2 ln xi0) cos(2 pi xi1), z1 = same radius * sin(2 pi xi1),
+ *             z2 = sqrt(-2 ln xi2) cos(2 pi xi3)                                            */
+void orc_noise_normal3(uint64_t seed, uint64_t index, uint32_t step, uint32_t tag, double z[3]) {
+    double xi[4];
+    orc_noise_uniform(seed, index, step, tag, xi);
+    double r0 = sqrt(-2.0 * log(xi[0])), r2 = sqrt(-2.0 * log(xi[2]));
+    z[0] = r0 * cos(2.0 * PI * xi[1]);
+    z[1] = r0 * sin(2.0 * PI * xi[1]);
+    z[2] = r2 * cos(2.0 * PI * xi[3]);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+int orc_create(int nx, int ny, int nz, double tau, const int kind[3], const double u_lo[9],
+               const double u_hi[9], orc_ctx** out) {
+    if (!out || nx < 1 || ny < 1 || nz < 1 || !(tau > 0.5) || !kind) return -1;
+    orc_ctx* c = (orc_ctx*)calloc(1, sizeof(orc_ctx));
+    for (int i = 0; i < Q; ++i) OPP[i] = opposite(i);
+    c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
+    c->cells = (long)nx * ny * nz;
+    c->tau = (real)tau;
+    for (int a = 0; a < 3; ++a) {
+        if (kind[a] != ORC_PERIODIC && kind[a] != ORC_WALL) { free(c); return -1; }
+        c->kind[a] = kind[a];
+        for (int d = 0; d < 3; ++d) {
+            c->u_lo[a][d] = u_lo ? (real)u_lo[3 * a + d] : 0;
+            c->u_hi[a][d] = u_hi ? (real)u_hi[3 * a + d] : 0;
+        }
+    }
+    c->f = (real*)calloc((size_t)Q * c->cells, sizeof(real));
+    c->fstar = (real*)calloc((size_t)Q * c->cells, sizeof(real));
+    c->g_last = (real*)calloc((size_t)3 * c->cells, sizeof(real));
+    if (!c->f || !c->fstar || !c->g_last) { orc_destroy(c); return -1; }
+    *out = c;
+    return 0;
+}
+
+int orc_destroy(orc_ctx* c) {
+    if (!c) return -1;
+    free(c->f); free(c->fstar); free(c->g_last);
+    free(c->X); free(c->F); free(c->U); free(c->edge); free(c->rest); free(c->kspring);
+    free(c);
+    return 0;
+}
+
+/* O-2: f_i = feq_i(rho, u) (Eq. 20) + amp (2 xi - 1), xi = Philox uniform keyed on
+ * (index = cell*19 + (i-1), step 0, tag 1), first output word. */
+int orc_set_equilibrium(orc_ctx* c, const double* rho, const double* u, double amp, uint64_t seed) {
+    if (!c) return -1;
+    const long N = c->cells;
+    for (long q = 0; q < N; ++q) {
+        real r = rho ? (real)rho[q] : (real)1;
+        real v[3] = {u ? (real)u[q] : 0, u ? (real)u[N + q] : 0, u ? (real)u[2 * N + q] : 0};
+        for (int i = 0; i < Q; ++i) {
+            real val = feq(i, r, v);
+            if (amp > 0) {
+                double xi[4];
+                orc_noise_uniform(seed, (uint64_t)q * Q + (uint64_t)i, 0u, 1u, xi);
+                val += (real)(amp * (2.0 * xi[0] - 1.0));
+            }
+            c->f[FI(i, q)] = val;
+        }
+    }
+    memset(c->g_last, 0, (size_t)3 * N * sizeof(real));
+    return 0;
+}
+
+/* O-3 steps 1-5 for one cell: moments (Eq. 17-18), v = u + g/(2 rho) (L201), f_eq(rho, v)
+ * (Eq. 20), BGK relaxation (Eq. 16) and the Guo term (Eq. 19 read per G3: the tensor
+ * (c c^T - cs^2 I) and v, equivalent to S_i = (1 - 1/2tau) w_i [3 (c_i - v).g + 9 (c_i.v)(c_i.g)]). */
+static void collide_cell(const orc_ctx* c, const real fin[Q], const real g[3], real fout[Q]) {
+    real rho = 0, j[3] = {0, 0, 0};
+    for (int i = 0; i < Q; ++i) {
+        rho += fin[i];
+        for (int d = 0; d < 3; ++d) j[d] += C[i][d] * fin[i];
+    }
+    real v[3];
+    for (int d = 0; d < 3; ++d) v[d] = (j[d] + g[d] / 2) / rho;
+    for (int i = 0; i < Q; ++i) {
+        real cv = C[i][0] * v[0] + C[i][1] * v[1] + C[i][2] * v[2];
+        real cg = C[i][0] * g[0] + C[i][1] * g[1] + C[i][2] * g[2];
+        real cmv_g = (C[i][0] - v[0]) * g[0] + (C[i][1] - v[1]) * g[1] + (C[i][2] - v[2]) * g[2];
+        real S = ((real)1 - (real)1 / (2 * c->tau)) * (real)weight(i) * ((real)3 * cmv_g + (real)9 * cv * cg);
+        fout[i] = fin[i] - (fin[i] - feq(i, rho, v)) / c->tau + S;
+    }
+}
+
+/* O-3: collide every cell, then stream: periodic axes wrap (L217); a link leaving through a wall
+ * face is bounced back into the opposite direction at the same cell with Ladd's moving-wall
+ * term, f_new,ibar(x) = f*_i(x) - 6 w_i rho_w (c_i.u_w), rho_w = 1 (G9: halfway bounce-back,
+ * walls half a spacing outside the first/last fluid layer).  Corner rule: the wall velocity is
+ * that of the first wall axis (x, y, z order) the link leaves through. */
+int orc_step(orc_ctx* c, const double* g) {
+    if (!c) return -1;
+    const long N = c->cells;
+    const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
+#pragma omp parallel for schedule(static)
+    for (long q = 0; q < N; ++q) {
+        real fin[Q], fout[Q], gq[3];
+        for (int i = 0; i < Q; ++i) fin[i] = c->f[FI(i, q)];
+        for (int d = 0; d < 3; ++d) gq[d] = g ? (real)g[(size_t)d * N + q] : 0;
+        collide_cell(c, fin, gq, fout);
+        for (int i = 0; i < Q; ++i) c->fstar[FI(i, q)] = fout[i];
+        for (int d = 0; d < 3; ++d) c->g_last[(size_t)d * N + q] = gq[d];
+    }
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < ny; ++y)
+            for (int x = 0; x < nx; ++x) {
+                const long q = x + (long)nx * (y + (long)ny * z);
+                const int xs[3] = {x, y, z};
+                for (int i = 0; i < Q; ++i) {
+                    int xp[3];
+                    const real* uw = NULL;
+                    for (int a = 0; a < 3; ++a) {
+                        xp[a] = xs[a] + C[i][a];
+                        if (xp[a] < 0) {
+                            if (c->kind[a] == ORC_PERIODIC) xp[a] += c->n[a];
+                            else if (!uw) uw = c->u_lo[a];
+                        } else if (xp[a] >= c->n[a]) {
+                            if (c->kind[a] == ORC_PERIODIC) xp[a] -= c->n[a];
+                            else if (!uw) uw = c->u_hi[a];
+                        }
+                    }
+                    const real fs = c->fstar[FI(i, q)];
+                    if (uw) {
+                        real cu = C[i][0] * uw[0] + C[i][1] * uw[1] + C[i][2] * uw[2];
+                        c->f[FI(OPP[i], q)] = fs - (real)6 * (real)weight(i) * (real)1 * cu;
+                    } else {
+                        const long qp = xp[0] + (long)nx * (xp[1] + (long)ny * xp[2]);
+                        c->f[FI(i, qp)] = fs;
+                    }
+                }
+            }
+    return 0;
+}
+
+/* O-4: rho = sum f_i (Eq. 17); v = (sum c_i f_i + g_last/2)/rho (Eq. 18) */
+int orc_read_macros(orc_ctx* c, double* rho, double* u) {
+    if (!c) return -1;
+    const long N = c->cells;
+    for (long q = 0; q < N; ++q) {
+        real r = 0, j[3] = {0, 0, 0};
+        for (int i = 0; i < Q; ++i) {
+            real fi = c->f[FI(i, q)];
+            r += fi;
+            for (int d = 0; d < 3; ++d) j[d] += C[i][d] * fi;
+        }
+        if (rho) rho[q] = (double)r;
+        if (u)
+            for (int d = 0; d < 3; ++d) u[(size_t)d * N + q] = (double)((j[d] + c->g_last[(size_t)d * N + q] / 2) / r);
+    }
+    return 0;
+}
+
+int orc_read_populations(orc_ctx* c, double* f) {
+    if (!c || !f) return -1;
+    for (int i = 0; i < Q; ++i)
+        for (long q = 0; q < c->cells; ++q) f[(size_t)i * c->cells + q] = (double)c->f[FI(i, q)];
+    return 0;
+}
+int orc_write_populations(orc_ctx* c, const double* f) {
+    if (!c || !f) return -1;
+    for (int i = 0; i < Q; ++i)
+        for (long q = 0; q < c->cells; ++q) c->f[FI(i, q)] = (real)f[(size_t)i * c->cells + q];
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+int orc_add_mesh(orc_ctx* c, int n_nodes, const double* xyz, int n_edges, const int* edges,
+                 const double* rest, double k, int* out_mesh_id) {
+    if (!c || n_nodes < 1 || !xyz || n_edges < 0 || (n_edges && !edges)) return -1;
+    for (int e = 0; e < n_edges; ++e)
+        if (edges[2 * e] < 0 || edges[2 * e] >= n_nodes || edges[2 * e + 1] < 0 || edges[2 * e + 1] >= n_nodes ||
+            edges[2 * e] == edges[2 * e + 1])
+            return -1;
+    if (c->n_nodes + n_nodes > c->cap_nodes) {
+        c->cap_nodes = 2 * (c->n_nodes + n_nodes);
+        c->X = (real*)realloc(c->X, (size_t)3 * c->cap_nodes * sizeof(real));
+        c->F = (real*)realloc(c->F, (size_t)3 * c->cap_nodes * sizeof(real));
+        c->U = (real*)realloc(c->U, (size_t)3 * c->cap_nodes * sizeof(real));
+    }
+    if (c->n_edges + n_edges > c->cap_edges) {
+        c->cap_edges = 2 * (c->n_edges + n_edges);
+        c->edge = (int*)realloc(c->edge, (size_t)2 * c->cap_edges * sizeof(int));
+        c->rest = (real*)realloc(c->rest, (size_t)c->cap_edges * sizeof(real));
+        c->kspring = (real*)realloc(c->kspring, (size_t)c->cap_edges * sizeof(real));
+    }
+    const int off = c->n_nodes;
+    for (int m = 0; m < 3 * n_nodes; ++m) {
+        c->X[3 * off + m] = (real)xyz[m];
+        c->F[3 * off + m] = 0;
+        c->U[3 * off + m] = 0;
+    }
+    for (int e = 0; e < n_edges; ++e) {
+        const int a = edges[2 * e], b = edges[2 * e + 1], ge = c->n_edges + e;
+        c->edge[2 * ge] = off + a;
+        c->edge[2 * ge + 1] = off + b;
+        if (rest) c->rest[ge] = (real)rest[e];
+        else {
+            double s = 0;
+            for (int d = 0; d < 3; ++d) s += (xyz[3 * b + d] - xyz[3 * a + d]) * (xyz[3 * b + d] - xyz[3 * a + d]);
+            c->rest[ge] = (real)sqrt(s);
+        }
+        c->kspring[ge] = (real)k;
+    }
+    c->n_nodes += n_nodes;
+    c->n_edges += n_edges;
+    if (out_mesh_id) *out_mesh_id = c->n_meshes;
+    c->n_meshes += 1;
+    c->forces_valid = 0;
+    return 0;
+}
+
+/* O-5: F <- 0; for each edge (a,b): R = X_b - X_a, l = |R|, e = k (l - L) R / l; F_a += e,
+ * F_b -= e.  Eq. 2-3 (L92-99) with the sign read per G1: the force on point i is -grad_{X_i} of
+ * Eq. 2, i.e. +k(|R|-L)R/|R| with R = X_j - X_i (attracting when stretched).  If sigma > 0,
+ * F_m,d += sigma z_d(m, step): Philox normals keyed on (global node m, step, tag 2). */
+int orc_compute_membrane_forces(orc_ctx* c, double sigma, uint64_t seed, uint64_t step) {
+    if (!c) return -1;
+    for (int m = 0; m < 3 * c->n_nodes; ++m) c->F[m] = 0;
+    for (int e = 0; e < c->n_edges; ++e) {
+        const int a = c->edge[2 * e], b = c->edge[2 * e + 1];
+        real R[3], l2 = 0;
+        for (int d = 0; d < 3; ++d) {
+            R[d] = c->X[3 * b + d] - c->X[3 * a + d];
+            l2 += R[d] * R[d];
+        }
+        const real l = (real)sqrt((double)l2);
+        if (!(l > 0)) return -1;
+        for (int d = 0; d < 3; ++d) {
+            const real ed = c->kspring[e] * (l - c->rest[e]) * R[d] / l;
+            c->F[3 * a + d] += ed;
+            c->F[3 * b + d] -= ed;
+        }
+    }
+    if (sigma > 0)
+        for (int m = 0; m < c->n_nodes; ++m) {
+            double z[3];
+            orc_noise_normal3(seed, (uint64_t)m, (uint32_t)step, 2u, z);
+            for (int d = 0; d < 3; ++d) c->F[3 * m + d] += (real)(sigma * z[d]);
+        }
+    c->forces_valid = 1;
+    return 0;
+}
+
+double orc_spring_energy(orc_ctx* c) {
+    double H = 0;
+    for (int e = 0; e < c->n_edges; ++e) {
+        const int a = c->edge[2 * e], b = c->edge[2 * e + 1];
+        double l2 = 0;
+        for (int d = 0; d < 3; ++d) {
+            double r = (double)c->X[3 * b + d] - (double)c->X[3 * a + d];
+            l2 += r * r;
+        }
+        const double dl = sqrt(l2) - (double)c->rest[e];
+        H += 0.5 * (double)c->kspring[e] * dl * dl;     /* Eq. 2 (L94) */
+    }
+    return H;
+}
+
+/* Stencil of node X (O-6/O-7): base b_d = floor(X_d) - 1; cells q_d = b_d + o_d, o in {0..3}^3;
+ * weight W = prod_d phi(X_d - q_d) (Eq. 35-36 with h = 1, so h^3 delta_h = phi phi phi);
+ * periodic axes: index q_d mod n_d; wall axes: the cell is skipped if outside (G15).
+ * Returns the wrapped linear cell index or -1 if dropped. */
+static long stencil_cell(const orc_ctx* c, const real X[3], const int o[3], real* W) {
+    long idx[3];
+    real w = 1;
+    for (int d = 0; d < 3; ++d) {
+        const long b = (long)floor((double)X[d]) - 1;
+        long qd = b + o[d];
+        w *= phi(X[d] - (real)qd);
+        if (c->kind[d] == ORC_PERIODIC) {
+            qd %= c->n[d];
+            if (qd < 0) qd += c->n[d];
+        } else if (qd < 0 || qd >= c->n[d]) {
+            *W = 0;
+            return -1;
+        }
+        idx[d] = qd;
+    }
+    *W = w;
+    return idx[0] + (long)c->n[0] * (idx[1] + (long)c->n[1] * idx[2]);
+}
+
+/* O-6: g_ijk = sum_m F_m phi phi phi (Eq. 34); g starts from zero each step. */
+int orc_spread(orc_ctx* c, double* g) {
+    if (!c || !g) return -1;
+    if (c->n_nodes && !c->forces_valid) return -4;
+    const long N = c->cells;
+    real* acc = (real*)calloc((size_t)3 * N, sizeof(real));
+    for (int m = 0; m < c->n_nodes; ++m)
+        for (int oz = 0; oz < 4; ++oz)
+            for (int oy = 0; oy < 4; ++oy)
+                for (int ox = 0; ox < 4; ++ox) {
+                    const int o[3] = {ox, oy, oz};
+                    real W;
+                    const long q = stencil_cell(c, &c->X[3 * m], o, &W);
+                    if (q < 0) continue;
+                    for (int d = 0; d < 3; ++d) acc[(size_t)d * N + q] += W * c->F[3 * m + d];
+                }
+    for (size_t s = 0; s < (size_t)3 * N; ++s) g[s] = (double)acc[s];
+    free(acc);
+    return 0;
+}
+
+static void interpolate(const orc_ctx* c, const real* w /*3*cells*/, real* U) {
+    const long N = c->cells;
+#pragma omp parallel for schedule(static)
+    for (int m = 0; m < c->n_nodes; ++m) {
+        real Um[3] = {0, 0, 0};
+        for (int oz = 0; oz < 4; ++oz)
+            for (int oy = 0; oy < 4; ++oy)
+                for (int ox = 0; ox < 4; ++ox) {
+                    const int o[3] = {ox, oy, oz};
+                    real W;
+                    const long q = stencil_cell(c, &c->X[3 * m], o, &W);
+                    if (q < 0) continue;
+                    for (int d = 0; d < 3; ++d) Um[d] += W * w[(size_t)d * N + q];
+                }
+        for (int d = 0; d < 3; ++d) U[3 * m + d] = Um[d];
+    }
+}
+
+int orc_interpolate_field(orc_ctx* c, const double* w, double* U) {
+    if (!c || !w || !U) return -1;
+    const long N = c->cells;
+    real* wr = (real*)malloc((size_t)3 * N * sizeof(real));
+    real* Ur = (real*)malloc((size_t)3 * (c->n_nodes + 1) * sizeof(real));
+    for (size_t s = 0; s < (size_t)3 * N; ++s) wr[s] = (real)w[s];
+    interpolate(c, wr, Ur);
+    for (int m = 0; m < 3 * c->n_nodes; ++m) U[m] = (double)Ur[m];
+    free(wr); free(Ur);
+    return 0;
+}
+
+/* O-7: U_m = sum_ijk v_ijk phi phi phi (Eq. 33) with v the macroscopic velocity of the
+ * CURRENT lattice state (after orc_step; reading A of G11: v = (sum c f^{n+1} + g^n/2)/rho^{n+1})
+ * and the stencil around the not-yet-moved X_m (G13); then X_m <- X_m + U_m (forward Euler, G12;
+ * Fig. 1 "positions were updated based on the velocities").  Positions stay unwrapped (G17).
+ * Returns -5 if a node left the channel through a wall axis (X_d outside [-1/2, n_d - 1/2]). */
+int orc_interpolate_advance(orc_ctx* c) {
+    if (!c) return -1;
+    const long N = c->cells;
+    real* v = (real*)malloc((size_t)3 * N * sizeof(real));
+    for (long q = 0; q < N; ++q) {
+        real r = 0, j[3] = {0, 0, 0};
+        for (int i = 0; i < Q; ++i) {
+            real fi = c->f[FI(i, q)];
+            r += fi;
+            for (int d = 0; d < 3; ++d) j[d] += C[i][d] * fi;
+        }
+        for (int d = 0; d < 3; ++d) v[(size_t)d * N + q] = (j[d] + c->g_last[(size_t)d * N + q] / 2) / r;
+    }
+    interpolate(c, v, c->U);
+    free(v);
+    int left = 0;
+    for (int m = 0; m < c->n_nodes; ++m)
+        for (int d = 0; d < 3; ++d) {
+            c->X[3 * m + d] += c->U[3 * m + d];
+            if (c->kind[d] == ORC_WALL &&
+                (c->X[3 * m + d] < (real)-0.5 || c->X[3 * m + d] > (real)c->n[d] - (real)0.5))
+                left = 1;
+        }
+    c->forces_valid = 0;
+    return left ? -5 : 0;
+}
+
+int orc_n_nodes(orc_ctx* c) { return c ? c->n_nodes : -1; }
+int orc_read_nodes(orc_ctx* c, double* xyz) {
+    if (!c || !xyz) return -1;
+    for (int m = 0; m < 3 * c->n_nodes; ++m) xyz[m] = (double)c->X[m];
+    return 0;
+}
+int orc_write_nodes(orc_ctx* c, const double* xyz) {
+    if (!c || !xyz) return -1;
+    for (int m = 0; m < 3 * c->n_nodes; ++m) c->X[m] = (real)xyz[m];
+    c->forces_valid = 0;
+    return 0;
+}
+int orc_read_forces(orc_ctx* c, double* F) {
+    if (!c || !F) return -1;
+    for (int m = 0; m < 3 * c->n_nodes; ++m) F[m] = (double)c->F[m];
+    return 0;
+}
+int orc_write_forces(orc_ctx* c, const double* F) {
+    if (!c || !F) return -1;
+    for (int m = 0; m < 3 * c->n_nodes; ++m) c->F[m] = (real)F[m];
+    c->forces_valid = 1;
+    return 0;
+}
+int orc_read_node_velocities(orc_ctx* c, double* U) {
+    if (!c || !U) return -1;
+    for (int m = 0; m < 3 * c->n_nodes; ++m) U[m] = (double)c->U[m];
+    return 0;
+}

@@ -1,0 +1,74 @@
+/* oracle/orc.h -- CPU ORACLE, TEST INFRASTRUCTURE ONLY.
+ *
+ * A plain, slow, obviously-correct implementation of the per-time-step fluid-structure hot path of
+ * arXiv:1312.2234 (section 3.3, 3.4.2, Eq. 2-3, 15-21, 31-36), written from the paper.
+ * It shares no code with the CUDA library.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may call it; the product path never does.
+ *
+ * All pointers are HOST pointers.  All floating point arrays at this interface are double,
+ * whatever the internal precision (the default build is fp64; -DORC_REAL_FLOAT builds the fp32
+ * diagnostic mode).  Linear cell index q = i + nx*(j + ny*k); fields are SoA: rho[cells],
+ * u[3*cells] = (ux[cells], uy[cells], uz[cells]); populations f[19*cells] = f_i at [i*cells + q]
+ * with i = (paper's 1-based index) - 1, the order fixed by PAPER.md Eq. 23-30 (see orc.c).
+ *
+ * Return codes: 0 ok, -1 invalid argument, -4 wrong call order, -5 a node left the channel.
+ */
+#ifndef ORC_H
+#define ORC_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_ctx orc_ctx;
+
+enum { ORC_PERIODIC = 0, ORC_WALL = 1 };
+
+/* lattice constants: c[19][3] and w[19] in the paper's order (Eq. 21, Eq. 23-30) */
+void orc_lattice(int* c_out /*19*3*/, double* w_out /*19*/);
+int  orc_real_bytes(void);   /* 8 (fp64 build) or 4 (fp32 build) */
+
+/* PAPER.md Eq. 36: phi(r) = (1 + cos(pi r / 2))/4 for |r| < 2, else 0 */
+double orc_phi(double r);
+/* PAPER.md Eq. 20 (one population, paper index i0 = i-1) */
+double orc_feq(int i0, double rho, const double v[3]);
+/* Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11) and the derived uniform / normal variates */
+void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+double orc_uniform01(uint32_t r);                                  /* ((r>>8)+0.5) 2^-24 */
+void   orc_noise_uniform(uint64_t seed, uint64_t index, uint32_t step, uint32_t tag, double xi[4]);
+void   orc_noise_normal3(uint64_t seed, uint64_t index, uint32_t step, uint32_t tag, double z[3]);
+
+int orc_create(int nx, int ny, int nz, double tau, const int kind[3],
+               const double u_lo[9] /*[axis][comp]*/, const double u_hi[9], orc_ctx** out);
+int orc_destroy(orc_ctx*);
+
+/* f_i = feq_i(rho, u) + amp (2 xi - 1); rho NULL = 1, u NULL = 0 */
+int orc_set_equilibrium(orc_ctx*, const double* rho, const double* u, double noise_amp, uint64_t seed);
+/* one collide + stream + boundary step with force density g[3*cells] (NULL = 0) */
+int orc_step(orc_ctx*, const double* g);
+/* rho = sum f_i, v = (sum c_i f_i + g_last/2)/rho of the current state */
+int orc_read_macros(orc_ctx*, double* rho, double* u);
+int orc_read_populations(orc_ctx*, double* f /*19*cells*/);
+int orc_write_populations(orc_ctx*, const double* f);
+
+int orc_add_mesh(orc_ctx*, int n_nodes, const double* xyz /*AoS*/, int n_edges, const int* edges,
+                 const double* rest /*NULL = lengths of xyz*/, double k, int* out_mesh_id);
+int orc_compute_membrane_forces(orc_ctx*, double sigma, uint64_t seed, uint64_t step);
+int orc_spread(orc_ctx*, double* g /*3*cells, overwritten*/);
+int orc_interpolate_advance(orc_ctx*);
+int orc_n_nodes(orc_ctx*);
+int orc_read_nodes(orc_ctx*, double* xyz /*AoS*/);
+int orc_write_nodes(orc_ctx*, const double* xyz);
+int orc_read_forces(orc_ctx*, double* F /*AoS*/);
+int orc_write_forces(orc_ctx*, const double* F);
+int orc_read_node_velocities(orc_ctx*, double* U /*AoS, of the last interpolate*/);
+/* Eq. 2 summed over all edges of all meshes: H_SCE = sum k/2 (|R| - L)^2 */
+double orc_spring_energy(orc_ctx*);
+/* U_m = sum_cells w[q] phi phi phi around the CURRENT node positions, for any field w[3*cells];
+ * no advance (used for the adjointness pin) */
+int orc_interpolate_field(orc_ctx*, const double* w, double* U /*AoS*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
