@@ -1,0 +1,151 @@
+/* plb.h -- C-ABI of libplb: the per-time-step fluid-structure hot path of arXiv:1312.2234
+ * (Wu, Xu, Kim, Alber) as hand-written CUDA for one B200 (sm_100a).
+ *
+ * One coupled step (Fig. 1) is four calls, in this order:
+ *     ib_compute_membrane_forces -> ib_spread -> lbm_step(forcing) -> ib_interpolate_advance
+ *
+ * Conventions
+ *   - Lattice units h = dt = 1, c_s^2 = 1/3.  Lattice node (i,j,k) is the integer
+ *     point (i,j,k) (L268); linear cell index q = i + nx*(j + ny*k), x fastest.
+ *   - D3Q19, populations numbered as in the paper (Eq. 21 / Eq. 23-30): index i-1 at this
+ *     interface.  c = +x,-x,+y,-y,+z,-z, +x+y,+x-y,+x+z,+x-z, -x+y,-x-y,-x+z,-x-z, +y+z,+y-z,
+ *     -y+z,-y-z, 0; weights 2/36 (x6), 1/36 (x12), 12/36.
+ *   - "d_" arguments are DEVICE pointers owned by the caller; "h_" arguments are HOST pointers,
+ *     copied during the call (the caller keeps them).  No torch types cross this boundary.
+ *   - Scalar fields are float[cells]; vector fields handed to lbm_set_equilibrium /
+ *     lbm_read_macros are SoA float[3*cells] = (x[cells], y[cells], z[cells]).
+ *   - The FORCING field is AoS: float4 per cell = (g_x, g_y, g_z, 0), 16-byte aligned, so that
+ *     the spread can use 128-bit vector atomics.
+ *   - The library never allocates device memory: the caller passes one workspace of
+ *     lbm_workspace_bytes() bytes (256-byte aligned) to lbm_create, which carves it.
+ *   - Calls that take only device pointers are asynchronous on the context's stream.  Calls that
+ *     take host pointers synchronise that stream before returning.
+ *   - Every call returns 0 on success or a negative code (below); plb_last_error() gives a
+ *     thread-local message.  No exceptions, no aborts, no printing.  There is NO CPU fallback:
+ *     with no CUDA device every compute call fails with PLB_ERR_CUDA.
+ */
+#ifndef PLB_H
+#define PLB_H
+#include <stddef.h>
+#if defined(__GNUC__)
+#define PLB_API __attribute__((visibility("default")))
+#else
+#define PLB_API
+#endif
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct plb_ctx plb_ctx; /* opaque */
+
+typedef struct { int nx, ny, nz; } plb_grid;
+
+enum { PLB_PERIODIC = 0, PLB_WALL_BB = 1 }; /* per axis */
+
+/* kind[a]: PLB_PERIODIC wraps populations across axis a.  PLB_WALL_BB closes both
+ * faces of axis a with link-wise halfway bounce-back: all n_a layers are fluid, the walls lie half
+ * a spacing outside (at -1/2 and n_a - 1/2), a link leaving through a face returns into the
+ * opposite direction at the same node with Ladd's moving-wall term -6 w_i rho_w (c_i . u_w),
+ * rho_w = 1 (reading G9).  u_lo[a] / u_hi[a] = wall velocity at the low / high face of
+ * axis a.  A link leaving through two wall faces at once takes the velocity of the first such
+ * axis in x, y, z order. */
+typedef struct {
+    int   kind[3];
+    float u_lo[3][3];
+    float u_hi[3][3];
+} plb_boundary;
+
+enum {
+    PLB_OK            =  0,
+    PLB_ERR_ARG       = -1, /* invalid argument */
+    PLB_ERR_WORKSPACE = -2, /* workspace too small / capacity exceeded */
+    PLB_ERR_CUDA      = -3, /* CUDA error (message in plb_last_error) */
+    PLB_ERR_ORDER     = -4, /* wrong call order (e.g. ib_spread before forces) */
+    PLB_ERR_NODE_LEFT = -5  /* a node left the channel through a wall axis */
+};
+
+PLB_API const char* plb_last_error(void);
+
+/* Bytes of workspace lbm_create needs for this grid and mesh capacity (two fp32 lattices, the
+ * sparse velocity field, segment bookkeeping, node and edge arrays). */
+PLB_API int lbm_workspace_bytes(const plb_grid* grid, long max_nodes, long max_edges, size_t* out_bytes);
+
+/* Create a context.  tau > 1/2 is the BGK relaxation time (Eq. 16).  d_workspace must stay
+ * valid until lbm_destroy.  cuda_stream is a cudaStream_t (NULL = the legacy default stream).
+ * The populations are undefined until lbm_set_equilibrium or lbm_write_populations. */
+PLB_API int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d_workspace,
+               size_t workspace_bytes, long max_nodes, long max_edges, void* cuda_stream,
+               plb_ctx** out);
+PLB_API int lbm_destroy(plb_ctx* ctx); /* frees host bookkeeping only */
+
+/* f_i = f_i^eq(rho, u) (Eq. 20) + noise_amp (2 xi - 1).  d_rho NULL = 1, d_u NULL = 0.
+ * xi = Philox4x32-10 uniform keyed on (seed; index = cell*19 + (i-1), step 0, tag 1), first
+ * output word, xi = ((r >> 8) + 1/2) 2^-24 (O-8).  Resets the step counter and g_last. */
+PLB_API int lbm_set_equilibrium(plb_ctx* ctx, const float* d_rho, const float* d_u, float noise_amp,
+                        unsigned long long seed);
+
+/* One fused collide + stream + boundary step (Eq. 16-21 with the Guo forcing of Eq. 19, periodic
+ * wrap L217, bounce-back as above).  d_forcing: float4 per cell, or NULL = no force.  When
+ * d_forcing is the buffer ib_spread last filled, only the cells that spread touched are read.
+ * The buffer must stay unmodified until ib_interpolate_advance / lbm_read_macros have consumed
+ * it (they add g/2 to the momentum, L201). */
+PLB_API int lbm_step(plb_ctx* ctx, const float* d_forcing);
+
+/* rho = sum f_i (Eq. 17), v = (sum c_i f_i + g_last/2)/rho (Eq. 18) of the current state.
+ * Either output may be NULL. */
+PLB_API int lbm_read_macros(plb_ctx* ctx, float* d_rho, float* d_u);
+
+/* Add one mesh (nodes = actin vertices, edges = filaments).  h_xyz: n_nodes x 3
+ * doubles (AoS, unwrapped lattice coordinates); h_edges: n_edges x 2 mesh-local node indices;
+ * h_rest: n_edges rest lengths L_ij (NULL = the lengths of h_xyz); k: spring stiffness of Eq. 2.
+ * Meshes are concatenated; global node index = running offset + local index. */
+PLB_API int ib_add_mesh(plb_ctx* ctx, int n_nodes, const double* h_xyz, int n_edges, const int* h_edges,
+                const float* h_rest, float k, int* out_mesh_id);
+/* n_meshes meshes of identical topology and rest lengths: h_xyz is n_meshes x n_nodes x 3. */
+PLB_API int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, int n_edges,
+                  const int* h_edges, const float* h_rest, float k, int* out_first_mesh_id);
+
+/* S1.  F <- 0; for every edge (a,b): R = X_b - X_a, e = k (|R| - L) R/|R|, F_a += e, F_b -= e
+ * (Eq. 2-3, sign read as F = -grad H, G1).  If noise_sigma > 0 adds
+ * noise_sigma * N(0,1) per node component from Philox keyed on (noise_seed; global node, step,
+ * tag 2) with Box-Muller (O-8). */
+PLB_API int ib_compute_membrane_forces(plb_ctx* ctx, float noise_sigma, unsigned long long noise_seed,
+                               unsigned long long step);
+
+/* S2.  g_ijk = sum_m F_m phi(i - X_m) phi(j - Y_m) phi(k - Z_m) (Eq. 34-36) with the
+ * 4-point cosine kernel phi(r) = (1 + cos(pi r/2))/4, |r| < 2, over the 4x4x4 cells
+ * floor(X) - 1 .. floor(X) + 2; periodic axes wrap the index, cells beyond a wall axis are
+ * dropped.  d_forcing (float4 per cell) must have been zero-filled once by the caller; each call
+ * first clears what the previous call on the same buffer wrote. */
+PLB_API int ib_spread(plb_ctx* ctx, float* d_forcing);
+
+/* S4 + S5.  U_m = sum_ijk v_ijk phi phi phi (Eq. 33) with v the velocity lbm_read_macros
+ * would return now (state after lbm_step, force just applied) and the stencil around the not yet
+ * moved X_m; then X_m <- X_m + U_m (forward Euler).  Positions are kept unwrapped in fp64.
+ * A node ending outside [-1/2, n_a - 1/2] on a wall axis raises a sticky flag that plb_status and
+ * ib_read_nodes report as PLB_ERR_NODE_LEFT. */
+PLB_API int ib_interpolate_advance(plb_ctx* ctx);
+
+/* ---- auxiliary, off the timed path (tests, checkpoints, end-to-end I/O) ---- */
+PLB_API int ib_n_nodes(plb_ctx* ctx, long* out);
+PLB_API int ib_read_nodes(plb_ctx* ctx, double* h_xyz);            /* n x 3 AoS */
+PLB_API int ib_write_nodes(plb_ctx* ctx, const double* h_xyz);
+PLB_API int ib_read_forces(plb_ctx* ctx, float* h_F);              /* n x 3 AoS */
+PLB_API int ib_write_forces(plb_ctx* ctx, const float* h_F);       /* marks forces valid (tests) */
+PLB_API int ib_read_node_velocities(plb_ctx* ctx, float* h_U);     /* n x 3 AoS, of the last interpolate */
+/* populations in the paper's order, true f_i (not the stored f_i - w_i), float[19*cells] SoA */
+PLB_API int lbm_read_populations(plb_ctx* ctx, float* d_f);
+PLB_API int lbm_write_populations(plb_ctx* ctx, const float* d_f);
+/* synchronise the stream; returns PLB_ERR_NODE_LEFT / PLB_ERR_CUDA if raised since creation */
+PLB_API int plb_status(plb_ctx* ctx);
+/* number of kernels this context has launched so far (for gpu_launches accounting) */
+PLB_API int plb_launch_count(plb_ctx* ctx, long* out);
+/* Philox4x32-10 block function on the device, for the known-answer test:
+ * d_ctr uint32[4n], d_key uint32[2n] -> d_out uint32[4n] */
+PLB_API int plb_philox4x32_10(void* cuda_stream, long n, const unsigned* d_ctr, const unsigned* d_key,
+                      unsigned* d_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

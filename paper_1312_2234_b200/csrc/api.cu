@@ -1,0 +1,489 @@
+// api.cu -- the C-ABI of libplb (include/plb.h): argument checks, workspace carving, call-order
+// bookkeeping.  Every step of the path runs in the kernels of lbm.cu / ib.cu.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "plb_internal.cuh"
+
+namespace plb {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int cuda_check(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return PLB_OK;
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return PLB_ERR_CUDA;
+}
+
+static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+struct Carve {
+    char* base;
+    size_t off;
+    template <typename T>
+    T* take(size_t count) {
+        T* p = reinterpret_cast<T*>(base + off);
+        off += align_up(count * sizeof(T));
+        return p;
+    }
+};
+
+// lays out the workspace; with base == nullptr it only measures
+static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes, long max_edges) {
+    Carve w{base, 0};
+    float* f0 = w.take<float>((size_t)Q * cells);
+    float* f1 = w.take<float>((size_t)Q * cells);
+    float4* vel = w.take<float4>((size_t)cells);
+    int* seg_flag = w.take<int>((size_t)n_segs);
+    int* seg_list = w.take<int>((size_t)n_segs);
+    int* counters = w.take<int>(64);
+    double* X0 = w.take<double>((size_t)max_nodes);
+    double* X1 = w.take<double>((size_t)max_nodes);
+    double* X2 = w.take<double>((size_t)max_nodes);
+    float4* F = w.take<float4>((size_t)max_nodes);
+    float4* U = w.take<float4>((size_t)max_nodes);
+    int2* edges = w.take<int2>((size_t)max_edges);
+    float2* eprm = w.take<float2>((size_t)max_edges);
+    if (c) {
+        c->f[0] = f0; c->f[1] = f1; c->vel = vel;
+        c->seg_flag = seg_flag; c->seg_list = seg_list; c->counters = counters;
+        c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U;
+        c->edges = edges; c->edge_prm = eprm;
+    }
+    return w.off;
+}
+
+static int check_grid(const plb_grid* g, long* cells) {
+    if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) {
+        set_error("invalid grid");
+        return PLB_ERR_ARG;
+    }
+    const long long n = (long long)g->nx * g->ny * g->nz;
+    if (n >= (1LL << 31) - 256) {
+        set_error("grid too large: %lld cells (limit 2^31)", n);
+        return PLB_ERR_ARG;
+    }
+    *cells = (long)n;
+    return PLB_OK;
+}
+
+static int sync_status(Ctx* c) {
+    int rc = cuda_check(cudaStreamSynchronize(c->stream), "cudaStreamSynchronize");
+    if (rc) return rc;
+    int h[2] = {0, 0};
+    rc = cuda_check(cudaMemcpy(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost), "read status");
+    if (rc) return rc;
+    if (h[1] & STATUS_ZERO_EDGE) {
+        set_error("a mesh edge has zero length");
+        return PLB_ERR_ARG;
+    }
+    if (h[1] & STATUS_NODE_LEFT) {
+        set_error("a node left the channel through a wall axis");
+        return PLB_ERR_NODE_LEFT;
+    }
+    return PLB_OK;
+}
+
+}  // namespace plb
+
+using namespace plb;
+
+#define REQUIRE_CTX(ctx)                 \
+    if (!(ctx)) {                        \
+        set_error("null context");       \
+        return PLB_ERR_ARG;              \
+    }
+
+extern "C" {
+
+const char* plb_last_error(void) { return g_err; }
+
+int lbm_workspace_bytes(const plb_grid* grid, long max_nodes, long max_edges, size_t* out_bytes) {
+    long cells;
+    int rc = check_grid(grid, &cells);
+    if (rc) return rc;
+    if (!out_bytes || max_nodes < 0 || max_edges < 0) {
+        set_error("invalid capacity / null output");
+        return PLB_ERR_ARG;
+    }
+    const long n_segs = (cells + SEG - 1) / SEG;
+    *out_bytes = carve(nullptr, nullptr, cells, n_segs, max_nodes, max_edges);
+    return PLB_OK;
+}
+
+int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d_workspace, size_t workspace_bytes,
+               long max_nodes, long max_edges, void* cuda_stream, plb_ctx** out) {
+    long cells;
+    int rc = check_grid(grid, &cells);
+    if (rc) return rc;
+    if (!out || !bnd || !d_workspace || !(tau > 0.5f) || max_nodes < 0 || max_edges < 0) {
+        set_error("lbm_create: invalid argument (tau must exceed 1/2)");
+        return PLB_ERR_ARG;
+    }
+    if (((uintptr_t)d_workspace & 255) != 0) {
+        set_error("lbm_create: workspace must be 256-byte aligned");
+        return PLB_ERR_ARG;
+    }
+    for (int a = 0; a < 3; ++a)
+        if (bnd->kind[a] != PLB_PERIODIC && bnd->kind[a] != PLB_WALL_BB) {
+            set_error("lbm_create: invalid boundary kind on axis %d", a);
+            return PLB_ERR_ARG;
+        }
+    const long n_segs = (cells + SEG - 1) / SEG;
+    const size_t need = carve(nullptr, nullptr, cells, n_segs, max_nodes, max_edges);
+    if (workspace_bytes < need) {
+        set_error("lbm_create: workspace of %zu bytes is smaller than the %zu needed", workspace_bytes, need);
+        return PLB_ERR_WORKSPACE;
+    }
+    int dev = 0, sms = 0;
+    rc = cuda_check(cudaGetDevice(&dev), "cudaGetDevice");
+    if (rc) return rc;
+    rc = cuda_check(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
+    if (rc) return rc;
+
+    plb_ctx* c = new (std::nothrow) plb_ctx();
+    if (!c) {
+        set_error("out of host memory");
+        return PLB_ERR_ARG;
+    }
+    c->grid = *grid;
+    c->tau = tau;
+    c->bnd = *bnd;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->n_segs = n_segs;
+    c->cur = 0;
+    c->cap_nodes = max_nodes; c->cap_edges = max_edges; c->n_nodes = 0; c->n_edges = 0;
+    c->g_last = nullptr; c->g_last_mode = FORCE_NONE; c->spread_target = nullptr;
+    c->spread_current = false; c->forces_valid = false; c->populated = false;
+    c->launches = 0;
+    c->sm_count = sms;
+    c->mesh_node_off.push_back(0);
+    c->mesh_edge_off.push_back(0);
+    carve(c, (char*)d_workspace, cells, n_segs, max_nodes, max_edges);
+
+    LbmParams& p = c->prm;
+    p.nx = grid->nx; p.ny = grid->ny; p.nz = grid->nz; p.cells = (int)cells;
+    p.omega = 1.0f / tau;
+    p.pref = 1.0f - 0.5f / tau;
+    for (int a = 0; a < 3; ++a) {
+        p.wall[a] = bnd->kind[a] == PLB_WALL_BB;
+        for (int d = 0; d < Q; ++d) {
+            const double w = d < 6 ? 1.0 / 18.0 : (d < 18 ? 1.0 / 36.0 : 1.0 / 3.0);
+            const double lo = CX(d) * (double)bnd->u_lo[a][0] + CY(d) * (double)bnd->u_lo[a][1] + CZ(d) * (double)bnd->u_lo[a][2];
+            const double hi = CX(d) * (double)bnd->u_hi[a][0] + CY(d) * (double)bnd->u_hi[a][1] + CZ(d) * (double)bnd->u_hi[a][2];
+            p.corr[a][0][d] = (float)(6.0 * w * lo);
+            p.corr[a][1][d] = (float)(6.0 * w * hi);
+        }
+    }
+    rc = cuda_check(cudaMemsetAsync(c->seg_flag, 0, (size_t)n_segs * sizeof(int), c->stream), "clear segment flags");
+    if (!rc) rc = cuda_check(cudaMemsetAsync(c->counters, 0, 64 * sizeof(int), c->stream), "clear counters");
+    if (rc) {
+        delete c;
+        return rc;
+    }
+    *out = c;
+    return PLB_OK;
+}
+
+int lbm_destroy(plb_ctx* ctx) {
+    REQUIRE_CTX(ctx);
+    cudaStreamSynchronize(ctx->stream);
+    delete ctx;
+    return PLB_OK;
+}
+
+int lbm_set_equilibrium(plb_ctx* ctx, const float* d_rho, const float* d_u, float noise_amp, unsigned long long seed) {
+    REQUIRE_CTX(ctx);
+    if (noise_amp < 0.f) {
+        set_error("noise_amp must be >= 0");
+        return PLB_ERR_ARG;
+    }
+    ctx->g_last = nullptr;
+    ctx->g_last_mode = FORCE_NONE;
+    ctx->populated = true;
+    return launch_set_equilibrium(ctx, d_rho, d_u, noise_amp, seed);
+}
+
+int lbm_step(plb_ctx* ctx, const float* d_forcing) {
+    REQUIRE_CTX(ctx);
+    if (!ctx->populated) {
+        set_error("lbm_step before lbm_set_equilibrium / lbm_write_populations");
+        return PLB_ERR_ORDER;
+    }
+    int mode = FORCE_NONE;
+    if (d_forcing) {
+        if (((uintptr_t)d_forcing & 15) != 0) {
+            set_error("forcing buffer must be 16-byte aligned (float4 per cell)");
+            return PLB_ERR_ARG;
+        }
+        mode = ((const float4*)d_forcing == ctx->spread_target) ? FORCE_SPARSE : FORCE_DENSE;
+    }
+    const int rc = launch_lbm_step(ctx, (const float4*)d_forcing, mode);
+    ctx->g_last = (const float4*)d_forcing;
+    ctx->g_last_mode = mode;
+    return rc;
+}
+
+int lbm_read_macros(plb_ctx* ctx, float* d_rho, float* d_u) {
+    REQUIRE_CTX(ctx);
+    if (!ctx->populated) {
+        set_error("lbm_read_macros before the populations were set");
+        return PLB_ERR_ORDER;
+    }
+    if (!d_rho && !d_u) return PLB_OK;
+    return launch_read_macros(ctx, d_rho, d_u);
+}
+
+int lbm_read_populations(plb_ctx* ctx, float* d_f) {
+    REQUIRE_CTX(ctx);
+    if (!d_f || !ctx->populated) {
+        set_error("lbm_read_populations: null output or populations not set");
+        return d_f ? PLB_ERR_ORDER : PLB_ERR_ARG;
+    }
+    return launch_read_populations(ctx, d_f);
+}
+
+int lbm_write_populations(plb_ctx* ctx, const float* d_f) {
+    REQUIRE_CTX(ctx);
+    if (!d_f) {
+        set_error("lbm_write_populations: null input");
+        return PLB_ERR_ARG;
+    }
+    ctx->g_last = nullptr;
+    ctx->g_last_mode = FORCE_NONE;
+    ctx->populated = true;
+    return launch_write_populations(ctx, d_f);
+}
+
+// ------------------------------------------------------------------------------------------------
+int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, int n_edges, const int* h_edges,
+                  const float* h_rest, float k, int* out_first_mesh_id) {
+    REQUIRE_CTX(ctx);
+    if (n_meshes < 1 || n_nodes < 1 || !h_xyz || n_edges < 0 || (n_edges > 0 && !h_edges)) {
+        set_error("ib_add_meshes: invalid argument");
+        return PLB_ERR_ARG;
+    }
+    for (int e = 0; e < n_edges; ++e) {
+        const int a = h_edges[2 * e], b = h_edges[2 * e + 1];
+        if (a < 0 || a >= n_nodes || b < 0 || b >= n_nodes || a == b) {
+            set_error("ib_add_meshes: edge %d = (%d, %d) is out of range or degenerate", e, a, b);
+            return PLB_ERR_ARG;
+        }
+    }
+    const long add_nodes = (long)n_meshes * n_nodes, add_edges = (long)n_meshes * n_edges;
+    if (ctx->n_nodes + add_nodes > ctx->cap_nodes || ctx->n_edges + add_edges > ctx->cap_edges) {
+        set_error("ib_add_meshes: capacity exceeded (%ld/%ld nodes, %ld/%ld edges)", ctx->n_nodes + add_nodes,
+                  ctx->cap_nodes, ctx->n_edges + add_edges, ctx->cap_edges);
+        return PLB_ERR_WORKSPACE;
+    }
+    if (ctx->n_nodes + add_nodes >= (1L << 31)) {
+        set_error("ib_add_meshes: more than 2^31 nodes");
+        return PLB_ERR_ARG;
+    }
+    // host-side marshalling: AoS -> SoA positions, mesh-local -> global edge indices
+    std::vector<double> soa((size_t)3 * add_nodes);
+    for (long m = 0; m < add_nodes; ++m)
+        for (int d = 0; d < 3; ++d) soa[(size_t)d * add_nodes + m] = h_xyz[3 * m + d];
+    std::vector<int2> eg((size_t)add_edges);
+    std::vector<float2> ep((size_t)add_edges);
+    for (int s = 0; s < n_meshes; ++s) {
+        const long noff = ctx->n_nodes + (long)s * n_nodes;
+        const double* x = h_xyz + (size_t)3 * s * n_nodes;
+        for (int e = 0; e < n_edges; ++e) {
+            const int a = h_edges[2 * e], b = h_edges[2 * e + 1];
+            float L;
+            if (h_rest) L = h_rest[e];
+            else {
+                double s2 = 0;
+                for (int d = 0; d < 3; ++d) s2 += (x[3 * b + d] - x[3 * a + d]) * (x[3 * b + d] - x[3 * a + d]);
+                L = (float)sqrt(s2);
+            }
+            eg[(size_t)s * n_edges + e] = make_int2((int)(noff + a), (int)(noff + b));
+            ep[(size_t)s * n_edges + e] = make_float2(L, k);
+        }
+    }
+    int rc = PLB_OK;
+    for (int d = 0; d < 3 && !rc; ++d)
+        rc = cuda_check(cudaMemcpyAsync(ctx->X[d] + ctx->n_nodes, soa.data() + (size_t)d * add_nodes,
+                                        (size_t)add_nodes * sizeof(double), cudaMemcpyHostToDevice, ctx->stream),
+                        "upload node positions");
+    if (!rc) rc = cuda_check(cudaMemsetAsync(ctx->F + ctx->n_nodes, 0, (size_t)add_nodes * sizeof(float4), ctx->stream), "clear forces");
+    if (!rc) rc = cuda_check(cudaMemsetAsync(ctx->U + ctx->n_nodes, 0, (size_t)add_nodes * sizeof(float4), ctx->stream), "clear node velocities");
+    if (!rc && add_edges) {
+        rc = cuda_check(cudaMemcpyAsync(ctx->edges + ctx->n_edges, eg.data(), (size_t)add_edges * sizeof(int2),
+                                        cudaMemcpyHostToDevice, ctx->stream), "upload edges");
+        if (!rc) rc = cuda_check(cudaMemcpyAsync(ctx->edge_prm + ctx->n_edges, ep.data(), (size_t)add_edges * sizeof(float2),
+                                                 cudaMemcpyHostToDevice, ctx->stream), "upload edge parameters");
+    }
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    if (rc) return rc;
+    if (out_first_mesh_id) *out_first_mesh_id = (int)ctx->mesh_node_off.size() - 1;
+    for (int s = 0; s < n_meshes; ++s) {
+        ctx->n_nodes += n_nodes;
+        ctx->n_edges += n_edges;
+        ctx->mesh_node_off.push_back(ctx->n_nodes);
+        ctx->mesh_edge_off.push_back(ctx->n_edges);
+    }
+    ctx->forces_valid = false;
+    ctx->spread_current = false;
+    return PLB_OK;
+}
+
+int ib_add_mesh(plb_ctx* ctx, int n_nodes, const double* h_xyz, int n_edges, const int* h_edges, const float* h_rest,
+                float k, int* out_mesh_id) {
+    return ib_add_meshes(ctx, 1, n_nodes, h_xyz, n_edges, h_edges, h_rest, k, out_mesh_id);
+}
+
+int ib_compute_membrane_forces(plb_ctx* ctx, float noise_sigma, unsigned long long noise_seed, unsigned long long step) {
+    REQUIRE_CTX(ctx);
+    if (noise_sigma < 0.f) {
+        set_error("noise_sigma must be >= 0");
+        return PLB_ERR_ARG;
+    }
+    ctx->forces_valid = true;
+    return launch_membrane_forces(ctx, noise_sigma, noise_seed, step);
+}
+
+int ib_spread(plb_ctx* ctx, float* d_forcing) {
+    REQUIRE_CTX(ctx);
+    if (!d_forcing || ((uintptr_t)d_forcing & 15) != 0) {
+        set_error("ib_spread: forcing buffer must be non-null and 16-byte aligned");
+        return PLB_ERR_ARG;
+    }
+    if (ctx->n_nodes && !ctx->forces_valid) {
+        set_error("ib_spread before ib_compute_membrane_forces");
+        return PLB_ERR_ORDER;
+    }
+    // clear what the previous spread wrote (into whichever buffer it used) and drop its segment list
+    if (ctx->spread_target) {
+        const int rc = launch_clear_spread(ctx, ctx->spread_target);
+        if (rc) return rc;
+    }
+    ctx->spread_target = (float4*)d_forcing;
+    ctx->spread_current = true;
+    return launch_spread(ctx, (float4*)d_forcing);
+}
+
+int ib_interpolate_advance(plb_ctx* ctx) {
+    REQUIRE_CTX(ctx);
+    if (ctx->n_nodes == 0) return PLB_OK;
+    if (!ctx->populated || !ctx->spread_current) {
+        set_error("ib_interpolate_advance must follow ib_spread (and lbm_step) for the current node positions");
+        return PLB_ERR_ORDER;
+    }
+    int rc = launch_sparse_moments(ctx);
+    if (rc) return rc;
+    rc = launch_interpolate_advance(ctx);
+    ctx->spread_current = false;
+    ctx->forces_valid = false;
+    return rc;
+}
+
+// ------------------------------------------------------------------------------------------------
+int ib_n_nodes(plb_ctx* ctx, long* out) {
+    REQUIRE_CTX(ctx);
+    if (!out) return PLB_ERR_ARG;
+    *out = ctx->n_nodes;
+    return PLB_OK;
+}
+
+int ib_read_nodes(plb_ctx* ctx, double* h_xyz) {
+    REQUIRE_CTX(ctx);
+    if (!h_xyz) return PLB_ERR_ARG;
+    const long n = ctx->n_nodes;
+    std::vector<double> soa((size_t)3 * n);
+    int rc = PLB_OK;
+    for (int d = 0; d < 3 && !rc; ++d)
+        rc = cuda_check(cudaMemcpyAsync(soa.data() + (size_t)d * n, ctx->X[d], (size_t)n * sizeof(double),
+                                        cudaMemcpyDeviceToHost, ctx->stream), "download node positions");
+    if (rc) return rc;
+    rc = sync_status(ctx);
+    for (long m = 0; m < n; ++m)
+        for (int d = 0; d < 3; ++d) h_xyz[3 * m + d] = soa[(size_t)d * n + m];
+    return rc;
+}
+
+int ib_write_nodes(plb_ctx* ctx, const double* h_xyz) {
+    REQUIRE_CTX(ctx);
+    if (!h_xyz) return PLB_ERR_ARG;
+    const long n = ctx->n_nodes;
+    std::vector<double> soa((size_t)3 * n);
+    for (long m = 0; m < n; ++m)
+        for (int d = 0; d < 3; ++d) soa[(size_t)d * n + m] = h_xyz[3 * m + d];
+    int rc = PLB_OK;
+    for (int d = 0; d < 3 && !rc; ++d)
+        rc = cuda_check(cudaMemcpyAsync(ctx->X[d], soa.data() + (size_t)d * n, (size_t)n * sizeof(double),
+                                        cudaMemcpyHostToDevice, ctx->stream), "upload node positions");
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    ctx->forces_valid = false;
+    ctx->spread_current = false;
+    return rc;
+}
+
+static int read_node_float4(plb_ctx* ctx, const float4* d_src, float* h_out) {
+    const long n = ctx->n_nodes;
+    std::vector<float4> tmp((size_t)n);
+    int rc = cuda_check(cudaMemcpyAsync(tmp.data(), d_src, (size_t)n * sizeof(float4), cudaMemcpyDeviceToHost, ctx->stream),
+                        "download node data");
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    if (rc) return rc;
+    for (long m = 0; m < n; ++m) {
+        h_out[3 * m] = tmp[m].x; h_out[3 * m + 1] = tmp[m].y; h_out[3 * m + 2] = tmp[m].z;
+    }
+    return PLB_OK;
+}
+
+int ib_read_forces(plb_ctx* ctx, float* h_F) {
+    REQUIRE_CTX(ctx);
+    if (!h_F) return PLB_ERR_ARG;
+    return read_node_float4(ctx, ctx->F, h_F);
+}
+
+int ib_read_node_velocities(plb_ctx* ctx, float* h_U) {
+    REQUIRE_CTX(ctx);
+    if (!h_U) return PLB_ERR_ARG;
+    return read_node_float4(ctx, ctx->U, h_U);
+}
+
+int ib_write_forces(plb_ctx* ctx, const float* h_F) {
+    REQUIRE_CTX(ctx);
+    if (!h_F) return PLB_ERR_ARG;
+    const long n = ctx->n_nodes;
+    std::vector<float4> tmp((size_t)n);
+    for (long m = 0; m < n; ++m) tmp[m] = make_float4(h_F[3 * m], h_F[3 * m + 1], h_F[3 * m + 2], 0.f);
+    int rc = cuda_check(cudaMemcpyAsync(ctx->F, tmp.data(), (size_t)n * sizeof(float4), cudaMemcpyHostToDevice, ctx->stream),
+                        "upload forces");
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    ctx->forces_valid = true;
+    return rc;
+}
+
+int plb_status(plb_ctx* ctx) {
+    REQUIRE_CTX(ctx);
+    return sync_status(ctx);
+}
+
+int plb_launch_count(plb_ctx* ctx, long* out) {
+    REQUIRE_CTX(ctx);
+    if (!out) return PLB_ERR_ARG;
+    *out = ctx->launches;
+    return PLB_OK;
+}
+
+int plb_philox4x32_10(void* cuda_stream, long n, const unsigned* d_ctr, const unsigned* d_key, unsigned* d_out) {
+    if (n < 0 || (n > 0 && (!d_ctr || !d_key || !d_out))) {
+        set_error("plb_philox4x32_10: invalid argument");
+        return PLB_ERR_ARG;
+    }
+    return launch_philox((cudaStream_t)cuda_stream, n, d_ctr, d_key, d_out);
+}
+
+}  // extern "C"

@@ -1,0 +1,129 @@
+// plb_internal.cuh -- device helpers and host context shared by the libplb translation units.
+// (Nothing here is shared with oracle/: the CPU oracle is an independent implementation.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <vector>
+#include "../../include/plb.h"
+
+namespace plb {
+
+constexpr int Q = 19;
+constexpr int SEG = 32;        // cells per activity segment = one warp of the LBM kernel
+constexpr int SEG_SHIFT = 5;
+
+// D3Q19 velocity set in the paper's numbering (Eq. 21, Eq. 23-30; index = paper's i - 1).
+__host__ __device__ constexpr int CX(int d) {
+    constexpr int t[Q] = {1, -1, 0, 0, 0, 0, 1, 1, 1, 1, -1, -1, -1, -1, 0, 0, 0, 0, 0};
+    return t[d];
+}
+__host__ __device__ constexpr int CY(int d) {
+    constexpr int t[Q] = {0, 0, 1, -1, 0, 0, 1, -1, 0, 0, 1, -1, 0, 0, 1, 1, -1, -1, 0};
+    return t[d];
+}
+__host__ __device__ constexpr int CZ(int d) {
+    constexpr int t[Q] = {0, 0, 0, 0, 1, -1, 0, 0, 1, -1, 0, 0, 1, -1, 1, -1, 1, -1, 0};
+    return t[d];
+}
+__host__ __device__ constexpr int OPP(int d) {
+    constexpr int t[Q] = {1, 0, 3, 2, 5, 4, 11, 10, 13, 12, 7, 6, 9, 8, 17, 16, 15, 14, 18};
+    return t[d];
+}
+__host__ __device__ constexpr float WGT(int d) {
+    return d < 6 ? (1.0f / 18.0f) : (d < 18 ? (1.0f / 36.0f) : (1.0f / 3.0f));
+}
+
+struct LbmParams {
+    int nx, ny, nz;
+    int cells;                 // nx*ny*nz < 2^31
+    int wall[3];               // 1 = bounce-back on this axis
+    float omega;               // 1/tau
+    float pref;                // 1 - 1/(2 tau)
+    float corr[3][2][Q];       // [axis][0 = low face, 1 = high face][d] = 6 w_d (c_d . u_wall)
+};
+
+enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
+
+// status bits raised by kernels (sticky)
+enum { STATUS_NODE_LEFT = 1, STATUS_ZERO_EDGE = 2 };
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), written from the paper's description.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c.x), lo0 = M0 * c.x;
+        const uint32_t hi1 = __umulhi(M1, c.z), lo1 = M1 * c.z;
+        c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+        k.x += W0;
+        k.y += W1;
+    }
+    return c;
+}
+// xi = ((r >> 8) + 1/2) 2^-24, exact in fp32, never 0 or 1
+__device__ __forceinline__ float uniform01(uint32_t r) {
+    return ((float)(r >> 8) + 0.5f) * (1.0f / 16777216.0f);
+}
+__device__ __forceinline__ uint4 noise_words(unsigned long long seed, unsigned long long index,
+                                             uint32_t step, uint32_t tag) {
+    return philox4x32_10(make_uint4((uint32_t)index, (uint32_t)(index >> 32), step, tag),
+                         make_uint2((uint32_t)seed, (uint32_t)(seed >> 32)));
+}
+
+// ---------------------------------------------------------------------------------------------
+// host context
+// ---------------------------------------------------------------------------------------------
+struct Ctx {
+    plb_grid grid;
+    float tau;
+    plb_boundary bnd;
+    LbmParams prm;
+    cudaStream_t stream;
+    long n_segs;
+    // lattice (carved from the workspace)
+    float* f[2];
+    int cur;
+    float4* vel;               // (vx, vy, vz, rho) at the active cells, cells entries
+    int* seg_flag;             // n_segs
+    int* seg_list;             // n_segs
+    int* counters;             // [0] active segment count, [1] status bits
+    // meshes
+    long cap_nodes, cap_edges, n_nodes, n_edges;
+    double* X[3];              // SoA fp64 unwrapped positions
+    float4* F;                 // nodal forces (Fx, Fy, Fz, 0)
+    float4* U;                 // nodal velocities of the last interpolate
+    int2* edges;               // global node index pairs
+    float2* edge_prm;          // (rest length, k)
+    std::vector<long> mesh_node_off, mesh_edge_off;
+    // bookkeeping
+    const float4* g_last;
+    int g_last_mode;           // ForceMode used by the last lbm_step
+    float4* spread_target;     // buffer ib_spread last filled (its touched cells are listed in seg_list)
+    bool spread_current;       // seg_list matches the current node positions
+    bool forces_valid;
+    bool populated;
+    long launches;
+    int sm_count;
+};
+
+void set_error(const char* fmt, ...);
+int cuda_check(cudaError_t e, const char* what);
+
+// kernels launchers (lbm.cu / ib.cu); all asynchronous on c->stream, return a PLB_* code
+int launch_set_equilibrium(Ctx* c, const float* d_rho, const float* d_u, float amp, unsigned long long seed);
+int launch_lbm_step(Ctx* c, const float4* g, int mode);
+int launch_read_macros(Ctx* c, float* d_rho, float* d_u);
+int launch_read_populations(Ctx* c, float* d_f);
+int launch_write_populations(Ctx* c, const float* d_f);
+int launch_sparse_moments(Ctx* c);
+int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigned long long step);
+int launch_clear_spread(Ctx* c, float4* g);
+int launch_spread(Ctx* c, float4* g);
+int launch_interpolate_advance(Ctx* c);
+int launch_philox(cudaStream_t s, long n, const unsigned* ctr, const unsigned* key, unsigned* out);
+
+}  // namespace plb
+
+struct plb_ctx : plb::Ctx {};
