@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the coupled LBM + immersed-boundary hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: ib_compute_membrane_forces ->
+ib_spread -> lbm_step(forcing) -> ib_interpolate_advance, through the C-ABI of libplb.  The
+default workload is BASELINE.json's config 4 (512 x 128 x 1024 shear channel, 1024 platelets,
+657,408 nodes): the coupled configuration the north_star's targets are stated on; it fits one
+GPU (10.2 GB of lattice).  Prints ONE JSON line (rank 0).
+
+Multi-GPU (--gpus N under torchrun): the path has no exchange step in this build ("replicas
+only"): every rank runs the same workload on its own GPU, no data-path collective;
+value = units all ranks processed / max-over-ranks time ("scaling": "weak").
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
+sample of the same workload; it is a deliberately plain program, a reported baseline only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "coupled LBM+IB MLUPS (fp32 D3Q19)"
+UNIT = "MLUPS"
+BYTES_PER_CELL = 2 * 19 * 4          # algorithmic bytes of S3 per cell per step
+FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+NOMINAL_HBM_GBS = 8000.0
+
+
+def parse_args(argv=None):
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=50)
+    p.add_argument("--warmup", type=int, default=5)
+    p.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    p.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    p.add_argument("--dist-dry-run", action="store_true",
+                   help="CPU test of the N>1 plumbing (gloo): fake per-rank times, real barrier/max/aggregation")
+    return p.parse_args(argv)
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+# ---------------------------------------------------------------------------------------------
+# workload naming / sampling
+# ---------------------------------------------------------------------------------------------
+def describe(w):
+    s = "C%s %dx%dx%d" % (w.name[1:], w.nx, w.ny, w.nz)
+    if w.n_meshes:
+        s += ", %d platelets (%d nodes, %d edges)" % (w.n_meshes, w.n_nodes, w.n_edges)
+    else:
+        s += ", no immersed boundary"
+    return s
+
+
+def cpu_sample(config):
+    """Bounded sample of the bench workload for the oracle legs: the same recipe (tau, wall speed,
+    mesh shape, platelet number density, channel height) on a smaller footprint."""
+    from paper_1312_2234_b200 import workloads as wl
+    if config == 4:
+        return wl.config4(nx=128, ny=128, nz=128, n_meshes=32), "C4 recipe on a 128x128x128 footprint, 32 platelets (same number density and channel height)"
+    if config == 3:
+        return wl.config3(nx=128, ny=64, nz=128, n_meshes=4), "C3 recipe on a 128x64x128 footprint, 4 platelets"
+    if config == 5:
+        return wl.config5(n=256, grid_xz=8, layers=2, subdiv=4), "C5 recipe with 128 of the 8192 platelets"
+    if config == 2:
+        return wl.config2(n=128), "C2 recipe at 128^3"
+    return wl.config1(), "C1 whole"
+
+
+def aggregate(cells_per_rank, steps, world, max_seconds):
+    """whole-job MLUPS: the cell updates of all ranks over the slowest rank's time"""
+    return cells_per_rank * steps * world / max_seconds / 1e6
+
+
+def max_over_ranks(x, device):
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(x)
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def barrier(device):
+    import torch
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        if device.type == "cuda":
+            dist.barrier(device_ids=[device.index])
+        else:
+            dist.barrier()
+    if device.type == "cuda":
+        torch.cuda.synchronize(device)
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md)
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            text, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            text, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in text.splitlines():
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json, copy bandwidth)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(config):
+    """DRAM bytes per launch of the LBM kernel (dram__bytes_read.sum + dram__bytes_write.sum of one
+    ncu --set full capture), from the committed summary profiles/lbm_dram_traffic.txt, or None.
+    Line format:  C<config> <bytes per launch>  # which capture"""
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "lbm_dram_traffic.txt")):
+            parts = line.split("#")[0].split()
+            if len(parts) >= 2 and parts[0] == "C%d" % config:
+                return float(parts[1])
+    except Exception:
+        pass
+    return None
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle legs (host cores)
+# ---------------------------------------------------------------------------------------------
+def time_oracle(config, steps, warmup):
+    """The CPU oracle as it stands, on all host cores, on a bounded sample of the workload."""
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    os.environ.setdefault("OMP_NUM_THREADS", str(cores))
+    threads = int(os.environ["OMP_NUM_THREADS"])
+    from oracle import orc
+    w, what = cpu_sample(config)
+    ora = orc.Oracle.from_workload(w)
+    for s in range(warmup):
+        ora.coupled_step(w.force_sigma, w.force_seed, s)
+    t0 = time.perf_counter()
+    for s in range(warmup, warmup + steps):
+        ora.coupled_step(w.force_sigma, w.force_seed, s)
+    dt = time.perf_counter() - t0
+    ora.close()
+    return {"value": w.cells * steps / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%s; %d coupled steps (%d cells, %d nodes) in %.2f s" % (what, steps, w.cells, w.n_nodes, dt)}, dt, w
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    from paper_1312_2234_b200 import workloads as wl
+    full = wl.CONFIGS[args.config].__doc__ or ""
+    cb, dt, w = time_oracle(args.config, args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "C%d" % args.config, "sample": cb["sample"]},
+        "cpu_baseline": cb,
+        "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_dist_dry(args):
+    """CPU-only check of the N>1 plumbing with gloo: each rank pretends its timed region took
+    (rank + 1) * 10 ms; barrier, max-over-ranks and aggregation are the real code."""
+    import torch
+    import torch.distributed as dist
+    rank, world, _ = dist_env()
+    if world > 1:
+        dist.init_process_group("gloo", init_method="env://")
+    dev = torch.device("cpu")
+    barrier(dev)
+    fake = 0.010 * (rank + 1)
+    tmax = max_over_ranks(fake, dev)
+    barrier(dev)
+    if rank == 0:
+        cells = 1000
+        print(json.dumps({"metric": METRIC, "value": aggregate(cells, args.steps, world, tmax), "unit": UNIT,
+                          "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": 1e3 * tmax / args.steps, "scaling": "weak", "dry_run": True}))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1312_2234_b200 import binding as plb
+    from paper_1312_2234_b200 import build as plb_build
+    from paper_1312_2234_b200 import workloads as wl
+
+    rank, world, local_rank = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libplb has no CPU fallback")
+    if rank == 0 or world == 1:
+        plb_build.build()
+    device = torch.device("cuda", local_rank if world > 1 else 0)
+    torch.cuda.set_device(device)
+    if world > 1:
+        dist.init_process_group("nccl", init_method="env://", device_id=device)
+    barrier(device)
+
+    w = wl.config(args.config)
+    sim = plb.Simulation.from_workload(w, device=str(device))
+    coupled = w.n_meshes > 0
+    K, W = args.steps, args.warmup
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def one_step(s, marks=None):
+        if coupled:
+            if marks is not None: marks[0].record()
+            plb.ib_compute_membrane_forces(sim.h, w.force_sigma, w.force_seed, s)
+            if marks is not None: marks[1].record()
+            plb.ib_spread(sim.h, sim.forcing)
+            if marks is not None: marks[2].record()
+            plb.lbm_step(sim.h, sim.forcing)
+            if marks is not None: marks[3].record()
+            plb.ib_interpolate_advance(sim.h)
+            if marks is not None: marks[4].record()
+        else:
+            if marks is not None: marks[2].record()
+            plb.lbm_step(sim.h, None)
+            if marks is not None: marks[3].record()
+
+    # ---- device-resident leg: inputs already in HBM, CUDA events on the launching stream
+    for s in range(W):
+        one_step(s)
+    marks = [[ev() for _ in range(5)] for _ in range(K)]
+    t_beg, t_end = ev(), ev()
+    barrier(device)
+    launches0 = sim.launch_count()
+    clocks = ClockSampler(device.index)
+    t_beg.record()
+    for s in range(K):
+        one_step(W + s, marks[s])
+    t_end.record()
+    barrier(device)
+    clk = clocks.stop()
+    launches = sim.launch_count() - launches0
+    sim.status()
+    seconds = max_over_ranks(t_beg.elapsed_time(t_end) * 1e-3, device)
+    value = aggregate(w.cells, K, world, seconds)
+    lbm_ms = sum(m[2].elapsed_time(m[3]) for m in marks) / K
+    split = {"lbm_step": lbm_ms}
+    if coupled:
+        split.update(ib_compute_membrane_forces=sum(m[0].elapsed_time(m[1]) for m in marks) / K,
+                     ib_spread=sum(m[1].elapsed_time(m[2]) for m in marks) / K,
+                     ib_interpolate_advance=sum(m[3].elapsed_time(m[4]) for m in marks) / K)
+    step_ms = 1e3 * t_beg.elapsed_time(t_end) * 1e-3 / K
+    ib_share = (sum(split.values()) - lbm_ms) / sum(split.values())
+
+    # ---- end-to-end leg: the membrane state crosses the C-ABI as HOST buffers every step
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(sim, w, K, W, world, device, plb, one_step)
+
+    # ---- roofline of the dominant kernel (lbm_step_kernel: 152 B per cell per launch)
+    peak, peak_src = hbm_peak()
+    achieved = BYTES_PER_CELL * w.cells / (lbm_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "lbm_step_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": ncu_traffic(args.config), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": BYTES_PER_CELL * w.cells, "avg_launch_ms": lbm_ms,
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "lbm_only_mlups": w.cells / (lbm_ms * 1e-3) / 1e6}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": 1e3 * seconds / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": describe(w), "cells": w.cells, "nodes": w.n_nodes, "tau": w.tau,
+                   "l2": "inputs exceed L2 (%.2f GB of populations per step)" % (BYTES_PER_CELL * w.cells / 1e9),
+                   "multi_gpu": "replicas only (no exchange step in this build)", "notes": w.notes},
+        "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+        "coupled_steps_per_s": K * world / seconds, "split_ms": split, "ib_share": ib_share,
+        "step_ms_rank0": step_ms,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cb, _, _ = time_oracle(args.config, 10, 1)
+        line["cpu_baseline"] = cb
+    elif rank == 0:
+        line["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_e2e(sim, w, K, W, world, device, plb, one_step):
+    """Same metric through the C-ABI with HOST buffers: every step the node positions go in from
+    pinned host memory (ib_write_nodes) and come back out (ib_read_nodes), copies inside the timed
+    region.  Without meshes (C2) the step's result read back is the density field."""
+    import numpy as np
+    import torch
+    coupled = w.n_meshes > 0
+    if coupled:
+        n = sim.n_nodes
+        pinned = torch.empty((n, 3), dtype=torch.float64).pin_memory()
+        X = pinned.numpy()
+        plb.ib_read_nodes(sim.h, X)
+        h2d = d2h = n * 24
+    else:
+        pinned = torch.empty(w.cells, dtype=torch.float32).pin_memory()
+        rho = torch.empty(w.cells, dtype=torch.float32, device=device)
+        h2d, d2h = 0, w.cells * 4
+
+    def e2e_step(s):
+        if coupled:
+            plb.ib_write_nodes(sim.h, X)
+            one_step(s)
+            plb.ib_read_nodes(sim.h, X)
+        else:
+            one_step(s)
+            plb.lbm_read_macros(sim.h, rho, None)
+            pinned.copy_(rho, non_blocking=False)
+
+    for s in range(3):
+        e2e_step(s)
+    barrier(device)
+    t0 = time.perf_counter()
+    for s in range(K):
+        e2e_step(s)
+    barrier(device)
+    dt = max_over_ranks(time.perf_counter() - t0, device)
+    return {"value": aggregate(w.cells, K, world, dt), "unit": UNIT, "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * dt / K,
+            "what": "ib_write_nodes(pinned host) -> 4 coupled calls -> ib_read_nodes(pinned host), per step"
+                    if coupled else "lbm_step -> lbm_read_macros -> density field to pinned host, per step"}
+
+
+def main(argv=None):
+    args = parse_args(argv)
+    if args.dist_dry_run:
+        return run_dist_dry(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -50,12 +50,13 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     double* X2 = w.take<double>((size_t)max_nodes);
     float4* F = w.take<float4>((size_t)max_nodes);
     float4* U = w.take<float4>((size_t)max_nodes);
+    double* stage = w.take<double>((size_t)3 * max_nodes);
     int2* edges = w.take<int2>((size_t)max_edges);
     float2* eprm = w.take<float2>((size_t)max_edges);
     if (c) {
         c->f[0] = f0; c->f[1] = f1; c->vel = vel;
         c->seg_flag = seg_flag; c->seg_list = seg_list; c->counters = counters;
-        c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U;
+        c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
         c->edges = edges; c->edge_prm = eprm;
     }
     return w.off;
@@ -399,29 +400,27 @@ int ib_read_nodes(plb_ctx* ctx, double* h_xyz) {
     REQUIRE_CTX(ctx);
     if (!h_xyz) return PLB_ERR_ARG;
     const long n = ctx->n_nodes;
-    std::vector<double> soa((size_t)3 * n);
-    int rc = PLB_OK;
-    for (int d = 0; d < 3 && !rc; ++d)
-        rc = cuda_check(cudaMemcpyAsync(soa.data() + (size_t)d * n, ctx->X[d], (size_t)n * sizeof(double),
-                                        cudaMemcpyDeviceToHost, ctx->stream), "download node positions");
-    if (rc) return rc;
-    rc = sync_status(ctx);
-    for (long m = 0; m < n; ++m)
-        for (int d = 0; d < 3; ++d) h_xyz[3 * m + d] = soa[(size_t)d * n + m];
-    return rc;
+    if (n) {
+        // SoA -> AoS on the device, then one copy straight into the caller's buffer
+        int rc = launch_nodes_transpose(ctx, /*to_aos=*/true);
+        if (rc) return rc;
+        rc = cuda_check(cudaMemcpyAsync(h_xyz, ctx->stage, (size_t)3 * n * sizeof(double), cudaMemcpyDeviceToHost,
+                                        ctx->stream), "download node positions");
+        if (rc) return rc;
+    }
+    return sync_status(ctx);
 }
 
 int ib_write_nodes(plb_ctx* ctx, const double* h_xyz) {
     REQUIRE_CTX(ctx);
     if (!h_xyz) return PLB_ERR_ARG;
     const long n = ctx->n_nodes;
-    std::vector<double> soa((size_t)3 * n);
-    for (long m = 0; m < n; ++m)
-        for (int d = 0; d < 3; ++d) soa[(size_t)d * n + m] = h_xyz[3 * m + d];
     int rc = PLB_OK;
-    for (int d = 0; d < 3 && !rc; ++d)
-        rc = cuda_check(cudaMemcpyAsync(ctx->X[d], soa.data() + (size_t)d * n, (size_t)n * sizeof(double),
-                                        cudaMemcpyHostToDevice, ctx->stream), "upload node positions");
+    if (n) {
+        rc = cuda_check(cudaMemcpyAsync(ctx->stage, h_xyz, (size_t)3 * n * sizeof(double), cudaMemcpyHostToDevice,
+                                        ctx->stream), "upload node positions");
+        if (!rc) rc = launch_nodes_transpose(ctx, /*to_aos=*/false);
+    }
     if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
     ctx->forces_valid = false;
     ctx->spread_current = false;

@@ -176,6 +176,19 @@ __global__ void __launch_bounds__(256) interpolate_advance_kernel(double* __rest
     }
 }
 
+// positions: device SoA <-> AoS staging buffer (so host transfers are one contiguous copy)
+__global__ void __launch_bounds__(256) nodes_transpose_kernel(double* __restrict__ X, double* __restrict__ Y,
+                                                              double* __restrict__ Z, double* __restrict__ aos,
+                                                              const long n, const bool to_aos) {
+    const long t = blockIdx.x * 256L + threadIdx.x;
+    if (t >= 3 * n) return;
+    const long m = t / 3;
+    const int d = (int)(t - 3 * m);
+    double* comp = d == 0 ? X : (d == 1 ? Y : Z);
+    if (to_aos) aos[t] = comp[m];
+    else        comp[m] = aos[t];
+}
+
 __global__ void philox_kernel(const long n, const uint4* __restrict__ ctr, const uint2* __restrict__ key,
                               uint4* __restrict__ out) {
     const long t = blockIdx.x * (long)blockDim.x + threadIdx.x;
@@ -222,6 +235,14 @@ int launch_interpolate_advance(Ctx* c) {
         c->X[0], c->X[1], c->X[2], c->U, c->n_nodes, c->vel, c->counters, c->prm);
     c->launches++;
     return cuda_check(cudaGetLastError(), "interpolate_advance_kernel");
+}
+
+int launch_nodes_transpose(Ctx* c, bool to_aos) {
+    if (c->n_nodes == 0) return PLB_OK;
+    nodes_transpose_kernel<<<(unsigned)((3 * c->n_nodes + 255) / 256), 256, 0, c->stream>>>(
+        c->X[0], c->X[1], c->X[2], c->stage, c->n_nodes, to_aos);
+    c->launches++;
+    return cuda_check(cudaGetLastError(), "nodes_transpose_kernel");
 }
 
 int launch_philox(cudaStream_t s, long n, const unsigned* ctr, const unsigned* key, unsigned* out) {

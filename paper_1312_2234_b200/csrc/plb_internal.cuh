@@ -94,6 +94,7 @@ struct Ctx {
     double* X[3];              // SoA fp64 unwrapped positions
     float4* F;                 // nodal forces (Fx, Fy, Fz, 0)
     float4* U;                 // nodal velocities of the last interpolate
+    double* stage;             // 3 * cap_nodes: AoS staging for ib_read_nodes / ib_write_nodes
     int2* edges;               // global node index pairs
     float2* edge_prm;          // (rest length, k)
     std::vector<long> mesh_node_off, mesh_edge_off;
@@ -122,6 +123,7 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
 int launch_clear_spread(Ctx* c, float4* g);
 int launch_spread(Ctx* c, float4* g);
 int launch_interpolate_advance(Ctx* c);
+int launch_nodes_transpose(Ctx* c, bool to_aos);
 int launch_philox(cudaStream_t s, long n, const unsigned* ctr, const unsigned* key, unsigned* out);
 
 }  // namespace plb

@@ -61,94 +61,89 @@ def compare(w, sim, ora, check=True):
     return out
 
 
+
+
 # ---------------------------------------------------------------------------------------------
-# Block parity at FULL size: one coupled step of a sub-block of the lattice is recomputed by the
-# oracle from the GPU's own pre-step state and compared on the block interior.  One LBM step only
-# couples nearest neighbours and a node only touches floor(X)-1 .. floor(X)+2, so with a halo of
-# H >= 4 cells on the periodic axes the interior of the block is exact; wall axes are taken whole.
+# Block parity at FULL size, from the SEEDED INPUTS ONLY (nothing the oracle consumes comes from
+# the CUDA path): the oracle runs the first `steps` coupled steps on a sub-block of the workload
+# cut out of the generator's own initial state, and the result is compared on the block's inner
+# region.  Why the inner region is exact: one LBM step couples nearest neighbours, a node touches
+# cells floor(X)-1 .. floor(X)+2 and moves < 0.1 per step, so after `steps` steps a cell only
+# knows about cells / nodes within 3*steps of it.  The block is the inner region plus a halo of
+# 3*steps + mesh diameter + 1 on the periodic axes (wall axes are taken whole); every mesh with a
+# node within 3*steps of the inner region is included whole and lies inside the block, so the
+# block's own periodic wrap never reaches the inner region.
 # ---------------------------------------------------------------------------------------------
-class BlockSpec:
-    def __init__(self, w, origin, width, halo=4):
+class Block:
+    def __init__(self, w, origin, inner, steps, mesh_diameter):
         self.n = (w.nx, w.ny, w.nz)
         self.kind = tuple(w.kind)
+        self.reach = 3 * steps
+        halo = self.reach + int(np.ceil(mesh_diameter)) + 1
         self.lo, self.size, self.inner = [], [], []
         for a in range(3):
-            if self.kind[a] == 1:                       # wall axis: whole extent
+            if self.kind[a] == 1 or inner + 2 * halo >= self.n[a]:      # wall axis / whole periodic axis: exact
                 self.lo.append(0); self.size.append(self.n[a]); self.inner.append((0, self.n[a]))
             else:
-                bw = min(width, self.n[a])
-                if bw == self.n[a]:                     # the block wraps onto itself: exact everywhere
-                    self.lo.append(0); self.size.append(bw); self.inner.append((0, bw))
-                else:
-                    self.lo.append(int(origin[a]) % self.n[a]); self.size.append(bw); self.inner.append((halo, bw - halo))
+                self.lo.append(int(origin[a]) - halo); self.size.append(inner + 2 * halo)
+                self.inner.append((halo, halo + inner))
 
-    def index(self, a, device=None):
+    def whole(self, a):
+        return self.size[a] == self.n[a]
+
+    def local(self, X):
+        """unwrapped positions [..., 3] -> block coordinates; a mesh is shifted as a whole by the
+        periodic image that brings its first node nearest to the block centre"""
+        Y = np.array(X, dtype=np.float64, copy=True)
+        for a in range(3):
+            if not self.whole(a):
+                centre = self.lo[a] + 0.5 * self.size[a]
+                shift = self.n[a] * np.round((Y[..., :1, a] - centre) / self.n[a])
+                Y[..., a] -= shift
+                Y[..., a] -= self.lo[a]
+        return Y
+
+    def cell_index(self, a):
+        return (np.arange(self.lo[a], self.lo[a] + self.size[a]) % self.n[a])
+
+    def take_field(self, t):
+        """t: torch tensor or ndarray [C, cells] of the full grid -> numpy [C, bz, by, bx] float64"""
+        nx, ny, nz = self.n
+        if isinstance(t, np.ndarray):
+            v = t.reshape(t.shape[0], nz, ny, nx)
+            return v[:, self.cell_index(2)][:, :, self.cell_index(1)][:, :, :, self.cell_index(0)].astype(np.float64)
         import torch
-        return (torch.arange(self.lo[a], self.lo[a] + self.size[a], device=device) % self.n[a])
-
-    def take(self, t):
-        """t: device tensor [C, nz, ny, nx] -> numpy [C, bz, by, bx] float64"""
-        ix, iy, iz = (self.index(a, t.device) for a in range(3))
-        return t.index_select(3, ix).index_select(2, iy).index_select(1, iz).cpu().numpy().astype(np.float64)
+        v = t.view(t.shape[0], nz, ny, nx)
+        ix = [torch.as_tensor(self.cell_index(a), device=t.device) for a in range(3)]
+        return v.index_select(1, ix[2]).index_select(2, ix[1]).index_select(3, ix[0]).cpu().numpy().astype(np.float64)
 
     def inner_slices(self):
         (x0, x1), (y0, y1), (z0, z1) = self.inner
         return (slice(None), slice(z0, z1), slice(y0, y1), slice(x0, x1))
 
-    def local_positions(self, X):
-        """Unwrapped positions -> block coordinates (nearest periodic image to the block centre)."""
-        Y = np.array(X, dtype=np.float64, copy=True)
+    def near_inner(self, Xl, margin):
+        """mask over [..., n_nodes] positions (block coordinates) within `margin` of the inner region"""
+        m = np.ones(Xl.shape[:-1], dtype=bool)
         for a in range(3):
-            if self.kind[a] == 0:
-                centre = self.lo[a] + 0.5 * self.size[a]
-                Y[:, a] -= self.n[a] * np.round((Y[:, a] - centre) / self.n[a])
-            Y[:, a] -= self.lo[a]
-        return Y
-
-    def nodes_near(self, Xl, margin=2.5):
-        m = np.ones(Xl.shape[0], dtype=bool)
-        for a in range(3):
-            if self.kind[a] == 0 and self.size[a] < self.n[a]:
-                m &= (Xl[:, a] > -margin) & (Xl[:, a] < self.size[a] + margin)
-        return m
-
-    def nodes_clean(self, Xl):
-        """nodes whose whole 4^3 stencil lies inside the clean interior"""
-        m = np.ones(Xl.shape[0], dtype=bool)
-        for a in range(3):
-            if self.kind[a] == 0 and self.size[a] < self.n[a]:
-                fl = np.floor(Xl[:, a])
-                m &= (fl - 1 >= self.inner[a][0]) & (fl + 2 < self.inner[a][1])
+            if not self.whole(a):
+                m &= (Xl[..., a] >= self.inner[a][0] - margin) & (Xl[..., a] <= self.inner[a][1] - 1 + margin)
         return m
 
 
-def block_oracle_step(w, blk, f_before, g_dev, X_before, F_nodes):
-    """Recompute one coupled step on the block with the oracle.  f_before: [19, bz, by, bx] true
-    populations; returns dict with the oracle's g, f_after, U, X_after (block-local) and masks."""
-    bx, by, bz = blk.size
-    ora = orc.Oracle(bx, by, bz, w.tau, w.kind, w.u_lo, w.u_hi)
-    ora.write_populations(f_before.reshape(19, -1))
-    res = {}
-    if X_before is not None and X_before.shape[0]:
-        Xl = blk.local_positions(X_before)
-        near = blk.nodes_near(Xl)
-        ora.add_mesh(Xl[near], np.zeros((0, 2), dtype=np.int32), None, 0.0)
-        ora.write_forces(F_nodes[near].astype(np.float64))
-        g = ora.spread()
-        ora.step(g)
-        ora.interpolate_advance_safe = None
-        try:
-            ora.interpolate_advance()
-        except orc.OracleError as e:          # nodes outside the block may "leave" its walls; ignored
-            if e.code != -5:
-                raise
-        res.update(g=g.reshape(3, bz, by, bx), near=near, clean=blk.nodes_clean(Xl[near]),
-                   U=ora.read_node_velocities(), X_after=ora.read_nodes(), Xl=Xl[near])
-    else:
-        g = None if g_dev is None else g_dev
-        ora.step(g)
-    res["f_after"] = ora.read_populations().reshape(19, bz, by, bx)
-    rho, u = ora.read_macros()
-    res["rho"] = rho.reshape(1, bz, by, bx)
-    res["u"] = u.reshape(3, bz, by, bx)
-    return res
+def block_workload(w, blk):
+    """Sub-workload of w on the block, built from the generator's outputs alone.  Returns
+    (Workload, mesh_ids): the meshes with a node within blk.reach of the inner region."""
+    import copy
+    wb = copy.copy(w)
+    wb.nx, wb.ny, wb.nz = blk.size
+    wb.u0 = None if w.u0 is None else blk.take_field(w.u0).reshape(3, -1)
+    assert w.noise_amp == 0.0, "population noise is keyed on the global cell index"
+    ids = np.zeros(0, dtype=np.int64)
+    if w.n_meshes:
+        Xl = blk.local(w.mesh_xyz)                                   # [meshes, nodes, 3]
+        ids = np.nonzero(blk.near_inner(Xl, blk.reach).any(axis=1))[0]
+        wb.mesh_xyz = np.ascontiguousarray(Xl[ids]) if len(ids) else None
+        for a in range(3):                                           # included meshes lie inside the block
+            if len(ids) and not blk.whole(a):
+                assert wb.mesh_xyz[..., a].min() >= 1.0 and wb.mesh_xyz[..., a].max() <= blk.size[a] - 2.0
+    return wb, ids

@@ -1,0 +1,228 @@
+"""GPU parity tests of the immersed-boundary / membrane part of libplb against the fp64 CPU
+oracle, through the C-ABI.  Same seeded inputs on both sides; nothing the oracle consumes or is
+compared with comes from the CUDA path.
+
+Tolerances: node positions within 1e-4 lattice units, |dv| <= 1e-4 u_ref, |drho| <= 1e-6 at the
+end of a run (BASELINE.json north_star); single calls to fp32 round-off of the quantities
+involved (stated at each assert)."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import orc                                    # noqa: E402
+from paper_1312_2234_b200 import binding as plb            # noqa: E402
+from paper_1312_2234_b200 import workloads as wl           # noqa: E402
+import parity_utils as pu                                  # noqa: E402
+
+FULL = os.environ.get("PLB_FULL", "0") == "1"
+DEV = "cuda:0"
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def dev(a, dtype=torch.float32):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(DEV).contiguous()
+
+
+# ------------------------------------------------------------------ O-8 Philox
+def test_philox_known_answers_on_device():
+    rows = [l.split() for l in open(os.path.join(GOLD, "philox4x32_10_kat.txt")) if l.strip() and l[0] != "#"]
+    ctr = np.array([[int(x, 16) for x in r[0:4]] for r in rows], dtype=np.uint32)
+    key = np.array([[int(x, 16) for x in r[4:6]] for r in rows], dtype=np.uint32)
+    exp = np.array([[int(x, 16) for x in r[6:10]] for r in rows], dtype=np.uint32)
+    d_ctr = torch.as_tensor(ctr.view(np.int32)).to(DEV)
+    d_key = torch.as_tensor(key.view(np.int32)).to(DEV)
+    d_out = torch.zeros_like(d_ctr)
+    plb.plb_philox4x32_10(d_ctr, d_key, d_out)
+    torch.cuda.synchronize()
+    assert (d_out.cpu().numpy().view(np.uint32) == exp).all()
+
+
+def test_philox_equals_oracle_on_many_counters():
+    rng = np.random.default_rng(41)
+    n = 100_000
+    ctr = rng.integers(0, 2 ** 32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    d_ctr = torch.as_tensor(ctr.view(np.int32)).to(DEV)
+    d_key = torch.as_tensor(key.view(np.int32)).to(DEV)
+    d_out = torch.zeros_like(d_ctr)
+    plb.plb_philox4x32_10(d_ctr, d_key, d_out)
+    out = d_out.cpu().numpy().view(np.uint32)
+    for t in rng.integers(0, n, size=2000):
+        assert out[t].tolist() == orc.philox4x32_10(ctr[t], key[t])
+
+
+# ------------------------------------------------------------------ helpers
+def mesh_pair(n, kind, xyz, edges, rest, k, tau=0.8, u_hi=None):
+    sim = plb.Simulation(*n, tau, kind, None, u_hi, max_nodes=xyz.shape[0], max_edges=max(1, edges.shape[0]))
+    ora = orc.Oracle(*n, tau, kind, None, u_hi)
+    sim.add_mesh(xyz, edges, rest, k)
+    ora.add_mesh(xyz, edges, rest, k)
+    return sim, ora
+
+
+def scattered_nodes(n, kind, count, seed):
+    """Seeded node cloud exercising every stencil case: periodic seams, unwrapped coordinates far
+    outside the box, exact integers, stencils that cross a wall (dropped cells, G15)."""
+    rng = np.random.default_rng(seed)
+    X = rng.random((count, 3)) * np.asarray(n, dtype=np.float64)
+    X[0] = (0.2, 3.3, n[2] - 0.1)
+    X[1] = (4.0, 5.0, 2.0)
+    X[2] = (n[0] - 0.01, 4.5, 0.01)
+    for a in range(3):
+        if kind[a] == 0:
+            X[3, a] += 3 * n[a]                # unwrapped, several boxes away
+            X[4, a] -= 2 * n[a]
+        else:
+            X[5, a] = 0.3                      # low wall: two layers of the stencil dropped
+            X[6, a] = n[a] - 1.2               # high wall
+            X[7, a] = -0.4
+            X[8, a] = n[a] - 0.6
+    return X
+
+
+# ------------------------------------------------------------------ O-5 membrane forces
+@pytest.mark.parametrize("sigma", [0.0, 1e-4])
+def test_membrane_forces_match_oracle(sigma):
+    w = wl.config1()
+    xyz = np.concatenate([w.mesh_xyz[0], w.mesh_xyz[0] + (300.0, 0.0, 700.0)])   # a far copy: large coordinates
+    e = np.concatenate([w.edges, w.edges + w.mesh_xyz.shape[1]])
+    rest = np.concatenate([w.rest, w.rest])
+    sim, ora = mesh_pair((32, 32, 64), w.kind, xyz, e, rest, w.k_spring)
+    sim.compute_membrane_forces(sigma, 99, 17)
+    ora.compute_membrane_forces(sigma, 99, 17)
+    F_g, F_o = sim.read_forces().astype(np.float64), ora.read_forces()
+    scale = np.abs(F_o).max()
+    assert scale > 1e-4
+    # sums of <= 6 edge terms of size <= scale, each formed with ~4 fp32 roundings
+    assert np.abs(F_g - F_o).max() <= 2e-6 * scale
+    if sigma == 0.0:
+        assert np.abs(F_g.sum(0)).max() <= 1e-7          # P14: springs sum to zero
+
+
+def test_membrane_force_default_rest_lengths_and_zero_edge():
+    rng = np.random.default_rng(43)
+    X = rng.random((12, 3)) * 4 + 8
+    e = np.array([(a, b) for a in range(12) for b in range(a + 1, 12)][:30], dtype=np.int32)
+    sim, ora = mesh_pair((24, 24, 24), (0, 0, 0), X, e, None, 0.05)
+    sim.compute_membrane_forces()
+    # rest = initial lengths => F = 0 up to the fp32 rounding of the stored rest length (k ulp(L))
+    assert np.abs(sim.read_forces()).max() <= 0.05 * 11 * 6e-8 * 7
+    Y = X.copy(); Y[1] = Y[0]                             # collapse an edge: |R| = 0 is an error
+    sim.write_nodes(Y)
+    sim.compute_membrane_forces()
+    with pytest.raises(plb.PlbError) as err:
+        sim.status()
+    assert err.value.code == plb.PLB_ERR_ARG
+
+
+# ------------------------------------------------------------------ O-6 spread
+@pytest.mark.parametrize("kind", [(0, 0, 0), (0, 1, 0), (1, 1, 1)])
+def test_spread_matches_oracle(kind):
+    n = (37, 19, 23)
+    X = scattered_nodes(n, kind, 400, 47)
+    F = np.random.default_rng(53).standard_normal((400, 3))
+    sim, ora = mesh_pair(n, kind, X, np.zeros((0, 2), dtype=np.int32), None, 0.0)
+    sim.write_forces(F)
+    ora.write_forces(F)
+    sim.spread()
+    g_g = pu.forcing_to_soa(sim)
+    g_o = ora.spread()
+    assert np.abs(g_o).max() > 0.1
+    assert np.abs(g_g - g_o).max() <= 2e-6               # ~10 contributions of O(1) per cell, fp32
+    full = np.ones(400, dtype=bool)
+    for a in range(3):
+        if kind[a] == 1:
+            full &= (np.floor(X[:, a]) - 1 >= 0) & (np.floor(X[:, a]) + 2 <= n[a] - 1)
+    if full.all():                                        # P10 on the GPU result
+        assert np.abs(g_g.sum(1) - F.sum(0)).max() <= 2e-4
+    # a second spread on the same buffer first clears what the first one wrote
+    X2 = scattered_nodes(n, kind, 400, 59)
+    sim.write_nodes(X2)
+    ora.write_nodes(X2)
+    sim.write_forces(F)
+    ora.write_forces(F)
+    sim.spread()
+    assert np.abs(pu.forcing_to_soa(sim) - ora.spread()).max() <= 2e-6
+
+
+def test_spread_requires_forces_and_buffer():
+    X = np.full((1, 3), 4.0)
+    sim, _ = mesh_pair((8, 8, 8), (0, 0, 0), X, np.zeros((0, 2), dtype=np.int32), None, 0.0)
+    with pytest.raises(plb.PlbError) as e:
+        sim.spread()
+    assert e.value.code == plb.PLB_ERR_ORDER
+    sim.compute_membrane_forces()
+    with pytest.raises(plb.PlbError) as e:
+        plb.ib_spread(sim.h, None)
+    assert e.value.code == plb.PLB_ERR_ARG
+
+
+# ------------------------------------------------------------------ O-7 interpolate + advance
+@pytest.mark.parametrize("kind", [(0, 0, 0), (0, 1, 0), (1, 1, 1)])
+def test_interpolate_advance_matches_oracle(kind):
+    n = (37, 19, 23)
+    cells = n[0] * n[1] * n[2]
+    X = scattered_nodes(n, kind, 400, 61)
+    for a in range(3):                                    # keep every node inside the channel
+        if kind[a] == 1:
+            X[:, a] = np.clip(X[:, a], -0.3, n[a] - 0.7)
+    F = 1e-2 * np.random.default_rng(67).standard_normal((400, 3))
+    rho, u = wl.random_fields(71, cells)
+    sim, ora = mesh_pair(n, kind, X, np.zeros((0, 2), dtype=np.int32), None, 0.0)
+    sim.set_equilibrium(dev(rho), dev(u))
+    ora.set_equilibrium(rho, u)
+    for s in (sim, ora):
+        s.write_forces(F)
+    sim.spread(); sim.step(sim.forcing); sim.interpolate_advance()
+    g = ora.spread(); ora.step(g); ora.interpolate_advance()
+    sim.status()
+    U_g, U_o = sim.read_node_velocities().astype(np.float64), ora.read_node_velocities()
+    assert np.abs(U_o).max() > 1e-3
+    assert np.abs(U_g - U_o).max() <= 1e-6                # 64 products of O(0.03) x O(1) in fp32
+    assert np.abs(sim.read_nodes() - ora.read_nodes()).max() <= 1e-6
+    # the macros after a forced step carry g/2 (L201)
+    rho_g, u_g = sim.read_macros()
+    rho_o, u_o = ora.read_macros()
+    assert np.abs(u_g.cpu().numpy() - u_o).max() <= 6e-7
+    assert np.abs(rho_g.cpu().numpy() - rho_o).max() <= 6e-7
+
+
+def test_node_leaving_channel_is_reported():
+    n = (8, 8, 8)
+    u = np.zeros((3, 512)); u[1] = 0.2                    # fluid moving towards the wall
+    X = np.array([[4.0, 7.49, 4.0]])
+    sim, ora = mesh_pair(n, (0, 1, 0), X, np.zeros((0, 2), dtype=np.int32), None, 0.0)
+    sim.set_equilibrium(None, dev(u))
+    ora.set_equilibrium(None, u)
+    sim.coupled_step()
+    with pytest.raises(orc.OracleError) as eo:
+        ora.coupled_step()
+    assert eo.value.code == -5
+    with pytest.raises(plb.PlbError) as eg:
+        sim.status()
+    assert eg.value.code == plb.PLB_ERR_NODE_LEFT
+
+
+def test_no_meshes_is_a_no_op():
+    sim = plb.Simulation(8, 8, 8, 0.8)
+    sim.set_equilibrium()
+    sim.coupled_step()
+    sim.status()
+    assert sim.n_nodes == 0 and float(sim.forcing.abs().max()) == 0.0
+
+
+def test_capacity_is_enforced():
+    X = np.full((4, 3), 4.0) + np.arange(4)[:, None] * 0.1
+    sim = plb.Simulation(8, 8, 8, 0.8, max_nodes=4, max_edges=1)
+    sim.add_mesh(X, np.array([[0, 1]], dtype=np.int32))
+    with pytest.raises(plb.PlbError) as e:
+        sim.add_mesh(X, np.array([[0, 1]], dtype=np.int32))
+    assert e.value.code == plb.PLB_ERR_WORKSPACE
+    with pytest.raises(plb.PlbError) as e:
+        plb.Simulation(8, 8, 8, 0.8, max_nodes=4, max_edges=1).add_mesh(X, np.array([[0, 4]], dtype=np.int32))
+    assert e.value.code == plb.PLB_ERR_ARG
