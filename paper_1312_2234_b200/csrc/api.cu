@@ -42,7 +42,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     float* f0 = w.take<float>((size_t)Q * cells);
     float* f1 = w.take<float>((size_t)Q * cells);
     float4* vel = w.take<float4>((size_t)cells);
-    int* seg_flag = w.take<int>((size_t)n_segs);
+    unsigned* seg_mask = w.take<unsigned>((size_t)(n_segs + 31) / 32);
     int* seg_list = w.take<int>((size_t)n_segs);
     int* counters = w.take<int>(64);
     double* X0 = w.take<double>((size_t)max_nodes);
@@ -55,7 +55,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     float2* eprm = w.take<float2>((size_t)max_edges);
     if (c) {
         c->f[0] = f0; c->f[1] = f1; c->vel = vel;
-        c->seg_flag = seg_flag; c->seg_list = seg_list; c->counters = counters;
+        c->seg_mask = seg_mask; c->seg_list = seg_list; c->counters = counters;
         c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
         c->edges = edges; c->edge_prm = eprm;
     }
@@ -184,7 +184,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
             p.corr[a][1][d] = (float)(6.0 * w * hi);
         }
     }
-    rc = cuda_check(cudaMemsetAsync(c->seg_flag, 0, (size_t)n_segs * sizeof(int), c->stream), "clear segment flags");
+    rc = cuda_check(cudaMemsetAsync(c->seg_mask, 0, (size_t)((n_segs + 31) / 32) * sizeof(unsigned), c->stream), "clear segment mask");
     if (!rc) rc = cuda_check(cudaMemsetAsync(c->counters, 0, 64 * sizeof(int), c->stream), "clear counters");
     if (rc) {
         delete c;

@@ -87,11 +87,20 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
 // the same (oy, oz) touch four consecutive cells = 64 contiguous bytes of the float4 field.
 constexpr int LANES_PER_NODE = 16;
 
+// set the activity bit of a segment; whoever sets it first appends the segment to the list
+__device__ __forceinline__ void mark_segment(const int seg, unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
+                                             int* __restrict__ counters) {
+    const unsigned bit = 1u << (seg & 31);
+    unsigned* word = seg_mask + (seg >> 5);
+    if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u)
+        seg_list[atomicAdd(counters, 1)] = seg;
+}
+
 // S2: g_ijk += F_m phi phi phi (Eq. 34).  Also records which 32-cell segments were touched.
 __global__ void __launch_bounds__(256) spread_kernel(const double* __restrict__ X, const double* __restrict__ Y,
                                                      const double* __restrict__ Z, const float4* __restrict__ F,
                                                      const long n_nodes, float4* __restrict__ g,
-                                                     int* __restrict__ seg_flag, int* __restrict__ seg_list,
+                                                     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
                                                      int* __restrict__ counters, const LbmParams p) {
     const long t = blockIdx.x * 256L + threadIdx.x;
     const long m = t / LANES_PER_NODE;
@@ -110,24 +119,23 @@ __global__ void __launch_bounds__(256) spread_kernel(const double* __restrict__ 
         const float W = wxy * weight_of(az, oz);
         const int cell = qx + p.nx * (qy + p.ny * qz);
         atomicAdd(g + cell, make_float4(W * Fm.x, W * Fm.y, W * Fm.z, 0.f));
-        const int seg = cell >> SEG_SHIFT;
-        if (seg_flag[seg] == 0 && atomicExch(seg_flag + seg, 1) == 0) seg_list[atomicAdd(counters, 1)] = seg;
+        mark_segment(cell >> SEG_SHIFT, seg_mask, seg_list, counters);
     }
 }
 
-// zero the cells of the segments the previous spread touched, and drop their flags
-__global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ g, int* __restrict__ seg_flag,
+// zero the cells of the segments the previous spread touched, and drop their activity bits
+__global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ g, unsigned* __restrict__ seg_mask,
                                                            const int* __restrict__ seg_list,
                                                            const int* __restrict__ counters, const int cells) {
-    const int lane = threadIdx.x & 31;
-    const int warp = (blockIdx.x * 256 + threadIdx.x) >> 5;
-    const int n_warps = (gridDim.x * 256) >> 5;
+    const int sub = threadIdx.x & (SEG - 1);
+    const int group = (blockIdx.x * 256 + threadIdx.x) >> SEG_SHIFT;
+    const int n_groups = (gridDim.x * 256) >> SEG_SHIFT;
     const int n_active = __ldg(counters);
-    for (int s = warp; s < n_active; s += n_warps) {
+    for (int s = group; s < n_active; s += n_groups) {
         const int seg = seg_list[s];
-        const int idx = seg * SEG + lane;
+        const int idx = seg * SEG + sub;
         if (idx < cells) g[idx] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (lane == 0) seg_flag[seg] = 0;
+        if (sub == 0) seg_mask[seg >> 5] = 0u;        // every set bit of the word is in the list
     }
 }
 
@@ -212,7 +220,7 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
 }
 
 int launch_clear_spread(Ctx* c, float4* g) {
-    clear_spread_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(g, c->seg_flag, c->seg_list, c->counters, c->prm.cells);
+    clear_spread_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(g, c->seg_mask, c->seg_list, c->counters, c->prm.cells);
     c->launches++;
     int rc = cuda_check(cudaGetLastError(), "clear_spread_kernel");
     if (rc) return rc;
@@ -223,7 +231,7 @@ int launch_spread(Ctx* c, float4* g) {
     if (c->n_nodes == 0) return PLB_OK;
     const long threads = c->n_nodes * LANES_PER_NODE;
     spread_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->F, c->n_nodes, g, c->seg_flag, c->seg_list, c->counters, c->prm);
+        c->X[0], c->X[1], c->X[2], c->F, c->n_nodes, g, c->seg_mask, c->seg_list, c->counters, c->prm);
     c->launches++;
     return cuda_check(cudaGetLastError(), "spread_kernel");
 }

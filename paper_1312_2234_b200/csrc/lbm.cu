@@ -25,9 +25,11 @@ __device__ __forceinline__ Cell cell_of(int idx, const LbmParams& p) {
     return c;
 }
 
-// Pull the 19 streamed populations (minus w_d) of cell (i,j,k) out of the pre-stream lattice.
+// Pull the 19 streamed populations (minus w_d) of cell (i,j,k) out of the pre-stream lattice
+// into column COL of h.  Generic in the boundary kinds of all three axes.
+template <int V, int COL>
 __device__ __forceinline__ void pull19(const float* __restrict__ src, const LbmParams& p, const Cell c,
-                                       const int idx, float h[Q]) {
+                                       const int idx, float (&h)[Q][V]) {
     const int nx = p.nx, ny = p.ny, nz = p.nz;
     const size_t N = (size_t)p.cells;
     const bool xlo = c.i == 0, xhi = c.i == nx - 1;
@@ -60,102 +62,272 @@ __device__ __forceinline__ void pull19(const float* __restrict__ src, const LbmP
         if (cy == -1 && byhi) { b = true; corr = p.corr[1][1][d]; }
         if (cx == 1 && bxlo) { b = true; corr = p.corr[0][0][d]; }
         if (cx == -1 && bxhi) { b = true; corr = p.corr[0][1][d]; }
-        if (b) h[d] = __ldg(src + (size_t)OPP(d) * N + idx) + corr;
-        else   h[d] = __ldg(src + (size_t)d * N + (idx + off));
+        if (b) h[d][COL] = __ldg(src + (size_t)OPP(d) * N + idx) + corr;
+        else   h[d][COL] = __ldg(src + (size_t)d * N + (idx + off));
     }
 }
 
 // delta rho = sum h_d, j = sum c_d h_d (Eq. 17-18; sum_d w_d c_d = 0 so the shift drops out of j)
-__device__ __forceinline__ void moments(const float h[Q], float& drho, float& jx, float& jy, float& jz) {
+template <int V, int COL>
+__device__ __forceinline__ void moments(const float (&h)[Q][V], float& drho, float& jx, float& jy, float& jz) {
     // pairwise sums keep the fp32 rounding small and symmetric
-    const float a01p = h[0] + h[1], a23p = h[2] + h[3], a45p = h[4] + h[5];
-    const float s6 = (h[6] + h[11]) + (h[7] + h[10]);      // xy diagonals
-    const float s8 = (h[8] + h[13]) + (h[9] + h[12]);      // xz diagonals
-    const float s14 = (h[14] + h[17]) + (h[15] + h[16]);   // yz diagonals
-    drho = ((a01p + a23p) + (a45p + h[18])) + ((s6 + s8) + s14);
-    jx = (h[0] - h[1]) + (((h[6] - h[11]) + (h[7] - h[10])) + ((h[8] - h[13]) + (h[9] - h[12])));
-    jy = (h[2] - h[3]) + (((h[6] - h[11]) - (h[7] - h[10])) + ((h[14] - h[17]) + (h[15] - h[16])));
-    jz = (h[4] - h[5]) + (((h[8] - h[13]) - (h[9] - h[12])) + ((h[14] - h[17]) - (h[15] - h[16])));
+    const float a01p = h[0][COL] + h[1][COL], a23p = h[2][COL] + h[3][COL], a45p = h[4][COL] + h[5][COL];
+    const float s6 = (h[6][COL] + h[11][COL]) + (h[7][COL] + h[10][COL]);      // xy diagonals
+    const float s8 = (h[8][COL] + h[13][COL]) + (h[9][COL] + h[12][COL]);      // xz diagonals
+    const float s14 = (h[14][COL] + h[17][COL]) + (h[15][COL] + h[16][COL]);   // yz diagonals
+    drho = ((a01p + a23p) + (a45p + h[18][COL])) + ((s6 + s8) + s14);
+    const float d611 = h[6][COL] - h[11][COL], d710 = h[7][COL] - h[10][COL];
+    const float d813 = h[8][COL] - h[13][COL], d912 = h[9][COL] - h[12][COL];
+    const float d1417 = h[14][COL] - h[17][COL], d1516 = h[15][COL] - h[16][COL];
+    jx = (h[0][COL] - h[1][COL]) + ((d611 + d710) + (d813 + d912));
+    jy = (h[2][COL] - h[3][COL]) + ((d611 - d710) + (d1417 + d1516));
+    jz = (h[4][COL] - h[5][COL]) + ((d813 - d912) + (d1417 - d1516));
 }
 
 // BGK relaxation (Eq. 16) towards f_eq(rho, v) (Eq. 20) with v = u + g/(2 rho) (L201) plus the
 // Guo term (Eq. 19 in the form S_d = (1 - 1/2tau) w_d [3 (c_d - v).g + 9 (c_d.v)(c_d.g)],
-// DESIGN.md G3), all on the shifted populations:  h_eq,d = w_d [drho + rho (3 c.v + 4.5 (c.v)^2 - 1.5 v^2)].
-template <bool FORCED>
-__device__ __forceinline__ void collide(float h[Q], const float gx, const float gy, const float gz,
+// DESIGN.md G3), on the shifted populations  h_eq,d = w_d [drho + rho (3 c.v + 4.5 (c.v)^2 - 1.5 v^2)].
+//
+// fp32 and thousands of steps: a relaxation whose rounded constants do not add up EXACTLY to the
+// conservation laws multiplies the momentum of every cell by 1 + O(2^-24) per step -- coherent,
+// so it piles up linearly (velocity) and quadratically (node positions).  Hence
+//  * everything is written in the momentum m = rho v = j + g/2:  rho (c.v) = c.m needs no division,
+//    rho (c.v)^2 = (c.m)^2/rho, rho v^2 = m.m/rho, v.g = m.g/rho;
+//  * the lattice constants are fp32 numbers within 1.2e-7 (relative) of 3 w_d, 1.5 w_d and w_d that
+//    satisfy the moment identities exactly in real arithmetic:
+//        2 KA + 8 KG = 1           (first moment of the odd part  = m)
+//        6 AA + 12 AG + A0 = 3/2   (zeroth moment of the second-order part = 0, with 1/4 and 1/8)
+//        6 WA + 12 WG + W0 = 1     (zeroth moment of the density part = drho)
+//  * the relaxation is out = h + omega (h_eq - h), so omega itself needs no special form.
+// What is left are roundings of single operations, which do not have a preferred sign.
+// A population and its opposite share the part even in c_d and differ in the sign of the odd part.
+__device__ __forceinline__ float lattice_const(const unsigned bits) { return __uint_as_float(bits); }
+#define PLB_KA lattice_const(0x3e2aaaacu)   /* ~1/6   */
+#define PLB_KG lattice_const(0x3daaaaaau)   /* ~1/12: (1 - 2 KA)/8 */
+#define PLB_AA lattice_const(0x3daaaaacu)   /* ~1/12  */
+#define PLB_A0 lattice_const(0x3efffffcu)   /* ~1/2:  3/2 - 12 AA; AG = AA/2 */
+#define PLB_WA lattice_const(0x3d638e38u)   /* ~1/18  */
+#define PLB_W0 lattice_const(0x3eaaaaacu)   /* ~1/3:  1 - 12 WA;   WG = WA/2 */
+
+struct PairCoef {
+    float Z, B, K;      // w drho - 1.5 w m.m/rho,  4.5 w / rho,  3 w
+    float P, PK;        // 3 w pref / rho,  3 w pref
+};
+
+template <bool FORCED, int V, int COL>
+__device__ __forceinline__ void relax_pair(float (&h)[Q][V], const int d, const int e, const float cm, const float cg,
+                                           const float mg, const float omega, const PairCoef& k) {
+    const float even = fmaf(k.B, cm * cm, k.Z);
+    const float odd = k.K * cm;
+    float od = fmaf(omega, (even + odd) - h[d][COL], h[d][COL]);
+    float oe = fmaf(omega, (even - odd) - h[e][COL], h[e][COL]);
+    if (FORCED) {                                        // Guo term S_d (not relaxed)
+        const float se = k.P * fmaf(3.0f * cm, cg, -mg);
+        const float so = k.PK * cg;
+        od += se + so;
+        oe += se - so;
+    }
+    h[d][COL] = od;
+    h[e][COL] = oe;
+}
+
+template <bool FORCED, int V, int COL>
+__device__ __forceinline__ void collide(float (&h)[Q][V], const float gx, const float gy, const float gz,
                                         const float omega, const float pref) {
-    float drho, jx, jy, jz;
-    moments(h, drho, jx, jy, jz);
-    const float rho = 1.0f + drho;
-    const float inv = 1.0f / rho;
-    float vx, vy, vz;
+    float drho, mx, my, mz;
+    moments<V, COL>(h, drho, mx, my, mz);
     if (FORCED) {
-        vx = (jx + 0.5f * gx) * inv; vy = (jy + 0.5f * gy) * inv; vz = (jz + 0.5f * gz) * inv;
-    } else {
-        vx = jx * inv; vy = jy * inv; vz = jz * inv;
+        mx = fmaf(0.5f, gx, mx); my = fmaf(0.5f, gy, my); mz = fmaf(0.5f, gz, mz);
     }
-    const float vv15 = 1.5f * (vx * vx + vy * vy + vz * vz);
-    const float vg3 = 3.0f * (vx * gx + vy * gy + vz * gz);
-#pragma unroll
-    for (int d = 0; d < Q; ++d) {
-        const float cx = (float)CX(d), cy = (float)CY(d), cz = (float)CZ(d);
-        const float cv = cx * vx + cy * vy + cz * vz;
-        const float heq = WGT(d) * (drho + rho * (3.0f * cv + 4.5f * cv * cv - vv15));
-        float out = h[d] + omega * (heq - h[d]);
-        if (FORCED) {
-            const float cg = cx * gx + cy * gy + cz * gz;
-            out += pref * WGT(d) * (3.0f * cg - vg3 + 9.0f * cv * cg);
-        }
-        h[d] = out;
-    }
+    const float inv = 1.0f / (1.0f + drho);
+    const float mm = (mx * mx + my * my + mz * mz) * inv;           // rho v^2
+    const float mg = FORCED ? (mx * gx + my * gy + mz * gz) : 0.f;  // rho v.g
+    const float pri = pref * inv;
+    PairCoef k1, k2;                       // axes (w = 1/18), diagonals (w = 1/36)
+    k1.Z = fmaf(PLB_WA, drho, -PLB_AA * mm); k1.B = 0.25f * inv;  k1.K = PLB_KA;
+    k2.Z = 0.5f * k1.Z;                      k2.B = 0.125f * inv; k2.K = PLB_KG;
+    k1.P = PLB_KA * pri; k1.PK = PLB_KA * pref;
+    k2.P = PLB_KG * pri; k2.PK = PLB_KG * pref;
+    relax_pair<FORCED, V, COL>(h, 0, 1, mx, gx, mg, omega, k1);
+    relax_pair<FORCED, V, COL>(h, 2, 3, my, gy, mg, omega, k1);
+    relax_pair<FORCED, V, COL>(h, 4, 5, mz, gz, mg, omega, k1);
+    relax_pair<FORCED, V, COL>(h, 6, 11, mx + my, gx + gy, mg, omega, k2);
+    relax_pair<FORCED, V, COL>(h, 7, 10, mx - my, gx - gy, mg, omega, k2);
+    relax_pair<FORCED, V, COL>(h, 8, 13, mx + mz, gx + gz, mg, omega, k2);
+    relax_pair<FORCED, V, COL>(h, 9, 12, mx - mz, gx - gz, mg, omega, k2);
+    relax_pair<FORCED, V, COL>(h, 14, 17, my + mz, gy + gz, mg, omega, k2);
+    relax_pair<FORCED, V, COL>(h, 15, 16, my - mz, gy - gz, mg, omega, k2);
+    // rest population: c = 0
+    const float rest = fmaf(PLB_W0, drho, -PLB_A0 * mm);
+    float o18 = fmaf(omega, rest - h[18][COL], h[18][COL]);
+    if (FORCED) o18 = fmaf(-pri, mg, o18);               // S_19 = w_19 * 3 * pref * (-v.g)
+    h[18][COL] = o18;
 }
 
 // ---------------------------------------------------------------------------------------------
-// S3: fused pull-stream + collide + boundary kernel.  One thread per cell, one warp per
-// 32-cell segment; loads along x are unit-stride, stores are aligned and coalesced.
+// S3, generic kernel: fused pull-stream + collide + boundary, one thread per cell.  Handles every
+// grid size and boundary mix; used when the vectorised kernel below does not apply.
 // ---------------------------------------------------------------------------------------------
 template <int MODE>
-__global__ void __launch_bounds__(256) lbm_step_kernel(const float* __restrict__ src, float* __restrict__ dst,
-                                                       const float4* __restrict__ g,
-                                                       const int* __restrict__ seg_flag, const LbmParams p) {
-    const int idx = blockIdx.x * 256 + threadIdx.x;
-    if (idx >= p.cells) return;
-    const Cell c = cell_of(idx, p);
-    float h[Q];
-    pull19(src, p, c, idx, h);
+__device__ __forceinline__ void step_one_cell(const float* __restrict__ src, float* __restrict__ dst,
+                                              const float4* __restrict__ g, const unsigned* __restrict__ seg_mask,
+                                              const LbmParams& p, const Cell c, const int idx) {
+    float h[Q][1];
+    pull19<1, 0>(src, p, c, idx, h);
     bool forced = false;
     float4 g4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (MODE == FORCE_DENSE) {
         g4 = __ldg(g + idx);
         forced = true;
     } else if (MODE == FORCE_SPARSE) {
-        if (__ldg(seg_flag + (idx >> SEG_SHIFT))) {      // warp-uniform
+        if (seg_active(seg_mask, idx)) {
             g4 = __ldg(g + idx);
             forced = true;
         }
     }
-    if (forced) collide<true>(h, g4.x, g4.y, g4.z, p.omega, p.pref);
-    else        collide<false>(h, 0.f, 0.f, 0.f, p.omega, p.pref);
+    if (forced) collide<true, 1, 0>(h, g4.x, g4.y, g4.z, p.omega, p.pref);
+    else        collide<false, 1, 0>(h, 0.f, 0.f, 0.f, p.omega, p.pref);
     const size_t N = (size_t)p.cells;
 #pragma unroll
-    for (int d = 0; d < Q; ++d) dst[(size_t)d * N + idx] = h[d];
+    for (int d = 0; d < Q; ++d) dst[(size_t)d * N + idx] = h[d][0];
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(256) lbm_step_kernel(const float* __restrict__ src, float* __restrict__ dst,
+                                                       const float4* __restrict__ g,
+                                                       const unsigned* __restrict__ seg_mask, const LbmParams p) {
+    const int idx = blockIdx.x * 256 + threadIdx.x;
+    if (idx >= p.cells) return;
+    step_one_cell<MODE>(src, dst, g, seg_mask, p, cell_of(idx, p), idx);
+}
+
+// ---------------------------------------------------------------------------------------------
+// S3, vectorised kernel (nx % V == 0, x periodic): one thread per V consecutive cells of a row.
+//  * c_x = 0 populations: one aligned 128-bit (V = 4) load;
+//  * c_x = +-1 populations: the aligned vector of the same V cells, shifted by one through the
+//    neighbouring lane (shfl), the lane at a warp / row edge fetching the one missing element;
+//  * stores are aligned vectors.  Rows on a bounce-back face take the generic per-cell path.
+// ---------------------------------------------------------------------------------------------
+template <int V> struct Vec;
+template <> struct Vec<4> {
+    static __device__ __forceinline__ void load(const float* p, float (&a)[4]) {
+        const float4 t = __ldg(reinterpret_cast<const float4*>(p));
+        a[0] = t.x; a[1] = t.y; a[2] = t.z; a[3] = t.w;
+    }
+};
+template <> struct Vec<2> {
+    static __device__ __forceinline__ void load(const float* p, float (&a)[2]) {
+        const float2 t = __ldg(reinterpret_cast<const float2*>(p));
+        a[0] = t.x; a[1] = t.y;
+    }
+};
+
+template <int MODE, int V, int COL>
+__device__ __forceinline__ void collide_cols(float (&h)[Q][V], const float4 (&g4)[V], const bool forced,
+                                             const float omega, const float pref) {
+    if (MODE != FORCE_NONE && forced) collide<true, V, COL>(h, g4[COL].x, g4[COL].y, g4[COL].z, omega, pref);
+    else                              collide<false, V, COL>(h, 0.f, 0.f, 0.f, omega, pref);
+    if constexpr (COL + 1 < V) collide_cols<MODE, V, COL + 1>(h, g4, forced, omega, pref);
+}
+
+template <int MODE, int V, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) lbm_step_vec_kernel(const float* __restrict__ src, float* __restrict__ dst,
+                                                                    const float4* __restrict__ g,
+                                                                    const unsigned* __restrict__ seg_mask,
+                                                                    const LbmParams p) {
+    constexpr unsigned FULL = 0xffffffffu;
+    const int nx = p.nx, ny = p.ny, nz = p.nz;
+    const unsigned nvec = (unsigned)p.cells / V;
+    unsigned t = blockIdx.x * THREADS + threadIdx.x;
+    const bool live = t < nvec;
+    if (!live) t = nvec - 1;                            // keeps the lane for the shuffles below
+    const int idx0 = (int)(t * V);
+    const unsigned row = (unsigned)idx0 / (unsigned)nx;
+    const int i0 = idx0 - (int)(row * (unsigned)nx);
+    const int k = (int)(row / (unsigned)ny);
+    const int j = (int)row - k * ny;
+    const bool wall_row = (p.wall[1] && (j == 0 || j == ny - 1)) || (p.wall[2] && (k == 0 || k == nz - 1));
+    const size_t N = (size_t)p.cells;
+    float h[Q][V];
+    if (!__all_sync(FULL, wall_row)) {
+        const int lane = threadIdx.x & 31;
+        const bool first = lane == 0 || i0 == 0;          // cell i0 - 1 is not in the lane below
+        const bool last = lane == 31 || i0 + V == nx;     // cell i0 + V is not in the lane above
+        const int xm = i0 == 0 ? nx - 1 : -1;             // offset of cell i0 - 1 (periodic)
+        const int xp = i0 + V == nx ? V - nx : V;         // offset of cell i0 + V (periodic)
+        const int dym = (j == 0 ? ny - 1 : -1) * nx, dyp = (j == ny - 1 ? 1 - ny : 1) * nx;
+        const int dzm = (k == 0 ? nz - 1 : -1) * nx * ny, dzp = (k == nz - 1 ? 1 - nz : 1) * nx * ny;
+#pragma unroll
+        for (int d = 0; d < Q; ++d) {
+            const int cx = CX(d), cy = CY(d), cz = CZ(d);
+            int off = 0;
+            if (cy == 1) off += dym;
+            if (cy == -1) off += dyp;
+            if (cz == 1) off += dzm;
+            if (cz == -1) off += dzp;
+            const float* base = src + (size_t)d * N + (idx0 + off);
+            float a[V];
+            Vec<V>::load(base, a);
+            if (cx == 0) {
+#pragma unroll
+                for (int c = 0; c < V; ++c) h[d][c] = a[c];
+            } else if (cx == 1) {                         // f_d(i) = T_d(i - 1)
+                float prev = __shfl_up_sync(FULL, a[V - 1], 1);
+                if (first) prev = __ldg(base + xm);
+                h[d][0] = prev;
+#pragma unroll
+                for (int c = 1; c < V; ++c) h[d][c] = a[c - 1];
+            } else {                                      // f_d(i) = T_d(i + 1)
+                float next = __shfl_down_sync(FULL, a[0], 1);
+                if (last) next = __ldg(base + xp);
+#pragma unroll
+                for (int c = 0; c + 1 < V; ++c) h[d][c] = a[c + 1];
+                h[d][V - 1] = next;
+            }
+        }
+    }
+    if (!live) return;
+    if (wall_row) {
+#pragma unroll 1
+        for (int c = 0; c < V; ++c) {
+            Cell cell;
+            cell.i = i0 + c; cell.j = j; cell.k = k;
+            step_one_cell<MODE>(src, dst, g, seg_mask, p, cell, idx0 + c);
+        }
+        return;
+    }
+    bool forced = false;
+    float4 g4[V];
+    if (MODE == FORCE_DENSE) forced = true;
+    if (MODE == FORCE_SPARSE) forced = seg_active(seg_mask, idx0);   // V divides SEG: one flag for all V cells
+    if (MODE != FORCE_NONE && forced) {
+#pragma unroll
+        for (int c = 0; c < V; ++c) g4[c] = __ldg(g + idx0 + c);
+    }
+    collide_cols<MODE, V, 0>(h, g4, forced, p.omega, p.pref);
+#pragma unroll
+    for (int d = 0; d < Q; ++d) {
+        float* out = dst + (size_t)d * N + idx0;
+        if constexpr (V == 4) *reinterpret_cast<float4*>(out) = make_float4(h[d][0], h[d][1], h[d][2], h[d][3]);
+        else                  *reinterpret_cast<float2*>(out) = make_float2(h[d][0], h[d][1]);
+    }
 }
 
 // rho and v = (j + g_last/2)/rho of the streamed state (what the next step will collide)
 template <int MODE>
 __global__ void __launch_bounds__(256) macros_kernel(const float* __restrict__ src, const float4* __restrict__ g,
-                                                     const int* __restrict__ seg_flag, float* __restrict__ rho_out,
+                                                     const unsigned* __restrict__ seg_mask, float* __restrict__ rho_out,
                                                      float* __restrict__ u_out, const LbmParams p) {
     const int idx = blockIdx.x * 256 + threadIdx.x;
     if (idx >= p.cells) return;
     const Cell c = cell_of(idx, p);
-    float h[Q];
-    pull19(src, p, c, idx, h);
+    float h[Q][1];
+    pull19<1, 0>(src, p, c, idx, h);
     float drho, jx, jy, jz;
-    moments(h, drho, jx, jy, jz);
+    moments<1, 0>(h, drho, jx, jy, jz);
     float4 g4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (MODE == FORCE_DENSE) g4 = __ldg(g + idx);
-    if (MODE == FORCE_SPARSE && __ldg(seg_flag + (idx >> SEG_SHIFT))) g4 = __ldg(g + idx);
+    if (MODE == FORCE_SPARSE && seg_active(seg_mask, idx)) g4 = __ldg(g + idx);
     const float rho = 1.0f + drho, inv = 1.0f / rho;
     if (rho_out) rho_out[idx] = rho;
     if (u_out) {
@@ -174,18 +346,18 @@ __global__ void __launch_bounds__(256) sparse_moments_kernel(const float* __rest
                                                              const int* __restrict__ seg_list,
                                                              const int* __restrict__ counters,
                                                              float4* __restrict__ vel, const LbmParams p) {
-    const int lane = threadIdx.x & 31;
-    const int warp = (blockIdx.x * 256 + threadIdx.x) >> 5;
-    const int n_warps = (gridDim.x * 256) >> 5;
+    const int sub = threadIdx.x & (SEG - 1);
+    const int group = (blockIdx.x * 256 + threadIdx.x) >> SEG_SHIFT;
+    const int n_groups = (gridDim.x * 256) >> SEG_SHIFT;
     const int n_active = __ldg(counters);
-    for (int s = warp; s < n_active; s += n_warps) {
-        const int idx = __ldg(seg_list + s) * SEG + lane;
+    for (int s = group; s < n_active; s += n_groups) {
+        const int idx = __ldg(seg_list + s) * SEG + sub;
         if (idx >= p.cells) continue;
         const Cell c = cell_of(idx, p);
-        float h[Q];
-        pull19(src, p, c, idx, h);
+        float h[Q][1];
+        pull19<1, 0>(src, p, c, idx, h);
         float drho, jx, jy, jz;
-        moments(h, drho, jx, jy, jz);
+        moments<1, 0>(h, drho, jx, jy, jz);
         float4 g4 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (MODE != FORCE_NONE) g4 = __ldg(g + idx);
         const float rho = 1.0f + drho, inv = 1.0f / rho;
@@ -279,10 +451,10 @@ __global__ void __launch_bounds__(256) read_populations_kernel(const float* __re
                                                                const LbmParams p) {
     const int idx = blockIdx.x * 256 + threadIdx.x;
     if (idx >= p.cells) return;
-    float h[Q];
-    pull19(src, p, cell_of(idx, p), idx, h);
+    float h[Q][1];
+    pull19<1, 0>(src, p, cell_of(idx, p), idx, h);
 #pragma unroll
-    for (int d = 0; d < Q; ++d) f[(size_t)d * p.cells + idx] = h[d] + WGT(d);
+    for (int d = 0; d < Q; ++d) f[(size_t)d * p.cells + idx] = h[d][0] + WGT(d);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -296,13 +468,28 @@ int launch_set_equilibrium(Ctx* c, const float* d_rho, const float* d_u, float a
     return cuda_check(cudaGetLastError(), "set_equilibrium_kernel");
 }
 
+// The vectorised kernel needs rows that are whole vectors and a periodic x axis; V = 4 cells per
+// thread, 128 threads per block (512 cells), at least 4 blocks per SM.
+constexpr int LBM_V = 4, LBM_THREADS = 128, LBM_MINB = 4;
+
+template <int MODE>
+static void launch_step_mode(Ctx* c, const float* src, float* dst, const float4* g) {
+    const LbmParams& p = c->prm;
+    if (p.nx % LBM_V == 0 && !p.wall[0]) {
+        const unsigned nvec = (unsigned)p.cells / LBM_V;
+        lbm_step_vec_kernel<MODE, LBM_V, LBM_THREADS, LBM_MINB>
+            <<<(nvec + LBM_THREADS - 1) / LBM_THREADS, LBM_THREADS, 0, c->stream>>>(src, dst, g, c->seg_mask, p);
+    } else {
+        lbm_step_kernel<MODE><<<grid_cells(c), 256, 0, c->stream>>>(src, dst, g, c->seg_mask, p);
+    }
+}
+
 int launch_lbm_step(Ctx* c, const float4* g, int mode) {
     const float* src = c->f[c->cur];
     float* dst = c->f[c->cur ^ 1];
-    const int grid = grid_cells(c);
-    if (mode == FORCE_NONE) lbm_step_kernel<FORCE_NONE><<<grid, 256, 0, c->stream>>>(src, dst, nullptr, nullptr, c->prm);
-    else if (mode == FORCE_DENSE) lbm_step_kernel<FORCE_DENSE><<<grid, 256, 0, c->stream>>>(src, dst, g, nullptr, c->prm);
-    else lbm_step_kernel<FORCE_SPARSE><<<grid, 256, 0, c->stream>>>(src, dst, g, c->seg_flag, c->prm);
+    if (mode == FORCE_NONE) launch_step_mode<FORCE_NONE>(c, src, dst, nullptr);
+    else if (mode == FORCE_DENSE) launch_step_mode<FORCE_DENSE>(c, src, dst, g);
+    else launch_step_mode<FORCE_SPARSE>(c, src, dst, g);
     c->launches++;
     c->cur ^= 1;
     return cuda_check(cudaGetLastError(), "lbm_step_kernel");
@@ -316,7 +503,7 @@ int launch_read_macros(Ctx* c, float* d_rho, float* d_u) {
     else if (c->g_last_mode == FORCE_DENSE)
         macros_kernel<FORCE_DENSE><<<grid, 256, 0, c->stream>>>(src, c->g_last, nullptr, d_rho, d_u, c->prm);
     else
-        macros_kernel<FORCE_SPARSE><<<grid, 256, 0, c->stream>>>(src, c->g_last, c->seg_flag, d_rho, d_u, c->prm);
+        macros_kernel<FORCE_SPARSE><<<grid, 256, 0, c->stream>>>(src, c->g_last, c->seg_mask, d_rho, d_u, c->prm);
     c->launches++;
     return cuda_check(cudaGetLastError(), "macros_kernel");
 }

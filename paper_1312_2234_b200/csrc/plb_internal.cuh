@@ -9,8 +9,11 @@
 namespace plb {
 
 constexpr int Q = 19;
-constexpr int SEG = 32;        // cells per activity segment = one warp of the LBM kernel
-constexpr int SEG_SHIFT = 5;
+// Activity segments: 8 consecutive cells (one 128-byte line of the float4 forcing field, one
+// 32-byte sector of a population row).  Bit (s & 31) of seg_mask[s >> 5] is set while segment s
+// holds spread force; seg_list enumerates the set bits.
+constexpr int SEG = 8;
+constexpr int SEG_SHIFT = 3;
 
 // D3Q19 velocity set in the paper's numbering (Eq. 21, Eq. 23-30; index = paper's i - 1).
 __host__ __device__ constexpr int CX(int d) {
@@ -46,6 +49,10 @@ enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 
 // status bits raised by kernels (sticky)
 enum { STATUS_NODE_LEFT = 1, STATUS_ZERO_EDGE = 2 };
+
+__device__ __forceinline__ bool seg_active(const unsigned* __restrict__ seg_mask, const int cell) {
+    return (__ldg(seg_mask + (cell >> (SEG_SHIFT + 5))) >> ((cell >> SEG_SHIFT) & 31)) & 1u;
+}
 
 // ---------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), written from the paper's description.
@@ -86,7 +93,7 @@ struct Ctx {
     float* f[2];
     int cur;
     float4* vel;               // (vx, vy, vz, rho) at the active cells, cells entries
-    int* seg_flag;             // n_segs
+    unsigned* seg_mask;        // one bit per segment, (n_segs + 31) / 32 words
     int* seg_list;             // n_segs
     int* counters;             // [0] active segment count, [1] status bits
     // meshes

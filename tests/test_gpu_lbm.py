@@ -123,6 +123,36 @@ def test_steps_match_oracle_all_boundaries(kind, forced):
     sim.status()
 
 
+# grids that take the vectorised kernel (nx % 4 == 0, x periodic): a warp spanning several rows
+# (nx = 8, 40), exactly one row (128), part of a row (256); partial last warp; walls in y and z
+VEC_SHAPES = [(40, 9, 11), (128, 7, 5), (8, 5, 5), (256, 4, 3), (4, 3, 2)]
+
+
+@pytest.mark.parametrize("n", VEC_SHAPES)
+@pytest.mark.parametrize("kind", [(0, 0, 0), (0, 1, 0), (0, 0, 1), (0, 1, 1)])
+@pytest.mark.parametrize("forced", [False, True])
+def test_steps_match_oracle_vector_path(n, kind, forced):
+    cells = n[0] * n[1] * n[2]
+    rho, u = wl.random_fields(41, cells)
+    u_lo, u_hi = wall_velocities(kind, 43)
+    sim, ora = make_pair(n, 0.7, kind, u_lo, u_hi)
+    sim.set_equilibrium(dev(rho), dev(u), 1e-4, 99)
+    ora.set_equilibrium(rho, u, 1e-4, 99)
+    rng = np.random.default_rng(47)
+    for s in range(5):
+        g = 1e-3 * (2 * rng.random((3, cells)) - 1) if forced else None
+        gd = pu.soa_to_forcing(sim, g) if forced else None
+        sim.step(gd)
+        ora.step(g)
+        f_g = sim.read_populations().cpu().numpy().astype(np.float64)
+        assert np.abs(f_g - ora.read_populations()).max() <= 3e-7, "step %d" % s
+    rho_g, u_g = sim.read_macros()
+    rho_o, u_o = ora.read_macros()
+    assert np.abs(rho_g.cpu().numpy() - rho_o).max() <= 6e-7
+    assert np.abs(u_g.cpu().numpy() - u_o).max() <= 6e-7
+    sim.status()
+
+
 def test_macros_before_any_step_and_null_outputs():
     n = (16, 8, 8)
     cells = n[0] * n[1] * n[2]
