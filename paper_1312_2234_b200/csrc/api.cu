@@ -1,5 +1,6 @@
 // api.cu -- the C-ABI of libplb (include/plb.h): argument checks, workspace carving, call-order
 // bookkeeping.  Every step of the path runs in the kernels of lbm.cu / ib.cu.
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -41,9 +42,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     Carve w{base, 0};
     float* f0 = w.take<float>((size_t)Q * cells);
     float* f1 = w.take<float>((size_t)Q * cells);
-    float4* vel = w.take<float4>((size_t)cells);
     unsigned* seg_mask = w.take<unsigned>((size_t)(n_segs + 31) / 32);
-    int* seg_list = w.take<int>((size_t)n_segs);
     int* counters = w.take<int>(64);
     double* X0 = w.take<double>((size_t)max_nodes);
     double* X1 = w.take<double>((size_t)max_nodes);
@@ -53,11 +52,12 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     double* stage = w.take<double>((size_t)3 * max_nodes);
     int2* edges = w.take<int2>((size_t)max_edges);
     float2* eprm = w.take<float2>((size_t)max_edges);
+    int2* ranges = w.take<int2>((size_t)max_nodes);
     if (c) {
-        c->f[0] = f0; c->f[1] = f1; c->vel = vel;
-        c->seg_mask = seg_mask; c->seg_list = seg_list; c->counters = counters;
+        c->f[0] = f0; c->f[1] = f1;
+        c->seg_mask = seg_mask; c->counters = counters;
         c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
-        c->edges = edges; c->edge_prm = eprm;
+        c->edges = edges; c->edge_prm = eprm; c->ranges = ranges;
     }
     return w.off;
 }
@@ -165,6 +165,8 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->g_last = nullptr; c->g_last_mode = FORCE_NONE; c->spread_target = nullptr;
     c->spread_current = false; c->forces_valid = false; c->populated = false;
     c->launches = 0;
+    c->n_ranges = 0;
+    c->tile_cap = 512;
     c->sm_count = sms;
     c->mesh_node_off.push_back(0);
     c->mesh_edge_off.push_back(0);
@@ -311,7 +313,33 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
             ep[(size_t)s * n_edges + e] = make_float2(L, k);
         }
     }
-    int rc = PLB_OK;
+    // node ranges of the IB thread blocks (a mesh, cut every IB_RANGE_NODES nodes) and the tile
+    // capacity their initial bounding boxes ask for (two cells of slack per axis for deformation)
+    constexpr int IB_RANGE_NODES = 4096;
+    std::vector<int2> rg;
+    int cap = ctx->tile_cap;
+    for (int s = 0; s < n_meshes; ++s) {
+        const long noff = ctx->n_nodes + (long)s * n_nodes;
+        const double* x = h_xyz + (size_t)3 * s * n_nodes;
+        for (int a = 0; a < n_nodes; a += IB_RANGE_NODES) {
+            const int b = a + IB_RANGE_NODES < n_nodes ? a + IB_RANGE_NODES : n_nodes;
+            rg.push_back(make_int2((int)(noff + a), (int)(noff + b)));
+            double vol = 1.0;
+            for (int d = 0; d < 3; ++d) {
+                double lo = floor(x[3 * a + d]), hi = lo;
+                for (int m = a + 1; m < b; ++m) {
+                    const double f = floor(x[3 * m + d]);
+                    lo = f < lo ? f : lo;
+                    hi = f > hi ? f : hi;
+                }
+                vol *= hi - lo + 4.0 + 2.0;
+            }
+            if (vol <= (double)ib_max_tile_cap() && (int)vol > cap) cap = (int)vol;
+        }
+    }
+    ctx->tile_cap = cap;
+    int rc = cuda_check(cudaMemcpyAsync(ctx->ranges + ctx->n_ranges, rg.data(), rg.size() * sizeof(int2),
+                                        cudaMemcpyHostToDevice, ctx->stream), "upload node ranges");
     for (int d = 0; d < 3 && !rc; ++d)
         rc = cuda_check(cudaMemcpyAsync(ctx->X[d] + ctx->n_nodes, soa.data() + (size_t)d * add_nodes,
                                         (size_t)add_nodes * sizeof(double), cudaMemcpyHostToDevice, ctx->stream),
@@ -326,6 +354,7 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
     }
     if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
     if (rc) return rc;
+    ctx->n_ranges += (long)rg.size();
     if (out_first_mesh_id) *out_first_mesh_id = (int)ctx->mesh_node_off.size() - 1;
     for (int s = 0; s < n_meshes; ++s) {
         ctx->n_nodes += n_nodes;
@@ -380,9 +409,7 @@ int ib_interpolate_advance(plb_ctx* ctx) {
         set_error("ib_interpolate_advance must follow ib_spread (and lbm_step) for the current node positions");
         return PLB_ERR_ORDER;
     }
-    int rc = launch_sparse_moments(ctx);
-    if (rc) return rc;
-    rc = launch_interpolate_advance(ctx);
+    const int rc = launch_interpolate_advance(ctx);
     ctx->spread_current = false;
     ctx->forces_valid = false;
     return rc;

@@ -3,7 +3,9 @@
 // Node data: positions SoA fp64 (unwrapped), forces / node velocities float4 AoS.
 // The forcing field is float4 per cell so that the spread is one 128-bit vector atomic per
 // (node, cell) pair (red.global.add.v4.f32, sm_90+).
+#include <climits>
 #include "plb_internal.cuh"
+#include "lbm_device.cuh"
 
 namespace plb {
 
@@ -83,104 +85,362 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
     return q < 0 ? q + n : q;
 }
 
-// S2 + S4 share the mapping: 16 lanes per node, lane = (ox, oy), loop over oz.  Four lanes with
-// the same (oy, oz) touch four consecutive cells = 64 contiguous bytes of the float4 field.
+// ---------------------------------------------------------------------------------------------
+// S2 and S4/S5 run one thread block per NODE RANGE (a mesh, or a slice of a very large mesh).
+// A platelet is a compact object: the 4x4x4 supports of its nodes overlap heavily (about 13
+// contributions per touched cell at config 4, 1000 at config 5), so the block accumulates /
+// gathers through a TILE of the lattice held in shared memory -- the bounding box of the
+// supports of its nodes -- and touches global memory once per tile cell:
+//   spread:       zero tile -> nodes scatter into the tile -> the non-zero tile cells go to the
+//                 forcing field with one 128-bit RED each.  The tile accumulates in 32-bit fixed
+//                 point with a per-block power-of-two scale (native shared-memory integer
+//                 atomics; the fp32 ones are compare-and-swap loops): order-independent, and
+//                 with a resolution of n_nodes/8 * 2^-30 of the largest nodal force component;
+//   interpolate:  mark the tile cells some node needs -> compact them -> their v straight from
+//                 the 19 pulled populations (no velocity field in HBM) -> nodes gather from the tile.
+// A range whose bounding box does not fit the tile (a non-compact "mesh") takes the direct path:
+// global REDs per (node, cell) and on-the-fly cell moments.  Both paths compute the same sums.
+// Within a block 16 lanes serve one node: lane = (ox, oy), loop over oz.
+// ---------------------------------------------------------------------------------------------
+constexpr int IB_THREADS = 512;
+constexpr int IB_CHUNK = 256;                      // nodes whose stencil records are staged at a time
 constexpr int LANES_PER_NODE = 16;
+constexpr int IB_GROUPS = IB_THREADS / LANES_PER_NODE;
 
-// set the activity bit of a segment; whoever sets it first appends the segment to the list
-__device__ __forceinline__ void mark_segment(const int seg, unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
-                                             int* __restrict__ counters) {
+struct MeshTile {
+    int o[3];            // unwrapped lattice coordinate of tile cell (0,0,0)
+    int e[3];            // extent in cells
+    int lo[3], hi[3];    // tile coordinates [lo, hi) that exist on the lattice (wall axes clip)
+    int enabled;
+    int mn[3], mx[3];    // reduction scratch: min / max of floor(X)
+    unsigned fmax_bits;  // reduction scratch: largest |F| component (non-negative float bits)
+    int n_need;          // interpolate: number of tile cells some node needs
+};
+
+// set the activity bit of the 8-cell segment of a cell
+__device__ __forceinline__ void mark_segment(const int cell, unsigned* __restrict__ seg_mask) {
+    const int seg = cell >> SEG_SHIFT;
     const unsigned bit = 1u << (seg & 31);
     unsigned* word = seg_mask + (seg >> 5);
-    if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u)
-        seg_list[atomicAdd(counters, 1)] = seg;
+    if ((*(volatile unsigned*)word & bit) == 0u) atomicOr(word, bit);
 }
 
-// S2: g_ijk += F_m phi phi phi (Eq. 34).  Also records which 32-cell segments were touched.
-__global__ void __launch_bounds__(256) spread_kernel(const double* __restrict__ X, const double* __restrict__ Y,
-                                                     const double* __restrict__ Z, const float4* __restrict__ F,
-                                                     const long n_nodes, float4* __restrict__ g,
-                                                     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
-                                                     int* __restrict__ counters, const LbmParams p) {
-    const long t = blockIdx.x * 256L + threadIdx.x;
-    const long m = t / LANES_PER_NODE;
-    if (m >= n_nodes) return;
-    const int sub = (int)(t % LANES_PER_NODE), ox = sub & 3, oy = sub >> 2;
-    const Axis ax = axis_of(__ldg(X + m)), ay = axis_of(__ldg(Y + m)), az = axis_of(__ldg(Z + m));
-    const float4 Fm = __ldg(F + m);
-    const int qx = wrap_index(ax.base + ox, p.nx, p.wall[0]);
-    const int qy = wrap_index(ay.base + oy, p.ny, p.wall[1]);
-    if (qx < 0 || qy < 0) return;
-    const float wxy = weight_of(ax, ox) * weight_of(ay, oy);
-#pragma unroll
-    for (int oz = 0; oz < 4; ++oz) {
-        const int qz = wrap_index(az.base + oz, p.nz, p.wall[2]);
-        if (qz < 0) continue;
-        const float W = wxy * weight_of(az, oz);
-        const int cell = qx + p.nx * (qy + p.ny * qz);
-        atomicAdd(g + cell, make_float4(W * Fm.x, W * Fm.y, W * Fm.z, 0.f));
-        mark_segment(cell >> SEG_SHIFT, seg_mask, seg_list, counters);
+// bounding box of the supports of nodes [n0, n1) -> tile geometry (all threads of the block);
+// with F != nullptr also the largest force component of the range
+__device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict__ X, const double* __restrict__ Y,
+                                           const double* __restrict__ Z, const float4* __restrict__ F, const int n0,
+                                           const int n1, const LbmParams& p, const int cap) {
+    if (threadIdx.x == 0) {
+        for (int a = 0; a < 3; ++a) { T.mn[a] = INT_MAX; T.mx[a] = INT_MIN; }
+        T.fmax_bits = 0u;
+        T.n_need = 0;
     }
-}
-
-// zero the cells of the segments the previous spread touched, and drop their activity bits
-__global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ g, unsigned* __restrict__ seg_mask,
-                                                           const int* __restrict__ seg_list,
-                                                           const int* __restrict__ counters, const int cells) {
-    const int sub = threadIdx.x & (SEG - 1);
-    const int group = (blockIdx.x * 256 + threadIdx.x) >> SEG_SHIFT;
-    const int n_groups = (gridDim.x * 256) >> SEG_SHIFT;
-    const int n_active = __ldg(counters);
-    for (int s = group; s < n_active; s += n_groups) {
-        const int seg = seg_list[s];
-        const int idx = seg * SEG + sub;
-        if (idx < cells) g[idx] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (sub == 0) seg_mask[seg >> 5] = 0u;        // every set bit of the word is in the list
-    }
-}
-
-// S4 + S5: U_m = sum v phi phi phi (Eq. 33) by a 16-lane shuffle reduction over the 4x4x4
-// stencil, then X_m += U_m in fp64.
-__global__ void __launch_bounds__(256) interpolate_advance_kernel(double* __restrict__ X, double* __restrict__ Y,
-                                                                  double* __restrict__ Z, float4* __restrict__ U,
-                                                                  const long n_nodes, const float4* __restrict__ vel,
-                                                                  int* __restrict__ counters, const LbmParams p) {
-    const long t = blockIdx.x * 256L + threadIdx.x;
-    const long m = t / LANES_PER_NODE;
-    const bool live = m < n_nodes;                      // dead lanes still take part in the shuffles
-    const int sub = (int)(t % LANES_PER_NODE), ox = sub & 3, oy = sub >> 2;
-    const double xm = live ? X[m] : 0.0, ym = live ? Y[m] : 0.0, zm = live ? Z[m] : 0.0;
-    const Axis ax = axis_of(xm), ay = axis_of(ym), az = axis_of(zm);
-    const int qx = wrap_index(ax.base + ox, p.nx, p.wall[0]);
-    const int qy = wrap_index(ay.base + oy, p.ny, p.wall[1]);
-    float ux = 0.f, uy = 0.f, uz = 0.f;
-    if (live && qx >= 0 && qy >= 0) {
-        const float wxy = weight_of(ax, ox) * weight_of(ay, oy);
-#pragma unroll
-        for (int oz = 0; oz < 4; ++oz) {
-            const int qz = wrap_index(az.base + oz, p.nz, p.wall[2]);
-            if (qz < 0) continue;
-            const float W = wxy * weight_of(az, oz);
-            const float4 v = vel[qx + p.nx * (qy + p.ny * qz)];
-            ux = fmaf(W, v.x, ux);
-            uy = fmaf(W, v.y, uy);
-            uz = fmaf(W, v.z, uz);
+    __syncthreads();
+    int mn[3] = {INT_MAX, INT_MAX, INT_MAX}, mx[3] = {INT_MIN, INT_MIN, INT_MIN};
+    float fmax = 0.f;
+    for (int m = n0 + (int)threadIdx.x; m < n1; m += IB_THREADS) {
+        const int f0 = (int)floor(X[m]), f1 = (int)floor(Y[m]), f2 = (int)floor(Z[m]);
+        mn[0] = min(mn[0], f0); mx[0] = max(mx[0], f0);
+        mn[1] = min(mn[1], f1); mx[1] = max(mx[1], f1);
+        mn[2] = min(mn[2], f2); mx[2] = max(mx[2], f2);
+        if (F) {
+            const float4 f = __ldg(F + m);
+            fmax = fmaxf(fmax, fmaxf(fabsf(f.x), fmaxf(fabsf(f.y), fabsf(f.z))));
         }
     }
-#pragma unroll
-    for (int o = LANES_PER_NODE / 2; o > 0; o >>= 1) {
-        ux += __shfl_xor_sync(0xffffffffu, ux, o);
-        uy += __shfl_xor_sync(0xffffffffu, uy, o);
-        uz += __shfl_xor_sync(0xffffffffu, uz, o);
+    mn[0] = __reduce_min_sync(0xffffffffu, mn[0]); mx[0] = __reduce_max_sync(0xffffffffu, mx[0]);
+    mn[1] = __reduce_min_sync(0xffffffffu, mn[1]); mx[1] = __reduce_max_sync(0xffffffffu, mx[1]);
+    mn[2] = __reduce_min_sync(0xffffffffu, mn[2]); mx[2] = __reduce_max_sync(0xffffffffu, mx[2]);
+    const unsigned fbits = __reduce_max_sync(0xffffffffu, __float_as_uint(fmax));
+    if ((threadIdx.x & 31) == 0) {
+        atomicMin(&T.mn[0], mn[0]); atomicMax(&T.mx[0], mx[0]);
+        atomicMin(&T.mn[1], mn[1]); atomicMax(&T.mx[1], mx[1]);
+        atomicMin(&T.mn[2], mn[2]); atomicMax(&T.mx[2], mx[2]);
+        if (F) atomicMax(&T.fmax_bits, fbits);
     }
-    if (live && sub == 0) {
-        U[m] = make_float4(ux, uy, uz, 0.f);
-        const double xn = xm + (double)ux, yn = ym + (double)uy, zn = zm + (double)uz;
-        X[m] = xn; Y[m] = yn; Z[m] = zn;
-        const bool left = (p.wall[0] && (xn < -0.5 || xn > (double)p.nx - 0.5)) ||
-                          (p.wall[1] && (yn < -0.5 || yn > (double)p.ny - 0.5)) ||
-                          (p.wall[2] && (zn < -0.5 || zn > (double)p.nz - 0.5));
-        if (left) atomicOr(counters + 1, STATUS_NODE_LEFT);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int n[3] = {p.nx, p.ny, p.nz};
+        long long vol = 1;
+        bool ok = n1 > n0;
+        for (int a = 0; a < 3; ++a) {
+            const long long ext = (long long)T.mx[a] - (long long)T.mn[a] + 4;
+            ok = ok && ext <= (long long)cap;
+            T.o[a] = T.mn[a] - 1;
+            T.e[a] = ok ? (int)ext : 1;
+            vol *= T.e[a];
+            ok = ok && vol <= (long long)cap;
+            if (p.wall[a] && ok) {
+                const long long lo = -(long long)T.o[a], hi = (long long)n[a] - (long long)T.o[a];
+                T.lo[a] = (int)max(0LL, min(lo, ext));
+                T.hi[a] = (int)max(0LL, min(hi, ext));
+            } else {
+                T.lo[a] = 0; T.hi[a] = T.e[a];
+            }
+        }
+        T.enabled = ok ? 1 : 0;
+    }
+    __syncthreads();
+}
+
+// global lattice cell of tile cell t (only called for cells inside [lo, hi) on wall axes)
+__device__ __forceinline__ Cell tile_cell(const MeshTile& T, const int t, const LbmParams& p) {
+    const int x = t % T.e[0], r = t / T.e[0];
+    const int y = r % T.e[1], z = r / T.e[1];
+    Cell c;
+    c.i = wrap_index(T.o[0] + x, p.nx, 0);
+    c.j = wrap_index(T.o[1] + y, p.ny, 0);
+    c.k = wrap_index(T.o[2] + z, p.nz, 0);
+    return c;
+}
+
+// per-node stencil records of one chunk of nodes, in shared memory
+struct Chunk {
+    int* b;        // [3][IB_CHUNK] base = floor(X) - 1, tile-relative if the tile is enabled
+    float* sc;     // [6][IB_CHUNK] sin / cos of pi frac / 2 per axis
+};
+
+__device__ __forceinline__ void chunk_record(const Chunk& ch, const MeshTile& T, const bool tiled, const int r,
+                                             const double x, const double y, const double z) {
+    const Axis ax = axis_of(x), ay = axis_of(y), az = axis_of(z);
+    ch.b[r] = tiled ? ax.base - T.o[0] : ax.base;
+    ch.b[IB_CHUNK + r] = tiled ? ay.base - T.o[1] : ay.base;
+    ch.b[2 * IB_CHUNK + r] = tiled ? az.base - T.o[2] : az.base;
+    ch.sc[r] = ax.s; ch.sc[IB_CHUNK + r] = ax.c;
+    ch.sc[2 * IB_CHUNK + r] = ay.s; ch.sc[3 * IB_CHUNK + r] = ay.c;
+    ch.sc[4 * IB_CHUNK + r] = az.s; ch.sc[5 * IB_CHUNK + r] = az.c;
+}
+__device__ __forceinline__ Axis chunk_axis(const Chunk& ch, const int a, const int r) {
+    Axis ax;
+    ax.base = ch.b[a * IB_CHUNK + r];
+    ax.s = ch.sc[2 * a * IB_CHUNK + r];
+    ax.c = ch.sc[(2 * a + 1) * IB_CHUNK + r];
+    return ax;
+}
+
+// S2: g_ijk += F_m phi phi phi (Eq. 34).  Also sets the activity bits of the touched segments.
+__global__ void __launch_bounds__(IB_THREADS) spread_mesh_kernel(
+    const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
+    const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
+    unsigned* __restrict__ seg_mask, const LbmParams p, const int cap) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ MeshTile T;
+    int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point
+    Chunk ch;
+    ch.b = tile + 3 * (size_t)cap;
+    ch.sc = reinterpret_cast<float*>(ch.b + 3 * IB_CHUNK);
+    float* rF = ch.sc + 6 * IB_CHUNK;                                  // [3][IB_CHUNK]
+    const int2 range = __ldg(ranges + blockIdx.x);
+    const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap);
+    const float fmax = __uint_as_float(T.fmax_bits);
+    if (!(fmax > 0.f)) return;                                         // nothing to spread
+    const bool tiled = T.enabled != 0 && fmax < 3.0e38f;
+    const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
+    // |tile value| <= n_nodes * max W * max|F| = bound; scale = 2^k with bound * scale < 2^30
+    const int k = max(-100, min(100, 29 - ilogbf(0.125f * (float)(n1 - n0) * fmax)));
+    const float scale = tiled ? ldexpf(1.0f, k) : 1.0f, inv_scale = ldexpf(1.0f, -k);
+    for (int t = tid; t < ncell; t += IB_THREADS) {
+        tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
+    }
+    const int sub = tid & (LANES_PER_NODE - 1), ox = sub & 3, oy = sub >> 2;
+    for (int c0 = n0; c0 < n1; c0 += IB_CHUNK) {
+        __syncthreads();
+        if (tid < IB_CHUNK && c0 + tid < n1) {
+            const int m = c0 + tid;
+            chunk_record(ch, T, tiled, tid, __ldg(X + m), __ldg(Y + m), __ldg(Z + m));
+            const float4 Fm = __ldg(F + m);
+            rF[tid] = Fm.x * scale; rF[IB_CHUNK + tid] = Fm.y * scale; rF[2 * IB_CHUNK + tid] = Fm.z * scale;
+        }
+        __syncthreads();
+        const int cnt = min(IB_CHUNK, n1 - c0);
+        for (int r = tid / LANES_PER_NODE; r < cnt; r += IB_GROUPS) {
+            const Axis ax = chunk_axis(ch, 0, r), ay = chunk_axis(ch, 1, r), az = chunk_axis(ch, 2, r);
+            const float Fx = rF[r], Fy = rF[IB_CHUNK + r], Fz = rF[2 * IB_CHUNK + r];
+            const float wxy = weight_of(ax, ox) * weight_of(ay, oy);
+            if (tiled) {
+                const int tx = ax.base + ox, ty = ay.base + oy;
+                if (tx < T.lo[0] || tx >= T.hi[0] || ty < T.lo[1] || ty >= T.hi[1]) continue;
+#pragma unroll
+                for (int oz = 0; oz < 4; ++oz) {
+                    const int tz = az.base + oz;
+                    if (tz < T.lo[2] || tz >= T.hi[2]) continue;
+                    const float W = wxy * weight_of(az, oz);
+                    const int t = (tz * e1 + ty) * e0 + tx;
+                    atomicAdd(tile + t, __float2int_rn(W * Fx));
+                    atomicAdd(tile + cap + t, __float2int_rn(W * Fy));
+                    atomicAdd(tile + 2 * cap + t, __float2int_rn(W * Fz));
+                }
+            } else {
+                const int qx = wrap_index(ax.base + ox, p.nx, p.wall[0]);
+                const int qy = wrap_index(ay.base + oy, p.ny, p.wall[1]);
+                if (qx < 0 || qy < 0) continue;
+#pragma unroll
+                for (int oz = 0; oz < 4; ++oz) {
+                    const int qz = wrap_index(az.base + oz, p.nz, p.wall[2]);
+                    if (qz < 0) continue;
+                    const float W = wxy * weight_of(az, oz);
+                    const int cell = qx + p.nx * (qy + p.ny * qz);
+                    atomicAdd(g + cell, make_float4(W * Fx, W * Fy, W * Fz, 0.f));
+                    mark_segment(cell, seg_mask);
+                }
+            }
+        }
+    }
+    if (!tiled) return;
+    __syncthreads();
+    for (int t = tid; t < ncell; t += IB_THREADS) {
+        const int qx = tile[t], qy = tile[cap + t], qz = tile[2 * cap + t];
+        if ((qx | qy | qz) != 0) {
+            const Cell c = tile_cell(T, t, p);
+            const int cell = c.i + p.nx * (c.j + p.ny * c.k);
+            atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
+            mark_segment(cell, seg_mask);
+        }
+    }
+}
+
+// zero the cells of the segments the previous spread touched, and drop their activity bits:
+// one thread per segment (a 128-byte line of the forcing field), one warp per mask word
+__global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ g, unsigned* __restrict__ seg_mask,
+                                                           const int n_segs, const int cells) {
+    const int seg = blockIdx.x * 256 + threadIdx.x;
+    const int word = seg >> 5;
+    const unsigned m = (seg < n_segs) ? seg_mask[word] : 0u;
+    if (__ballot_sync(0xffffffffu, m != 0u) == 0u) return;
+    if ((m >> (seg & 31)) & 1u) {
+        const int c0 = seg * SEG;
+#pragma unroll
+        for (int c = 0; c < SEG; ++c)
+            if (c0 + c < cells) g[c0 + c] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    __syncwarp();
+    if ((seg & 31) == 0 && m != 0u) seg_mask[word] = 0u;
+}
+
+// S4 + S5: U_m = sum v phi phi phi (Eq. 33) with v = (sum c_i f_i + g/2)/rho of the state after
+// lbm_step (G11), by a 16-lane shuffle reduction over the 4x4x4 stencil, then
+// X_m += U_m in fp64.
+__global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
+    double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z, float4* __restrict__ U,
+    const int2* __restrict__ ranges, const float* __restrict__ src, const float4* __restrict__ g,
+    int* __restrict__ counters, const LbmParams p, const int cap) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ MeshTile T;
+    float* tile = reinterpret_cast<float*>(smem_raw);                  // [3][cap] velocity
+    Chunk ch;
+    ch.b = reinterpret_cast<int*>(tile + 3 * (size_t)cap);
+    ch.sc = reinterpret_cast<float*>(ch.b + 3 * IB_CHUNK);
+    unsigned short* list = reinterpret_cast<unsigned short*>(ch.sc + 6 * IB_CHUNK);   // [cap] needed tile cells
+    const int2 range = __ldg(ranges + blockIdx.x);
+    const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
+    tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap);
+    const bool tiled = T.enabled != 0;
+    const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
+    if (tiled) {
+        unsigned* need = reinterpret_cast<unsigned*>(tile);           // marks live in the x plane of the tile
+        for (int t = tid; t < ncell; t += IB_THREADS) need[t] = 0u;
+        __syncthreads();
+        for (int m = n0 + tid; m < n1; m += IB_THREADS) {             // the 4^3 cells each node needs
+            const int bx = (int)floor(X[m]) - 1 - T.o[0], by = (int)floor(Y[m]) - 1 - T.o[1],
+                      bz = (int)floor(Z[m]) - 1 - T.o[2];
+            for (int oz = 0; oz < 4; ++oz) {
+                const int tz = bz + oz;
+                if (tz < T.lo[2] || tz >= T.hi[2]) continue;
+                for (int oy = 0; oy < 4; ++oy) {
+                    const int ty = by + oy;
+                    if (ty < T.lo[1] || ty >= T.hi[1]) continue;
+                    const int row = (tz * e1 + ty) * e0;
+#pragma unroll
+                    for (int ox = 0; ox < 4; ++ox) {
+                        const int tx = bx + ox;
+                        if (tx >= T.lo[0] && tx < T.hi[0]) need[row + tx] = 1u;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        // compact the needed cells so that every lane of the moment pass has a cell
+        for (int t0 = 0; t0 < ncell; t0 += IB_THREADS) {
+            const int t = t0 + tid;
+            const bool want = t < ncell && need[t] != 0u;
+            const unsigned vote = __ballot_sync(0xffffffffu, want);
+            int base = 0;
+            if ((tid & 31) == 0 && vote) base = atomicAdd(&T.n_need, __popc(vote));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (want) list[base + __popc(vote & ((1u << (tid & 31)) - 1u))] = (unsigned short)t;
+        }
+        __syncthreads();
+        const int n_need = T.n_need;
+        for (int e = tid; e < n_need; e += IB_THREADS) {
+            const int t = list[e];
+            const float4 v = cell_macros(src, g, p, tile_cell(T, t, p));
+            tile[t] = v.x; tile[cap + t] = v.y; tile[2 * cap + t] = v.z;
+        }
+    }
+    const int sub = tid & (LANES_PER_NODE - 1), ox = sub & 3, oy = sub >> 2;
+    for (int c0 = n0; c0 < n1; c0 += IB_CHUNK) {
+        __syncthreads();
+        if (tid < IB_CHUNK && c0 + tid < n1) {
+            const int m = c0 + tid;
+            chunk_record(ch, T, tiled, tid, X[m], Y[m], Z[m]);
+        }
+        __syncthreads();
+        const int cnt = min(IB_CHUNK, n1 - c0);
+        // the 16 lanes of a node iterate together: r is the same for a whole half-warp
+        for (int r = tid / LANES_PER_NODE; r < cnt; r += IB_GROUPS) {
+            const Axis ax = chunk_axis(ch, 0, r), ay = chunk_axis(ch, 1, r), az = chunk_axis(ch, 2, r);
+            const float wxy = weight_of(ax, ox) * weight_of(ay, oy);
+            float ux = 0.f, uy = 0.f, uz = 0.f;
+            if (tiled) {
+                const int tx = ax.base + ox, ty = ay.base + oy;
+                if (tx >= T.lo[0] && tx < T.hi[0] && ty >= T.lo[1] && ty < T.hi[1]) {
+#pragma unroll
+                    for (int oz = 0; oz < 4; ++oz) {
+                        const int tz = az.base + oz;
+                        if (tz < T.lo[2] || tz >= T.hi[2]) continue;
+                        const float W = wxy * weight_of(az, oz);
+                        const int t = (tz * e1 + ty) * e0 + tx;
+                        ux = fmaf(W, tile[t], ux);
+                        uy = fmaf(W, tile[cap + t], uy);
+                        uz = fmaf(W, tile[2 * cap + t], uz);
+                    }
+                }
+            } else {
+                const int qx = wrap_index(ax.base + ox, p.nx, p.wall[0]);
+                const int qy = wrap_index(ay.base + oy, p.ny, p.wall[1]);
+                if (qx >= 0 && qy >= 0) {
+                    for (int oz = 0; oz < 4; ++oz) {
+                        const int qz = wrap_index(az.base + oz, p.nz, p.wall[2]);
+                        if (qz < 0) continue;
+                        const float W = wxy * weight_of(az, oz);
+                        Cell c;
+                        c.i = qx; c.j = qy; c.k = qz;
+                        const float4 v = cell_macros(src, g, p, c);
+                        ux = fmaf(W, v.x, ux);
+                        uy = fmaf(W, v.y, uy);
+                        uz = fmaf(W, v.z, uz);
+                    }
+                }
+            }
+            const unsigned half = 0xffffu << (threadIdx.x & 16);
+#pragma unroll
+            for (int o = LANES_PER_NODE / 2; o > 0; o >>= 1) {
+                ux += __shfl_xor_sync(half, ux, o);
+                uy += __shfl_xor_sync(half, uy, o);
+                uz += __shfl_xor_sync(half, uz, o);
+            }
+            if (sub == 0) {
+                const int m = c0 + r;
+                U[m] = make_float4(ux, uy, uz, 0.f);
+                const double xn = X[m] + (double)ux, yn = Y[m] + (double)uy, zn = Z[m] + (double)uz;
+                X[m] = xn; Y[m] = yn; Z[m] = zn;
+                const bool left = (p.wall[0] && (xn < -0.5 || xn > (double)p.nx - 0.5)) ||
+                                  (p.wall[1] && (yn < -0.5 || yn > (double)p.ny - 0.5)) ||
+                                  (p.wall[2] && (zn < -0.5 || zn > (double)p.nz - 0.5));
+                if (left) atomicOr(counters + 1, STATUS_NODE_LEFT);
+            }
+        }
     }
 }
 
@@ -220,29 +480,46 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
 }
 
 int launch_clear_spread(Ctx* c, float4* g) {
-    clear_spread_kernel<<<c->sm_count * 8, 256, 0, c->stream>>>(g, c->seg_mask, c->seg_list, c->counters, c->prm.cells);
+    clear_spread_kernel<<<(unsigned)((c->n_segs + 255) / 256), 256, 0, c->stream>>>(g, c->seg_mask, (int)c->n_segs,
+                                                                                  c->prm.cells);
     c->launches++;
-    int rc = cuda_check(cudaGetLastError(), "clear_spread_kernel");
-    if (rc) return rc;
-    return cuda_check(cudaMemsetAsync(c->counters, 0, sizeof(int), c->stream), "reset segment counter");
+    return cuda_check(cudaGetLastError(), "clear_spread_kernel");
+}
+
+static size_t spread_smem(int cap) { return (size_t)cap * 12 + (size_t)IB_CHUNK * 48; }
+static size_t interp_smem(int cap) { return (size_t)cap * 12 + (size_t)IB_CHUNK * 36 + (((size_t)cap * 2 + 15) & ~(size_t)15); }
+
+// Largest tile (in cells) both kernels can hold with at least one block per SM; a tile cell index
+// must also fit the 16-bit entries of the interpolation's compact list.
+int ib_max_tile_cap() {
+    const size_t budget = 200 * 1024;
+    const size_t cap = (budget - (size_t)IB_CHUNK * 48 - 64) / 14;
+    return (int)(cap < 65535 ? cap : 65535);
 }
 
 int launch_spread(Ctx* c, float4* g) {
     if (c->n_nodes == 0) return PLB_OK;
-    const long threads = c->n_nodes * LANES_PER_NODE;
-    spread_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->F, c->n_nodes, g, c->seg_mask, c->seg_list, c->counters, c->prm);
+    const size_t smem = spread_smem(c->tile_cap);
+    int rc = cuda_check(cudaFuncSetAttribute(spread_mesh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                        "cudaFuncSetAttribute(spread_mesh_kernel)");
+    if (rc) return rc;
+    spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+        c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->prm, c->tile_cap);
     c->launches++;
-    return cuda_check(cudaGetLastError(), "spread_kernel");
+    return cuda_check(cudaGetLastError(), "spread_mesh_kernel");
 }
 
 int launch_interpolate_advance(Ctx* c) {
     if (c->n_nodes == 0) return PLB_OK;
-    const long threads = c->n_nodes * LANES_PER_NODE;
-    interpolate_advance_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->U, c->n_nodes, c->vel, c->counters, c->prm);
+    const size_t smem = interp_smem(c->tile_cap);
+    int rc = cuda_check(cudaFuncSetAttribute(interpolate_mesh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                        "cudaFuncSetAttribute(interpolate_mesh_kernel)");
+    if (rc) return rc;
+    const float4* g = (c->g_last_mode == FORCE_NONE) ? nullptr : c->g_last;
+    interpolate_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+        c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->f[c->cur], g, c->counters, c->prm, c->tile_cap);
     c->launches++;
-    return cuda_check(cudaGetLastError(), "interpolate_advance_kernel");
+    return cuda_check(cudaGetLastError(), "interpolate_mesh_kernel");
 }
 
 int launch_nodes_transpose(Ctx* c, bool to_aos) {

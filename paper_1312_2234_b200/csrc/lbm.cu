@@ -9,80 +9,9 @@
 // so one fused kernel does pull-stream -> moments -> BGK + Guo forcing -> aligned store.
 // The w_d shift keeps |stored value| ~ 1e-2 so that fp32 holds |d rho| <= 1e-6.
 #include "plb_internal.cuh"
+#include "lbm_device.cuh"
 
 namespace plb {
-
-struct Cell {
-    int i, j, k;
-};
-
-__device__ __forceinline__ Cell cell_of(int idx, const LbmParams& p) {
-    Cell c;
-    const unsigned t = (unsigned)idx / (unsigned)p.nx;
-    c.i = (int)((unsigned)idx - t * (unsigned)p.nx);
-    c.k = (int)(t / (unsigned)p.ny);
-    c.j = (int)(t - (unsigned)c.k * (unsigned)p.ny);
-    return c;
-}
-
-// Pull the 19 streamed populations (minus w_d) of cell (i,j,k) out of the pre-stream lattice
-// into column COL of h.  Generic in the boundary kinds of all three axes.
-template <int V, int COL>
-__device__ __forceinline__ void pull19(const float* __restrict__ src, const LbmParams& p, const Cell c,
-                                       const int idx, float (&h)[Q][V]) {
-    const int nx = p.nx, ny = p.ny, nz = p.nz;
-    const size_t N = (size_t)p.cells;
-    const bool xlo = c.i == 0, xhi = c.i == nx - 1;
-    const bool ylo = c.j == 0, yhi = c.j == ny - 1;
-    const bool zlo = c.k == 0, zhi = c.k == nz - 1;
-    // neighbour offsets with periodic wrap (a wall axis bounces instead, decided below)
-    const int dxm = xlo ? nx - 1 : -1, dxp = xhi ? 1 - nx : 1;
-    const int dym = (ylo ? ny - 1 : -1) * nx, dyp = (yhi ? 1 - ny : 1) * nx;
-    const int dzm = (zlo ? nz - 1 : -1) * nx * ny, dzp = (zhi ? 1 - nz : 1) * nx * ny;
-    const bool bxlo = p.wall[0] && xlo, bxhi = p.wall[0] && xhi;
-    const bool bylo = p.wall[1] && ylo, byhi = p.wall[1] && yhi;
-    const bool bzlo = p.wall[2] && zlo, bzhi = p.wall[2] && zhi;
-#pragma unroll
-    for (int d = 0; d < Q; ++d) {
-        const int cx = CX(d), cy = CY(d), cz = CZ(d);
-        // source cell x - c_d
-        int off = 0;
-        if (cx == 1) off += dxm;
-        if (cx == -1) off += dxp;
-        if (cy == 1) off += dym;
-        if (cy == -1) off += dyp;
-        if (cz == 1) off += dzm;
-        if (cz == -1) off += dzp;
-        // bounce-back: x - c_d lies beyond a wall face; z, y, x in this order so that x wins
-        bool b = false;
-        float corr = 0.f;
-        if (cz == 1 && bzlo) { b = true; corr = p.corr[2][0][d]; }
-        if (cz == -1 && bzhi) { b = true; corr = p.corr[2][1][d]; }
-        if (cy == 1 && bylo) { b = true; corr = p.corr[1][0][d]; }
-        if (cy == -1 && byhi) { b = true; corr = p.corr[1][1][d]; }
-        if (cx == 1 && bxlo) { b = true; corr = p.corr[0][0][d]; }
-        if (cx == -1 && bxhi) { b = true; corr = p.corr[0][1][d]; }
-        if (b) h[d][COL] = __ldg(src + (size_t)OPP(d) * N + idx) + corr;
-        else   h[d][COL] = __ldg(src + (size_t)d * N + (idx + off));
-    }
-}
-
-// delta rho = sum h_d, j = sum c_d h_d (Eq. 17-18; sum_d w_d c_d = 0 so the shift drops out of j)
-template <int V, int COL>
-__device__ __forceinline__ void moments(const float (&h)[Q][V], float& drho, float& jx, float& jy, float& jz) {
-    // pairwise sums keep the fp32 rounding small and symmetric
-    const float a01p = h[0][COL] + h[1][COL], a23p = h[2][COL] + h[3][COL], a45p = h[4][COL] + h[5][COL];
-    const float s6 = (h[6][COL] + h[11][COL]) + (h[7][COL] + h[10][COL]);      // xy diagonals
-    const float s8 = (h[8][COL] + h[13][COL]) + (h[9][COL] + h[12][COL]);      // xz diagonals
-    const float s14 = (h[14][COL] + h[17][COL]) + (h[15][COL] + h[16][COL]);   // yz diagonals
-    drho = ((a01p + a23p) + (a45p + h[18][COL])) + ((s6 + s8) + s14);
-    const float d611 = h[6][COL] - h[11][COL], d710 = h[7][COL] - h[10][COL];
-    const float d813 = h[8][COL] - h[13][COL], d912 = h[9][COL] - h[12][COL];
-    const float d1417 = h[14][COL] - h[17][COL], d1516 = h[15][COL] - h[16][COL];
-    jx = (h[0][COL] - h[1][COL]) + ((d611 + d710) + (d813 + d912));
-    jy = (h[2][COL] - h[3][COL]) + ((d611 - d710) + (d1417 + d1516));
-    jz = (h[4][COL] - h[5][COL]) + ((d813 - d912) + (d1417 - d1516));
-}
 
 // BGK relaxation (Eq. 16) towards f_eq(rho, v) (Eq. 20) with v = u + g/(2 rho) (L201) plus the
 // Guo term (Eq. 19 in the form S_d = (1 - 1/2tau) w_d [3 (c_d - v).g + 9 (c_d.v)(c_d.g)],
@@ -338,33 +267,6 @@ __global__ void __launch_bounds__(256) macros_kernel(const float* __restrict__ s
     }
 }
 
-// The same moments, only over the segments the last ib_spread touched (the 4^3 supports of the
-// nodes), written as float4 (vx, vy, vz, rho) for the interpolation gather.
-template <int MODE>
-__global__ void __launch_bounds__(256) sparse_moments_kernel(const float* __restrict__ src,
-                                                             const float4* __restrict__ g,
-                                                             const int* __restrict__ seg_list,
-                                                             const int* __restrict__ counters,
-                                                             float4* __restrict__ vel, const LbmParams p) {
-    const int sub = threadIdx.x & (SEG - 1);
-    const int group = (blockIdx.x * 256 + threadIdx.x) >> SEG_SHIFT;
-    const int n_groups = (gridDim.x * 256) >> SEG_SHIFT;
-    const int n_active = __ldg(counters);
-    for (int s = group; s < n_active; s += n_groups) {
-        const int idx = __ldg(seg_list + s) * SEG + sub;
-        if (idx >= p.cells) continue;
-        const Cell c = cell_of(idx, p);
-        float h[Q][1];
-        pull19<1, 0>(src, p, c, idx, h);
-        float drho, jx, jy, jz;
-        moments<1, 0>(h, drho, jx, jy, jz);
-        float4 g4 = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (MODE != FORCE_NONE) g4 = __ldg(g + idx);
-        const float rho = 1.0f + drho, inv = 1.0f / rho;
-        vel[idx] = make_float4((jx + 0.5f * g4.x) * inv, (jy + 0.5f * g4.y) * inv, (jz + 0.5f * g4.z) * inv, rho);
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 // initialisation / checkpoint kernels (off the timed path).  They write the pre-stream state T:
 //   T_d(x) = f_d(x + c_d)                               (interior / periodic)
@@ -506,17 +408,6 @@ int launch_read_macros(Ctx* c, float* d_rho, float* d_u) {
         macros_kernel<FORCE_SPARSE><<<grid, 256, 0, c->stream>>>(src, c->g_last, c->seg_mask, d_rho, d_u, c->prm);
     c->launches++;
     return cuda_check(cudaGetLastError(), "macros_kernel");
-}
-
-int launch_sparse_moments(Ctx* c) {
-    const float* src = c->f[c->cur];
-    const int grid = c->sm_count * 8;
-    if (c->g_last_mode == FORCE_NONE || !c->g_last)
-        sparse_moments_kernel<FORCE_NONE><<<grid, 256, 0, c->stream>>>(src, nullptr, c->seg_list, c->counters, c->vel, c->prm);
-    else
-        sparse_moments_kernel<FORCE_DENSE><<<grid, 256, 0, c->stream>>>(src, c->g_last, c->seg_list, c->counters, c->vel, c->prm);
-    c->launches++;
-    return cuda_check(cudaGetLastError(), "sparse_moments_kernel");
 }
 
 int launch_read_populations(Ctx* c, float* d_f) {

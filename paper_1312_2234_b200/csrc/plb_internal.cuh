@@ -11,7 +11,7 @@ namespace plb {
 constexpr int Q = 19;
 // Activity segments: 8 consecutive cells (one 128-byte line of the float4 forcing field, one
 // 32-byte sector of a population row).  Bit (s & 31) of seg_mask[s >> 5] is set while segment s
-// holds spread force; seg_list enumerates the set bits.
+// holds spread force.
 constexpr int SEG = 8;
 constexpr int SEG_SHIFT = 3;
 
@@ -92,10 +92,8 @@ struct Ctx {
     // lattice (carved from the workspace)
     float* f[2];
     int cur;
-    float4* vel;               // (vx, vy, vz, rho) at the active cells, cells entries
     unsigned* seg_mask;        // one bit per segment, (n_segs + 31) / 32 words
-    int* seg_list;             // n_segs
-    int* counters;             // [0] active segment count, [1] status bits
+    int* counters;             // [1] status bits
     // meshes
     long cap_nodes, cap_edges, n_nodes, n_edges;
     double* X[3];              // SoA fp64 unwrapped positions
@@ -105,6 +103,9 @@ struct Ctx {
     int2* edges;               // global node index pairs
     float2* edge_prm;          // (rest length, k)
     std::vector<long> mesh_node_off, mesh_edge_off;
+    int2* ranges;              // node ranges [first, last) served by one thread block of the IB kernels
+    long n_ranges;
+    int tile_cap;              // cells of the shared-memory lattice tile of the IB kernels
     // bookkeeping
     const float4* g_last;
     int g_last_mode;           // ForceMode used by the last lbm_step
@@ -125,11 +126,11 @@ int launch_lbm_step(Ctx* c, const float4* g, int mode);
 int launch_read_macros(Ctx* c, float* d_rho, float* d_u);
 int launch_read_populations(Ctx* c, float* d_f);
 int launch_write_populations(Ctx* c, const float* d_f);
-int launch_sparse_moments(Ctx* c);
 int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigned long long step);
 int launch_clear_spread(Ctx* c, float4* g);
 int launch_spread(Ctx* c, float4* g);
 int launch_interpolate_advance(Ctx* c);
+int ib_max_tile_cap();
 int launch_nodes_transpose(Ctx* c, bool to_aos);
 int launch_philox(cudaStream_t s, long n, const unsigned* ctr, const unsigned* key, unsigned* out);
 
