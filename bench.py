@@ -39,7 +39,7 @@ NOMINAL_HBM_GBS = 8000.0
 def parse_args(argv=None):
     p = argparse.ArgumentParser()
     p.add_argument("--gpus", type=int, default=1)
-    p.add_argument("--steps", type=int, default=50)
+    p.add_argument("--steps", type=int, default=500, help="timed coupled steps (default: config 4's own 500)")
     p.add_argument("--warmup", type=int, default=5)
     p.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -112,45 +112,101 @@ def barrier(device):
 # clocks during the timed region (B200_PROFILING.md)
 # ---------------------------------------------------------------------------------------------
 class ClockSampler:
-    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-              "clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons of one GPU, sampled every 20 ms by a thread (NVML, the same
+    counters `nvidia-smi --query-gpu=clocks.sm,clocks.max.sm,clocks_event_reasons.*` prints);
+    falls back to an `nvidia-smi -lms` child process when pynvml is missing.  Sampling runs from
+    start() to stop(); mark() opens the timed region, only samples after it are reported."""
+    SMI_FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+                  "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+                  "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
 
     def __init__(self, gpu_index):
-        self.proc = None
+        import threading
+        self.samples = []          # (t, sm_mhz, set of reasons)
+        self.sm_max = None
+        self.t_mark = None
+        self.how = None
+        self._stop = threading.Event()
+        self._thread = None
+        self._proc = None
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.FIELDS,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = gpu_index
+            if vis:
+                ids = [v.strip() for v in vis.split(",") if v.strip()]
+                if gpu_index < len(ids) and ids[gpu_index].isdigit():
+                    phys = int(ids[gpu_index])
+            h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            bits = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+
+            def poll():
+                while not self._stop.is_set():
+                    try:
+                        mhz = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                        r = int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                        self.samples.append((time.perf_counter(), mhz, {n for n, b in bits.items() if r & b}))
+                    except Exception:
+                        pass
+                    self._stop.wait(0.02)
+            self._thread = threading.Thread(target=poll, daemon=True)
+            self._thread.start()
+            self.how = "nvml, 20 ms"
+        except Exception:
+            self._start_smi(gpu_index)
+
+    def _start_smi(self, gpu_index):
+        import threading
+        try:
+            self._proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.SMI_FIELDS,
+                                           "--format=csv,noheader,nounits", "-lms", "50"],
+                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
-            self.proc = None
+            self._proc = None
+            return
+
+        def read():
+            for line in self._proc.stdout:
+                parts = [p.strip() for p in line.split(",")]
+                if len(parts) < 7:
+                    continue
+                try:
+                    mhz, mx = float(parts[0]), float(parts[1])
+                except ValueError:
+                    continue
+                self.sm_max = mx
+                self.samples.append((time.perf_counter(), mhz,
+                                     {n for n, v in zip(self.NAMES, parts[3:7]) if v.lower().startswith("active")}))
+        self._thread = threading.Thread(target=read, daemon=True)
+        self._thread.start()
+        self.how = "nvidia-smi -lms 50"
+
+    def mark(self):
+        self.t_mark = time.perf_counter()
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.proc is None:
-            return out
-        self.proc.terminate()
-        try:
-            text, _ = self.proc.communicate(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-            text, _ = self.proc.communicate()
-        sm, mx, reasons = [], [], set()
-        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for line in text.splitlines():
-            parts = [p.strip() for p in line.split(",")]
-            if len(parts) < 7:
-                continue
+        t_end = time.perf_counter()
+        self._stop.set()
+        if self._proc is not None:
+            self._proc.terminate()
             try:
-                sm.append(float(parts[0])); mx.append(float(parts[1]))
-            except ValueError:
-                continue
-            for name, val in zip(names, parts[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
-        if sm:
-            sm.sort()
-            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+                self._proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self._proc.kill()
+        if self._thread is not None:
+            self._thread.join(timeout=5)
+        t0 = self.t_mark if self.t_mark is not None else 0.0
+        inside = [s for s in self.samples if t0 <= s[0] <= t_end]
+        out = {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": len(inside), "how": self.how}
+        if inside:
+            sm = sorted(s[1] for s in inside)
+            reasons = set()
+            for s in inside:
+                reasons |= s[2]
+            out.update(sm_mhz=sm[len(sm) // 2], reasons=sorted(reasons))
         return out
 
 
@@ -286,13 +342,14 @@ def run_ours(args):
             if marks is not None: marks[3].record()
 
     # ---- device-resident leg: inputs already in HBM, CUDA events on the launching stream
+    clocks = ClockSampler(device.index)
     for s in range(W):
         one_step(s)
     marks = [[ev() for _ in range(5)] for _ in range(K)]
     t_beg, t_end = ev(), ev()
     barrier(device)
     launches0 = sim.launch_count()
-    clocks = ClockSampler(device.index)
+    clocks.mark()
     t_beg.record()
     for s in range(K):
         one_step(W + s, marks[s])
@@ -338,7 +395,7 @@ def run_ours(args):
         "step_ms_rank0": step_ms,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cb, _, _ = time_oracle(args.config, 10, 1)
+        cb, _, _ = time_oracle(args.config, 100 if args.config == 4 else 20, 2)
         line["cpu_baseline"] = cb
     elif rank == 0:
         line["cpu_baseline"] = None

@@ -148,6 +148,23 @@ def test_config5_full_size_block_and_invariants():
     print("C5 full-size block", full_size_block_parity(w, steps=1, inner=8, mesh_id=4000))
 
 
-@pytest.mark.skipif(not FULL, reason="full-length C3 oracle run takes minutes of CPU time (PLB_FULL=1)")
-def test_config3_full_length():
-    print("C3 full", run_and_compare(wl.config3()))
+def record(name, w, out):
+    """print the parity maxima; append them to $PLB_RESULTS (a text file) when set"""
+    line = "%s %dx%dx%d nodes=%d steps=%d  max|drho|=%.3g  max|dv|/u_ref=%.3g  max|dX|=%s" % (
+        name, w.nx, w.ny, w.nz, w.n_nodes, w.steps, out["drho"], out["dv_rel"],
+        ("%.3g" % out["dX"]) if "dX" in out else "-")
+    print(line)
+    path = os.environ.get("PLB_RESULTS")
+    if path:
+        with open(path, "a") as fh:
+            fh.write(line + "\n")
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(not FULL, reason="full-length, full-size oracle runs take minutes to an hour of CPU time (PLB_FULL=1)")
+@pytest.mark.parametrize("cfg", [3, 5, 4])
+def test_config_full_length_full_size(cfg):
+    """the whole configured run (C3: 2000 steps, C5: 200, C4: 500) at full size against the fp64
+    oracle, at the north_star tolerances (C4 needs ~25 GB of host memory for the oracle)"""
+    w = wl.config(cfg)
+    record("C%d full" % cfg, w, run_and_compare(w))
