@@ -138,7 +138,13 @@ int orc_create(int nx, int ny, int nz, double tau, const int kind[3], const doub
     c->cells = (long)nx * ny * nz;
     c->tau = (real)tau;
     for (int a = 0; a < 3; ++a) {
-        if (kind[a] != ORC_PERIODIC && kind[a] != ORC_WALL) { free(c); return -1; }
+        if (kind[a] != ORC_PERIODIC && kind[a] != ORC_WALL && kind[a] != ORC_WALL_HH) { free(c); return -1; }
+        /* NEXT-1: the on-site condition is written for a plane (L217); edges and corners where
+         * two closed axes meet are not defined by the paper -> the other two axes must be periodic */
+        if (kind[a] == ORC_WALL_HH && (a == 0 ? nx : a == 1 ? ny : nz) < 2) { free(c); return -1; }
+        if (kind[a] == ORC_WALL_HH)
+            for (int b = 0; b < 3; ++b)
+                if (b != a && kind[b] != ORC_PERIODIC) { free(c); return -1; }
         c->kind[a] = kind[a];
         for (int d = 0; d < 3; ++d) {
             c->u_lo[a][d] = u_lo ? (real)u_lo[3 * a + d] : 0;
@@ -161,6 +167,8 @@ int orc_destroy(orc_ctx* c) {
     return 0;
 }
 
+static void hecht_harting_faces(orc_ctx* c);   /* NEXT-1, below */
+
 /* O-2: f_i = feq_i(rho, u) (Eq. 20) + amp (2 xi - 1), xi = Philox uniform keyed on
  * (index = cell*19 + (i-1), step 0, tag 1), first output word. */
 int orc_set_equilibrium(orc_ctx* c, const double* rho, const double* u, double amp, uint64_t seed) {
@@ -180,6 +188,7 @@ int orc_set_equilibrium(orc_ctx* c, const double* rho, const double* u, double a
         }
     }
     memset(c->g_last, 0, (size_t)3 * N * sizeof(real));
+    hecht_harting_faces(c);
     return 0;
 }
 
@@ -200,6 +209,69 @@ static void collide_cell(const orc_ctx* c, const real fin[Q], const real g[3], r
         real cmv_g = (C[i][0] - v[0]) * g[0] + (C[i][1] - v[1]) * g[1] + (C[i][2] - v[2]) * g[2];
         real S = ((real)1 - (real)1 / (2 * c->tau)) * (real)weight(i) * ((real)3 * cmv_g + (real)9 * cv * cg);
         fout[i] = fin[i] - (fin[i] - feq(i, rho, v)) / c->tau + S;
+    }
+}
+
+/* NEXT-1.  Hecht-Harting on-site velocity boundary (the paper's ref. [34]; Eq. 23-30).
+ * The paper prints the plane z = 0 (inward normal n = +z): the populations with c.n = +1
+ * (i = 5, 9, 13, 15, 17) are undetermined after streaming and, with the wall velocity v,
+ *     rho  = [ sum_{c.n = 0} f_i + 2 sum_{c.n = -1} f_i ] / (1 - v.n)                 (first line of L219)
+ *     f_5  = f_6  + rho v_z / 3
+ *     f_9  = f_14 + rho (v_z + v_x)/6 - N_x     f_13 = f_10 + rho (v_z - v_x)/6 + N_x   (Eq. 25-26; "rho/eps" read rho/6, G5)
+ *     f_15 = f_18 + rho (v_z + v_y)/6 - N_y     f_17 = f_16 + rho (v_z - v_y)/6 + N_y   (Eq. 27-28)
+ *     N_t  = (1/2) [ sum_{c.n=0, c.t=+1} f_i - sum_{c.n=0, c.t=-1} f_i ] - rho v_t / 3   (Eq. 29-30)
+ * Any other face is the same statement with the axes renamed: n = inward unit normal
+ * (+e_a on the low face of axis a, -e_a on the high face), t runs over the two tangential axes,
+ * and an unknown population with c = n + s t (s = +-1) is  f_opp + rho (v.n + s v_t)/6 - s N_t.
+ * Paper-literal: the condition sets sum c_i f_i = rho v; a body force at the wall node enters
+ * only through the usual g/2 of the collision and of lbm_read_macros (reading G24). */
+static void hecht_harting_cell(real f[Q], int a, int face, const real vw[3]) {
+    const int sgn = face ? -1 : +1;                     /* n = sgn e_a */
+    const real vn = (real)sgn * vw[a];
+    real S0 = 0, Sm = 0, T[3] = {0, 0, 0};
+    for (int i = 0; i < Q; ++i) {
+        const int cn = sgn * C[i][a];
+        if (cn == 0) {
+            S0 += f[i];
+            for (int b = 0; b < 3; ++b) T[b] += C[i][b] * f[i];
+        } else if (cn == -1) Sm += f[i];
+    }
+    const real rho = (S0 + 2 * Sm) / ((real)1 - vn);
+    real N[3];
+    for (int b = 0; b < 3; ++b) N[b] = T[b] / 2 - rho * vw[b] / 3;
+    for (int i = 0; i < Q; ++i) {
+        if (sgn * C[i][a] != 1) continue;
+        int b = -1;
+        for (int d = 0; d < 3; ++d)
+            if (d != a && C[i][d] != 0) b = d;
+        if (b < 0) f[i] = f[OPP[i]] + rho * vn / 3;
+        else f[i] = f[OPP[i]] + rho * (vn + C[i][b] * vw[b]) / 6 - C[i][b] * N[b];
+    }
+}
+
+/* NEXT-1: on an on-site velocity wall the populations pointing into the fluid do not arrive by
+ * streaming ("undetermined", L217); they are filled from the others (Eq. 23-30) after every
+ * streaming step -- and after lbm_set_equilibrium / lbm_write_populations, so that the stored
+ * state always satisfies the wall condition (reading G25). */
+static void hecht_harting_faces(orc_ctx* c) {
+    const int nx = c->n[0], ny = c->n[1];
+    for (int a = 0; a < 3; ++a) {
+        if (c->kind[a] != ORC_WALL_HH) continue;
+        for (int face = 0; face < 2; ++face) {
+            const int b1 = (a + 1) % 3, b2 = (a + 2) % 3;
+#pragma omp parallel for schedule(static)
+            for (int s2 = 0; s2 < c->n[b2]; ++s2)
+                for (int s1 = 0; s1 < c->n[b1]; ++s1) {
+                    int xs[3];
+                    xs[a] = face ? c->n[a] - 1 : 0;
+                    xs[b1] = s1; xs[b2] = s2;
+                    const long q = xs[0] + (long)nx * (xs[1] + (long)ny * xs[2]);
+                    real fq[Q];
+                    for (int i = 0; i < Q; ++i) fq[i] = c->f[FI(i, q)];
+                    hecht_harting_cell(fq, a, face, face ? c->u_hi[a] : c->u_lo[a]);
+                    for (int i = 0; i < Q; ++i) c->f[FI(i, q)] = fq[i];
+                }
+        }
     }
 }
 
@@ -228,19 +300,22 @@ int orc_step(orc_ctx* c, const double* g) {
                 const long q = x + (long)nx * (y + (long)ny * z);
                 const int xs[3] = {x, y, z};
                 for (int i = 0; i < Q; ++i) {
-                    int xp[3];
+                    int xp[3], leaves = 0;
                     const real* uw = NULL;
                     for (int a = 0; a < 3; ++a) {
                         xp[a] = xs[a] + C[i][a];
                         if (xp[a] < 0) {
                             if (c->kind[a] == ORC_PERIODIC) xp[a] += c->n[a];
+                            else if (c->kind[a] == ORC_WALL_HH) leaves = 1;
                             else if (!uw) uw = c->u_lo[a];
                         } else if (xp[a] >= c->n[a]) {
                             if (c->kind[a] == ORC_PERIODIC) xp[a] -= c->n[a];
+                            else if (c->kind[a] == ORC_WALL_HH) leaves = 1;
                             else if (!uw) uw = c->u_hi[a];
                         }
                     }
                     const real fs = c->fstar[FI(i, q)];
+                    if (leaves) continue;      /* on-site wall: the population leaves the domain */
                     if (uw) {
                         real cu = C[i][0] * uw[0] + C[i][1] * uw[1] + C[i][2] * uw[2];
                         c->f[FI(OPP[i], q)] = fs - (real)6 * (real)weight(i) * (real)1 * cu;
@@ -250,6 +325,7 @@ int orc_step(orc_ctx* c, const double* g) {
                     }
                 }
             }
+    hecht_harting_faces(c);
     return 0;
 }
 
@@ -281,6 +357,7 @@ int orc_write_populations(orc_ctx* c, const double* f) {
     if (!c || !f) return -1;
     for (int i = 0; i < Q; ++i)
         for (long q = 0; q < c->cells; ++q) c->f[FI(i, q)] = (real)f[(size_t)i * c->cells + q];
+    hecht_harting_faces(c);
     return 0;
 }
 
@@ -478,6 +555,9 @@ int orc_interpolate_advance(orc_ctx* c) {
             c->X[3 * m + d] += c->U[3 * m + d];
             if (c->kind[d] == ORC_WALL &&
                 (c->X[3 * m + d] < (real)-0.5 || c->X[3 * m + d] > (real)c->n[d] - (real)0.5))
+                left = 1;
+            if (c->kind[d] == ORC_WALL_HH &&        /* on-site walls lie ON layers 0 and n - 1 */
+                (c->X[3 * m + d] < (real)0 || c->X[3 * m + d] > (real)c->n[d] - (real)1))
                 left = 1;
         }
     c->forces_valid = 0;

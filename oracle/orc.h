@@ -22,7 +22,10 @@ extern "C" {
 
 typedef struct orc_ctx orc_ctx;
 
-enum { ORC_PERIODIC = 0, ORC_WALL = 1 };
+/* ORC_WALL: halfway bounce-back + Ladd term (configs, G9).  ORC_WALL_HH: the paper's own wall, the
+ * Hecht-Harting on-site velocity condition (Eq. 23-30): wall ON the first/last layer; the other two
+ * axes must be periodic. */
+enum { ORC_PERIODIC = 0, ORC_WALL = 1, ORC_WALL_HH = 2 };
 
 /* lattice constants: c[19][3] and w[19] in the paper's order (Eq. 21, Eq. 23-30) */
 void orc_lattice(int* c_out /*19*3*/, double* w_out /*19*/);
