@@ -40,7 +40,7 @@ typedef struct plb_ctx plb_ctx; /* opaque */
 
 typedef struct { int nx, ny, nz; } plb_grid;
 
-enum { PLB_PERIODIC = 0, PLB_WALL_BB = 1 }; /* per axis */
+enum { PLB_PERIODIC = 0, PLB_WALL_BB = 1, PLB_WALL_HH = 2 }; /* per axis */
 
 /* kind[a]: PLB_PERIODIC wraps populations across axis a.  PLB_WALL_BB closes both
  * faces of axis a with link-wise halfway bounce-back: all n_a layers are fluid, the walls lie half
@@ -48,7 +48,14 @@ enum { PLB_PERIODIC = 0, PLB_WALL_BB = 1 }; /* per axis */
  * opposite direction at the same node with Ladd's moving-wall term -6 w_i rho_w (c_i . u_w),
  * rho_w = 1 (reading G9).  u_lo[a] / u_hi[a] = wall velocity at the low / high face of
  * axis a.  A link leaving through two wall faces at once takes the velocity of the first such
- * axis in x, y, z order. */
+ * axis in x, y, z order.
+ * PLB_WALL_HH is the wall the paper itself uses (L217-238): the Hecht-Harting on-site velocity
+ * condition.  The walls lie ON layers 0 and n_a - 1; after streaming, the populations of a wall
+ * cell that point into the fluid are "undetermined" and are closed from the others by Eq. 23-30
+ * (printed for the plane z = 0; other faces by renaming the axes), which sets
+ * sum_i c_i f_i = rho u_wall with rho from the first line of L219; wall cells then collide like
+ * any other.  lbm_set_equilibrium / lbm_write_populations close the wall layers too (DESIGN.md
+ * G24, G25).  Only one axis may be PLB_WALL_HH, the other two must be periodic, n_a >= 2. */
 typedef struct {
     int   kind[3];
     float u_lo[3][3];

@@ -14,7 +14,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libplb.so")
 
-PLB_PERIODIC, PLB_WALL_BB = 0, 1
+PLB_PERIODIC, PLB_WALL_BB, PLB_WALL_HH = 0, 1, 2
 PLB_OK, PLB_ERR_ARG, PLB_ERR_WORKSPACE, PLB_ERR_CUDA, PLB_ERR_ORDER, PLB_ERR_NODE_LEFT = 0, -1, -2, -3, -4, -5
 
 # every symbol include/plb.h declares: name -> (restype, argtypes)

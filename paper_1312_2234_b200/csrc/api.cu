@@ -134,9 +134,17 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
         return PLB_ERR_ARG;
     }
     for (int a = 0; a < 3; ++a)
-        if (bnd->kind[a] != PLB_PERIODIC && bnd->kind[a] != PLB_WALL_BB) {
+        if (bnd->kind[a] != PLB_PERIODIC && bnd->kind[a] != PLB_WALL_BB && bnd->kind[a] != PLB_WALL_HH) {
             set_error("lbm_create: invalid boundary kind on axis %d", a);
             return PLB_ERR_ARG;
+        }
+    for (int a = 0; a < 3; ++a)
+        if (bnd->kind[a] == PLB_WALL_HH) {
+            const int na = a == 0 ? grid->nx : (a == 1 ? grid->ny : grid->nz);
+            if (na < 2 || bnd->kind[(a + 1) % 3] != PLB_PERIODIC || bnd->kind[(a + 2) % 3] != PLB_PERIODIC) {
+                set_error("lbm_create: PLB_WALL_HH on axis %d needs n >= 2 and the other two axes periodic", a);
+                return PLB_ERR_ARG;
+            }
         }
     const long n_segs = (cells + SEG - 1) / SEG;
     const size_t need = carve(nullptr, nullptr, cells, n_segs, max_nodes, max_edges);
@@ -177,7 +185,11 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     p.omega = 1.0f / tau;
     p.pref = 1.0f - 0.5f / tau;
     for (int a = 0; a < 3; ++a) {
-        p.wall[a] = bnd->kind[a] == PLB_WALL_BB;
+        p.wall[a] = bnd->kind[a];
+        for (int d = 0; d < 3; ++d) {
+            p.uw[a][0][d] = bnd->u_lo[a][d];
+            p.uw[a][1][d] = bnd->u_hi[a][d];
+        }
         for (int d = 0; d < Q; ++d) {
             const double w = d < 6 ? 1.0 / 18.0 : (d < 18 ? 1.0 / 36.0 : 1.0 / 3.0);
             const double lo = CX(d) * (double)bnd->u_lo[a][0] + CY(d) * (double)bnd->u_lo[a][1] + CZ(d) * (double)bnd->u_lo[a][2];

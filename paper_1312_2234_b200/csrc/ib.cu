@@ -435,9 +435,12 @@ __global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
                 U[m] = make_float4(ux, uy, uz, 0.f);
                 const double xn = X[m] + (double)ux, yn = Y[m] + (double)uy, zn = Z[m] + (double)uz;
                 X[m] = xn; Y[m] = yn; Z[m] = zn;
-                const bool left = (p.wall[0] && (xn < -0.5 || xn > (double)p.nx - 0.5)) ||
-                                  (p.wall[1] && (yn < -0.5 || yn > (double)p.ny - 0.5)) ||
-                                  (p.wall[2] && (zn < -0.5 || zn > (double)p.nz - 0.5));
+                // halfway bounce-back walls lie at -1/2 and n - 1/2, on-site velocity walls at 0 and n - 1
+                const double m0 = p.wall[0] == PLB_WALL_HH ? 0.0 : 0.5, m1 = p.wall[1] == PLB_WALL_HH ? 0.0 : 0.5,
+                             m2 = p.wall[2] == PLB_WALL_HH ? 0.0 : 0.5;
+                const bool left = (p.wall[0] && (xn < -m0 || xn > (double)(p.nx - 1) + m0)) ||
+                                  (p.wall[1] && (yn < -m1 || yn > (double)(p.ny - 1) + m1)) ||
+                                  (p.wall[2] && (zn < -m2 || zn > (double)(p.nz - 1) + m2));
                 if (left) atomicOr(counters + 1, STATUS_NODE_LEFT);
             }
         }

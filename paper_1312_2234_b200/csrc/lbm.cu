@@ -276,6 +276,7 @@ struct Target {
     int idx;      // cell whose f is wanted
     int d;        // which population of that cell
     float corr;   // to subtract
+    bool dead;    // the link leaves through an on-site velocity wall: the slot is never read
 };
 
 template <int D>
@@ -283,17 +284,21 @@ __device__ __forceinline__ Target pre_stream_target(const LbmParams& p, const Ce
     constexpr int cx = CX(D), cy = CY(D), cz = CZ(D);
     const int nx = p.nx, ny = p.ny, nz = p.nz;
     int ti = c.i + cx, tj = c.j + cy, tk = c.k + cz;
-    bool b = false;
+    bool b = false, dead = false;
     float corr = 0.f;
-    // link D from x leaves through ...; z, y, x order so that x wins (corner rule)
-    if (tk < 0) { if (p.wall[2]) { b = true; corr = p.corr[2][0][OPP(D)]; } else tk += nz; }
-    if (tk >= nz) { if (p.wall[2]) { b = true; corr = p.corr[2][1][OPP(D)]; } else tk -= nz; }
-    if (tj < 0) { if (p.wall[1]) { b = true; corr = p.corr[1][0][OPP(D)]; } else tj += ny; }
-    if (tj >= ny) { if (p.wall[1]) { b = true; corr = p.corr[1][1][OPP(D)]; } else tj -= ny; }
-    if (ti < 0) { if (p.wall[0]) { b = true; corr = p.corr[0][0][OPP(D)]; } else ti += nx; }
-    if (ti >= nx) { if (p.wall[0]) { b = true; corr = p.corr[0][1][OPP(D)]; } else ti -= nx; }
+    // link D from x leaves through ...; z, y, x order so that x wins (corner rule).  Through an
+    // on-site velocity wall the population simply leaves: the slot is never read.
+    const bool bbx = p.wall[0] == PLB_WALL_BB, bby = p.wall[1] == PLB_WALL_BB, bbz = p.wall[2] == PLB_WALL_BB;
+    if (tk < 0) { if (bbz) { b = true; corr = p.corr[2][0][OPP(D)]; } else if (p.wall[2]) dead = true; else tk += nz; }
+    if (tk >= nz) { if (bbz) { b = true; corr = p.corr[2][1][OPP(D)]; } else if (p.wall[2]) dead = true; else tk -= nz; }
+    if (tj < 0) { if (bby) { b = true; corr = p.corr[1][0][OPP(D)]; } else if (p.wall[1]) dead = true; else tj += ny; }
+    if (tj >= ny) { if (bby) { b = true; corr = p.corr[1][1][OPP(D)]; } else if (p.wall[1]) dead = true; else tj -= ny; }
+    if (ti < 0) { if (bbx) { b = true; corr = p.corr[0][0][OPP(D)]; } else if (p.wall[0]) dead = true; else ti += nx; }
+    if (ti >= nx) { if (bbx) { b = true; corr = p.corr[0][1][OPP(D)]; } else if (p.wall[0]) dead = true; else ti -= nx; }
     Target t;
-    if (b) { t.idx = idx; t.d = OPP(D); t.corr = corr; }
+    t.dead = dead;
+    if (dead) { t.idx = idx; t.d = D; t.corr = 0.f; }
+    else if (b) { t.idx = idx; t.d = OPP(D); t.corr = corr; }
     else   { t.idx = ti + nx * (tj + ny * tk); t.d = D; t.corr = 0.f; }
     return t;
 }
@@ -321,7 +326,7 @@ __device__ __forceinline__ void init_one(float* __restrict__ dst, const LbmParam
                                          const float* rho_in, const float* u_in, const float amp,
                                          const unsigned long long seed) {
     const Target t = pre_stream_target<D>(p, c, idx);
-    dst[(size_t)D * p.cells + idx] = init_value(t.d, t.idx, rho_in, u_in, (size_t)p.cells, amp, seed) - t.corr;
+    dst[(size_t)D * p.cells + idx] = t.dead ? 0.f : init_value(t.d, t.idx, rho_in, u_in, (size_t)p.cells, amp, seed) - t.corr;
     if constexpr (D + 1 < Q) init_one<D + 1>(dst, p, c, idx, rho_in, u_in, amp, seed);
 }
 
@@ -338,7 +343,7 @@ __device__ __forceinline__ void write_one(float* __restrict__ dst, const float* 
                                           const Cell c, const int idx) {
     const Target t = pre_stream_target<D>(p, c, idx);
     const float wd = WGT(D);
-    dst[(size_t)D * p.cells + idx] = (__ldg(f + (size_t)t.d * p.cells + t.idx) - wd) - t.corr;
+    dst[(size_t)D * p.cells + idx] = t.dead ? 0.f : (__ldg(f + (size_t)t.d * p.cells + t.idx) - wd) - t.corr;
     if constexpr (D + 1 < Q) write_one<D + 1>(dst, f, p, c, idx);
 }
 

@@ -19,6 +19,53 @@ __device__ __forceinline__ Cell cell_of(int idx, const LbmParams& p) {
     return c;
 }
 
+__host__ __device__ constexpr int CA(int a, int d) { return a == 0 ? CX(d) : (a == 1 ? CY(d) : CZ(d)); }
+
+// Hecht-Harting on-site velocity wall (Eq. 23-30) on a cell of
+// the face of axis A with inward normal n = sgn e_A and wall velocity vw: the populations with
+// c.n = +1 did not arrive by streaming and are closed from the others,
+//     rho = [sum_{c.n=0} f + 2 sum_{c.n=-1} f]/(1 - v.n),       f_n = f_-n + rho v.n/3,
+//     f_{n + s t} = f_opp + rho (v.n + s v_t)/6 - s N_t,   N_t = (1/2) sum_{c.n=0} c_t f - rho v_t/3.
+// Written on the shifted values h = f - w:  sum_{c.n=0} w + 2 sum_{c.n=-1} w = 2/3 + 2/6 = 1 and
+// w_i = w_opp(i), so only the density needs the shift put back.
+template <int A, int V, int COL>
+__device__ __forceinline__ void hecht_harting_close(float (&h)[Q][V], const int sgn, const float* __restrict__ vw) {
+    const float vn = (float)sgn * vw[A];
+    float s0 = 0.f, sm = 0.f, T[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+    for (int d = 0; d < Q; ++d) {
+        const int ca = CA(A, d);
+        if (ca == 0) {
+            s0 += h[d][COL];
+#pragma unroll
+            for (int b = 0; b < 3; ++b)
+                if (b != A && CA(b, d) != 0) T[b] += (float)CA(b, d) * h[d][COL];
+        } else {
+            sm += (ca == -sgn) ? h[d][COL] : 0.f;
+        }
+    }
+    const float rho = (1.0f + (s0 + 2.0f * sm)) / (1.0f - vn);
+    float N[3];
+#pragma unroll
+    for (int b = 0; b < 3; ++b) N[b] = 0.5f * T[b] - rho * vw[b] * (1.0f / 3.0f);
+#pragma unroll
+    for (int d = 0; d < Q; ++d) {
+        const int ca = CA(A, d);
+        if (ca == 0) continue;
+        float val;
+        int bt = -1;
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+            if (b != A && CA(b, d) != 0) bt = b;
+        if (bt < 0) val = h[OPP(d)][COL] + rho * vn * (1.0f / 3.0f);
+        else {
+            const float ct = (float)CA(bt, d);
+            val = h[OPP(d)][COL] + rho * (vn + ct * vw[bt]) * (1.0f / 6.0f) - ct * N[bt];
+        }
+        if (ca == sgn) h[d][COL] = val;
+    }
+}
+
 // Pull the 19 streamed populations (minus w_d) of cell (i,j,k) out of the pre-stream lattice
 // into column COL of h.  Generic in the boundary kinds of all three axes.
 template <int V, int COL>
@@ -29,13 +76,17 @@ __device__ __forceinline__ void pull19(const float* __restrict__ src, const LbmP
     const bool xlo = c.i == 0, xhi = c.i == nx - 1;
     const bool ylo = c.j == 0, yhi = c.j == ny - 1;
     const bool zlo = c.k == 0, zhi = c.k == nz - 1;
-    // neighbour offsets with periodic wrap (a wall axis bounces instead, decided below)
+    // neighbour offsets with periodic wrap (a wall axis bounces / closes instead, decided below)
     const int dxm = xlo ? nx - 1 : -1, dxp = xhi ? 1 - nx : 1;
     const int dym = (ylo ? ny - 1 : -1) * nx, dyp = (yhi ? 1 - ny : 1) * nx;
     const int dzm = (zlo ? nz - 1 : -1) * nx * ny, dzp = (zhi ? 1 - nz : 1) * nx * ny;
-    const bool bxlo = p.wall[0] && xlo, bxhi = p.wall[0] && xhi;
-    const bool bylo = p.wall[1] && ylo, byhi = p.wall[1] && yhi;
-    const bool bzlo = p.wall[2] && zlo, bzhi = p.wall[2] && zhi;
+    const bool bxlo = p.wall[0] == PLB_WALL_BB && xlo, bxhi = p.wall[0] == PLB_WALL_BB && xhi;
+    const bool bylo = p.wall[1] == PLB_WALL_BB && ylo, byhi = p.wall[1] == PLB_WALL_BB && yhi;
+    const bool bzlo = p.wall[2] == PLB_WALL_BB && zlo, bzhi = p.wall[2] == PLB_WALL_BB && zhi;
+    // on-site velocity wall (at most one axis): face of this cell, 0 = none, +1 = low, -1 = high
+    const int hx = p.wall[0] == PLB_WALL_HH ? (xlo ? 1 : (xhi ? -1 : 0)) : 0;
+    const int hy = p.wall[1] == PLB_WALL_HH ? (ylo ? 1 : (yhi ? -1 : 0)) : 0;
+    const int hz = p.wall[2] == PLB_WALL_HH ? (zlo ? 1 : (zhi ? -1 : 0)) : 0;
 #pragma unroll
     for (int d = 0; d < Q; ++d) {
         const int cx = CX(d), cy = CY(d), cz = CZ(d);
@@ -56,9 +107,15 @@ __device__ __forceinline__ void pull19(const float* __restrict__ src, const LbmP
         if (cy == -1 && byhi) { b = true; corr = p.corr[1][1][d]; }
         if (cx == 1 && bxlo) { b = true; corr = p.corr[0][0][d]; }
         if (cx == -1 && bxhi) { b = true; corr = p.corr[0][1][d]; }
-        if (b) h[d][COL] = __ldg(src + (size_t)OPP(d) * N + idx) + corr;
-        else   h[d][COL] = __ldg(src + (size_t)d * N + (idx + off));
+        // on-site wall: x - c_d lies beyond the face -> "undetermined" (L217), closed below
+        const bool undetermined = (cx != 0 && cx == hx) || (cy != 0 && cy == hy) || (cz != 0 && cz == hz);
+        if (undetermined) h[d][COL] = 0.f;
+        else if (b) h[d][COL] = __ldg(src + (size_t)OPP(d) * N + idx) + corr;
+        else        h[d][COL] = __ldg(src + (size_t)d * N + (idx + off));
     }
+    if (hx) hecht_harting_close<0, V, COL>(h, hx, p.uw[0][hx < 0]);
+    if (hy) hecht_harting_close<1, V, COL>(h, hy, p.uw[1][hy < 0]);
+    if (hz) hecht_harting_close<2, V, COL>(h, hz, p.uw[2][hz < 0]);
 }
 
 // delta rho = sum h_d, j = sum c_d h_d (Eq. 17-18; sum_d w_d c_d = 0 so the shift drops out of j)

@@ -39,10 +39,11 @@ __host__ __device__ constexpr float WGT(int d) {
 struct LbmParams {
     int nx, ny, nz;
     int cells;                 // nx*ny*nz < 2^31
-    int wall[3];               // 1 = bounce-back on this axis
+    int wall[3];               // boundary kind of the axis: PLB_PERIODIC, PLB_WALL_BB or PLB_WALL_HH
     float omega;               // 1/tau
     float pref;                // 1 - 1/(2 tau)
     float corr[3][2][Q];       // [axis][0 = low face, 1 = high face][d] = 6 w_d (c_d . u_wall)
+    float uw[3][2][3];         // [axis][face] wall velocity (on-site velocity walls)
 };
 
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };

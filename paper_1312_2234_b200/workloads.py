@@ -24,7 +24,8 @@ import numpy as np
 SEED_BASE = 131222340  # seeds are SEED_BASE + config number
 
 PERIODIC = 0
-WALL = 1
+WALL = 1        # halfway bounce-back + moving-wall term (the BASELINE configs)
+WALL_HH = 2     # Hecht-Harting on-site velocity wall (the paper's own, Eq. 23-30)
 
 
 # --------------------------------------------------------------------------------------
@@ -268,6 +269,23 @@ def config5(n=256, grid_xz=64, layers=2, steps=200, subdiv=4, seed=SEED_BASE + 5
                     notes=["centres on a jittered %dx%dx%d lattice (spacing >= 3): the config's minimum centre "
                            "spacing of 11 cannot hold 8192 platelets in a 256x20x256 slab; meshes interpenetrate"
                            % (grid_xz, layers, grid_xz)])
+
+
+def with_onsite_walls(w: Workload) -> Workload:
+    """The same workload closed with the paper's own wall (Hecht-Harting on-site velocity
+    condition, walls ON layers 0 and n_y - 1) instead of the configs' halfway bounce-back; the
+    initial shear is the matching Couette steady state u_x(j) = u_wall j/(n_y - 1)."""
+    import copy
+    v = copy.copy(w)
+    assert tuple(w.kind) == (PERIODIC, WALL, PERIODIC)
+    v.kind = (PERIODIC, WALL_HH, PERIODIC)
+    u_wall = float(w.u_hi[1, 0])
+    u = np.zeros((3, w.nz, w.ny, w.nx), dtype=np.float64)
+    u[0] = (u_wall * np.arange(w.ny, dtype=np.float64) / (w.ny - 1))[None, :, None]
+    v.u0 = u.reshape(3, -1)
+    v.name = w.name + "-onsite"
+    v.notes = list(w.notes) + ["walls: Hecht-Harting on-site velocity condition (PAPER.md Eq. 23-30)"]
+    return v
 
 
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
