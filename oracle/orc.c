@@ -59,6 +59,13 @@ struct orc_ctx {
     real *X, *F, *U;                   /* AoS 3 per node */
     int *edge;                         /* global node index pairs */
     real *rest, *kspring;              /* per edge */
+    /* NEXT-2 (Eq. 4-5): triangles of the lipid-bilayer surface, per mesh */
+    int *mesh_off;                     /* first global node of mesh s (n_meshes + 1 entries) */
+    int n_tris, cap_tris;
+    int *tri;                          /* global node index triples, outward orientation */
+    int *tri_mesh;                     /* mesh of each triangle */
+    real *tri_S0;                      /* unstressed triangle area S_0 */
+    real *S0_tot, *V0, *k_s, *k_t, *k_v;   /* per mesh (k = 0 and no triangles until orc_set_triangles) */
     int forces_valid;
 };
 
@@ -163,6 +170,8 @@ int orc_destroy(orc_ctx* c) {
     if (!c) return -1;
     free(c->f); free(c->fstar); free(c->g_last);
     free(c->X); free(c->F); free(c->U); free(c->edge); free(c->rest); free(c->kspring);
+    free(c->mesh_off); free(c->tri); free(c->tri_mesh); free(c->tri_S0);
+    free(c->S0_tot); free(c->V0); free(c->k_s); free(c->k_t); free(c->k_v);
     free(c);
     return 0;
 }
@@ -403,8 +412,150 @@ int orc_add_mesh(orc_ctx* c, int n_nodes, const double* xyz, int n_edges, const 
     c->n_edges += n_edges;
     if (out_mesh_id) *out_mesh_id = c->n_meshes;
     c->n_meshes += 1;
+    c->mesh_off = (int*)realloc(c->mesh_off, (size_t)(c->n_meshes + 1) * sizeof(int));
+    c->mesh_off[c->n_meshes - 1] = off;
+    c->mesh_off[c->n_meshes] = c->n_nodes;
+    c->S0_tot = (real*)realloc(c->S0_tot, (size_t)c->n_meshes * sizeof(real));
+    c->V0 = (real*)realloc(c->V0, (size_t)c->n_meshes * sizeof(real));
+    c->k_s = (real*)realloc(c->k_s, (size_t)c->n_meshes * sizeof(real));
+    c->k_t = (real*)realloc(c->k_t, (size_t)c->n_meshes * sizeof(real));
+    c->k_v = (real*)realloc(c->k_v, (size_t)c->n_meshes * sizeof(real));
+    c->S0_tot[c->n_meshes - 1] = c->V0[c->n_meshes - 1] = 0;
+    c->k_s[c->n_meshes - 1] = c->k_t[c->n_meshes - 1] = c->k_v[c->n_meshes - 1] = 0;
     c->forces_valid = 0;
     return 0;
+}
+
+/* ---- NEXT-2: area and volume constraints (Eq. 4-5) -------------------------------
+ *   H_area   = k_s (S_tot - S0_tot)^2 / (2 S0_tot) + sum_triangles k_t (S - S_0)^2 / (2 S_0)
+ *   H_volume = k_v (V - V_0)^2 / (2 V_0)
+ * with, for a triangle (a, b, c) oriented outwards,  n = (X_b - X_a) x (X_c - X_a),  S = |n|/2,
+ * and for the closed surface  V = (1/6) sum_triangles X_a . (X_b x X_c)  (divergence theorem).
+ * Nodal force = -dH/dX (Eq. 11 read with the minus sign, G2):
+ *   dS/dX_a = (1/2) nhat x (X_c - X_b)   (cyclic in a, b, c),     dV/dX_a = (1/6) X_b x X_c  (cyclic). */
+static void cross3(const real a[3], const real b[3], real out[3]) {
+    out[0] = a[1] * b[2] - a[2] * b[1];
+    out[1] = a[2] * b[0] - a[0] * b[2];
+    out[2] = a[0] * b[1] - a[1] * b[0];
+}
+static real tri_area(const real* X, const int t[3], real nhat[3]) {
+    real ab[3], ac[3], n[3];
+    for (int d = 0; d < 3; ++d) {
+        ab[d] = X[3 * t[1] + d] - X[3 * t[0] + d];
+        ac[d] = X[3 * t[2] + d] - X[3 * t[0] + d];
+    }
+    cross3(ab, ac, n);
+    const real len = (real)sqrt((double)(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]));
+    if (nhat)
+        for (int d = 0; d < 3; ++d) nhat[d] = len > 0 ? n[d] / len : 0;
+    return len / 2;
+}
+static real tri_volume6(const real* X, const int t[3]) {   /* X_a . (X_b x X_c) */
+    real bc[3];
+    cross3(X + 3 * t[1], X + 3 * t[2], bc);
+    return X[3 * t[0]] * bc[0] + X[3 * t[0] + 1] * bc[1] + X[3 * t[0] + 2] * bc[2];
+}
+/* S_tot and V of mesh s at positions X */
+static void mesh_area_volume(const orc_ctx* c, const real* X, int s, real* S_tot, real* V) {
+    real S = 0, V6 = 0;
+    for (int t = 0; t < c->n_tris; ++t) {
+        if (c->tri_mesh[t] != s) continue;
+        S += tri_area(X, c->tri + 3 * t, NULL);
+        V6 += tri_volume6(X, c->tri + 3 * t);
+    }
+    *S_tot = S;
+    *V = V6 / 6;
+}
+
+int orc_set_triangles(orc_ctx* c, int mesh_id, int n_tris, const int* tris, const double* ref_xyz,
+                      double k_s, double k_t, double k_v) {
+    if (!c || mesh_id < 0 || mesh_id >= c->n_meshes || n_tris < 1 || !tris) return -1;
+    if (c->S0_tot[mesh_id] != 0) return -4;                       /* once per mesh */
+    const int off = c->mesh_off[mesh_id], nn = c->mesh_off[mesh_id + 1] - off;
+    for (int t = 0; t < 3 * n_tris; ++t)
+        if (tris[t] < 0 || tris[t] >= nn) return -1;
+    if (c->n_tris + n_tris > c->cap_tris) {
+        c->cap_tris = 2 * (c->n_tris + n_tris);
+        c->tri = (int*)realloc(c->tri, (size_t)3 * c->cap_tris * sizeof(int));
+        c->tri_mesh = (int*)realloc(c->tri_mesh, (size_t)c->cap_tris * sizeof(int));
+        c->tri_S0 = (real*)realloc(c->tri_S0, (size_t)c->cap_tris * sizeof(real));
+    }
+    /* the unstressed shape: ref_xyz (mesh-local node order), or the current positions */
+    real* R = (real*)malloc((size_t)3 * c->n_nodes * sizeof(real));
+    for (int m = 0; m < 3 * c->n_nodes; ++m) R[m] = c->X[m];
+    if (ref_xyz)
+        for (int m = 0; m < 3 * nn; ++m) R[3 * off + m] = (real)ref_xyz[m];
+    for (int t = 0; t < n_tris; ++t) {
+        const int gt = c->n_tris + t;
+        for (int v = 0; v < 3; ++v) c->tri[3 * gt + v] = off + tris[3 * t + v];
+        c->tri_mesh[gt] = mesh_id;
+        c->tri_S0[gt] = tri_area(R, c->tri + 3 * gt, NULL);
+        if (!(c->tri_S0[gt] > 0)) { free(R); return -1; }
+    }
+    c->n_tris += n_tris;
+    mesh_area_volume(c, R, mesh_id, &c->S0_tot[mesh_id], &c->V0[mesh_id]);
+    free(R);
+    if (!(c->V0[mesh_id] > 0)) return -1;                         /* not closed / not outward oriented */
+    c->k_s[mesh_id] = (real)k_s; c->k_t[mesh_id] = (real)k_t; c->k_v[mesh_id] = (real)k_v;
+    c->forces_valid = 0;
+    return 0;
+}
+
+int orc_mesh_area_volume(orc_ctx* c, int mesh_id, double* S_tot, double* V) {
+    if (!c || mesh_id < 0 || mesh_id >= c->n_meshes) return -1;
+    real S, Vv;
+    mesh_area_volume(c, c->X, mesh_id, &S, &Vv);
+    if (S_tot) *S_tot = (double)S;
+    if (V) *V = (double)Vv;
+    return 0;
+}
+
+/* H_area + H_volume of all meshes (Eq. 4-5) at the current positions */
+double orc_area_volume_energy(orc_ctx* c) {
+    double H = 0;
+    for (int s = 0; s < c->n_meshes; ++s) {
+        if (c->S0_tot[s] == 0) continue;
+        real S, V;
+        mesh_area_volume(c, c->X, s, &S, &V);
+        H += 0.5 * (double)c->k_s[s] * (double)(S - c->S0_tot[s]) * (double)(S - c->S0_tot[s]) / (double)c->S0_tot[s];
+        H += 0.5 * (double)c->k_v[s] * (double)(V - c->V0[s]) * (double)(V - c->V0[s]) / (double)c->V0[s];
+    }
+    for (int t = 0; t < c->n_tris; ++t) {
+        const double S = (double)tri_area(c->X, c->tri + 3 * t, NULL), S0 = (double)c->tri_S0[t];
+        H += 0.5 * (double)c->k_t[c->tri_mesh[t]] * (S - S0) * (S - S0) / S0;
+    }
+    return H;
+}
+
+/* F_m -= dH_area/dX_m + dH_volume/dX_m, triangle by triangle */
+static void area_volume_forces(orc_ctx* c) {
+    if (c->n_tris == 0) return;
+    real* alpha = (real*)malloc((size_t)c->n_meshes * sizeof(real));   /* k_s (S_tot - S0_tot)/S0_tot */
+    real* beta = (real*)malloc((size_t)c->n_meshes * sizeof(real));    /* k_v (V - V_0)/V_0 */
+    for (int s = 0; s < c->n_meshes; ++s) {
+        alpha[s] = beta[s] = 0;
+        if (c->S0_tot[s] == 0) continue;
+        real S, V;
+        mesh_area_volume(c, c->X, s, &S, &V);
+        alpha[s] = c->k_s[s] * (S - c->S0_tot[s]) / c->S0_tot[s];
+        beta[s] = c->k_v[s] * (V - c->V0[s]) / c->V0[s];
+    }
+    for (int t = 0; t < c->n_tris; ++t) {
+        const int* tv = c->tri + 3 * t;
+        const int s = c->tri_mesh[t];
+        real nhat[3];
+        const real S = tri_area(c->X, tv, nhat);
+        const real coefS = alpha[s] + c->k_t[s] * (S - c->tri_S0[t]) / c->tri_S0[t];
+        for (int v = 0; v < 3; ++v) {
+            const int a = tv[v], b = tv[(v + 1) % 3], cc = tv[(v + 2) % 3];
+            real cb[3], dS[3], dV[3];
+            for (int d = 0; d < 3; ++d) cb[d] = c->X[3 * cc + d] - c->X[3 * b + d];
+            cross3(nhat, cb, dS);                               /* 2 dS/dX_a */
+            cross3(c->X + 3 * b, c->X + 3 * cc, dV);            /* 6 dV/dX_a */
+            for (int d = 0; d < 3; ++d) c->F[3 * a + d] -= coefS * dS[d] / 2 + beta[s] * dV[d] / 6;
+        }
+    }
+    free(alpha); free(beta);
 }
 
 /* O-5: F <- 0; for each edge (a,b): R = X_b - X_a, l = |R|, e = k (l - L) R / l; F_a += e,
@@ -429,6 +580,7 @@ int orc_compute_membrane_forces(orc_ctx* c, double sigma, uint64_t seed, uint64_
             c->F[3 * b + d] -= ed;
         }
     }
+    area_volume_forces(c);
     if (sigma > 0)
         for (int m = 0; m < c->n_nodes; ++m) {
             double z[3];

@@ -56,6 +56,14 @@ int orc_write_populations(orc_ctx*, const double* f);
 
 int orc_add_mesh(orc_ctx*, int n_nodes, const double* xyz /*AoS*/, int n_edges, const int* edges,
                  const double* rest /*NULL = lengths of xyz*/, double k, int* out_mesh_id);
+/* NEXT-2 (Eq. 4-5): triangles (mesh-local node triples, outward orientation) of mesh mesh_id, the
+ * unstressed shape ref_xyz (n_nodes x 3, NULL = the current positions) that defines S_0, S0_tot, V_0,
+ * and the coefficients k_s (global area), k_t (local area), k_v (volume).  Once per mesh. */
+int orc_set_triangles(orc_ctx*, int mesh_id, int n_tris, const int* tris, const double* ref_xyz,
+                      double k_s, double k_t, double k_v);
+int orc_mesh_area_volume(orc_ctx*, int mesh_id, double* S_tot, double* V);
+double orc_area_volume_energy(orc_ctx*);   /* H_area + H_volume, Eq. 4-5 */
+/* springs (Eq. 2-3) + area / volume constraint forces (Eq. 4-5, meshes with triangles) + noise */
 int orc_compute_membrane_forces(orc_ctx*, double sigma, uint64_t seed, uint64_t step);
 int orc_spread(orc_ctx*, double* g /*3*cells, overwritten*/);
 int orc_interpolate_advance(orc_ctx*);

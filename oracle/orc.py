@@ -39,6 +39,9 @@ def lib(fp32: bool = False):
             "orc_write_populations": (C.c_int, [vp, dp]),
             "orc_add_mesh": (C.c_int, [vp, C.c_int, dp, C.c_int, ip, dp, C.c_double, ip]),
             "orc_compute_membrane_forces": (C.c_int, [vp, C.c_double, u64, u64]),
+            "orc_set_triangles": (C.c_int, [vp, C.c_int, C.c_int, ip, dp, C.c_double, C.c_double, C.c_double]),
+            "orc_mesh_area_volume": (C.c_int, [vp, C.c_int, dp, dp]),
+            "orc_area_volume_energy": (C.c_double, [vp]),
             "orc_spread": (C.c_int, [vp, dp]),
             "orc_interpolate_advance": (C.c_int, [vp]),
             "orc_n_nodes": (C.c_int, [vp]),
@@ -183,6 +186,20 @@ class Oracle:
         self._chk(self.L.orc_add_mesh(self.h, xyz.shape[0], _dp(xyz), edges.shape[0], _ip(edges), _dp(rest),
                                       float(k), C.byref(mid)), "orc_add_mesh")
         return mid.value
+
+    def set_triangles(self, mesh_id, tris, ref_xyz=None, k_s=0.0, k_t=0.0, k_v=0.0):
+        tris = np.ascontiguousarray(tris, dtype=np.int32)
+        ref_xyz = _f64(ref_xyz)
+        self._chk(self.L.orc_set_triangles(self.h, int(mesh_id), tris.shape[0], _ip(tris), _dp(ref_xyz),
+                                           float(k_s), float(k_t), float(k_v)), "orc_set_triangles")
+
+    def mesh_area_volume(self, mesh_id):
+        S, V = C.c_double(), C.c_double()
+        self._chk(self.L.orc_mesh_area_volume(self.h, int(mesh_id), C.byref(S), C.byref(V)), "orc_mesh_area_volume")
+        return S.value, V.value
+
+    def area_volume_energy(self):
+        return self.L.orc_area_volume_energy(self.h)
 
     @property
     def n_nodes(self):
