@@ -112,10 +112,23 @@ PLB_API int ib_add_mesh(plb_ctx* ctx, int n_nodes, const double* h_xyz, int n_ed
 PLB_API int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, int n_edges,
                   const int* h_edges, const float* h_rest, float k, int* out_first_mesh_id);
 
+/* Area and volume constraints of the lipid bilayer (Eq. 4-5)
+ * for meshes first_mesh_id .. first_mesh_id + n_meshes - 1, which must share one topology:
+ *   H_area   = k_s (S_tot - S0_tot)^2/(2 S0_tot) + sum_triangles k_t (S - S_0)^2/(2 S_0)
+ *   H_volume = k_v (V - V_0)^2/(2 V_0)
+ * h_tris: n_tris x 3 mesh-local node indices, oriented outwards (V_0 must come out positive; the
+ * surface must be closed).  h_ref_xyz: n_nodes x 3 doubles, the unstressed shape that defines
+ * S_0, S0_tot and V_0 (any rigid placement), or NULL = each mesh's current positions.  Once per
+ * mesh.  Capacity: 2 * max_nodes triangles (a closed genus-0 surface of N nodes has 2N - 4).
+ * From then on ib_compute_membrane_forces adds -dH/dX of these meshes to the spring forces. */
+PLB_API int ib_set_triangles(plb_ctx* ctx, int first_mesh_id, int n_meshes, int n_tris, const int* h_tris,
+                     const double* h_ref_xyz, float k_s, float k_t, float k_v);
+
 /* S1.  F <- 0; for every edge (a,b): R = X_b - X_a, e = k (|R| - L) R/|R|, F_a += e, F_b -= e
  * (Eq. 2-3, sign read as F = -grad H, G1).  If noise_sigma > 0 adds
  * noise_sigma * N(0,1) per node component from Philox keyed on (noise_seed; global node, step,
- * tag 2) with Box-Muller (O-8). */
+ * tag 2) with Box-Muller (O-8).  Meshes given triangles by ib_set_triangles also get
+ * the area / volume constraint forces of Eq. 4-5. */
 PLB_API int ib_compute_membrane_forces(plb_ctx* ctx, float noise_sigma, unsigned long long noise_seed,
                                unsigned long long step);
 

@@ -134,6 +134,8 @@ class Oracle:
         o.set_equilibrium(None, w.u0, w.noise_amp, w.noise_seed)
         for m in range(w.n_meshes):
             o.add_mesh(w.mesh_xyz[m], w.edges, w.rest, w.k_spring)
+            if w.k_area_global or w.k_area_local or w.k_volume:
+                o.set_triangles(m, w.tris, w.ref_xyz, w.k_area_global, w.k_area_local, w.k_volume)
         return o
 
     def _chk(self, rc, what):

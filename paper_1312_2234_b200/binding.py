@@ -30,6 +30,7 @@ SYMBOLS = {
     "lbm_read_macros": (_i, [_vp, _vp, _vp]),
     "ib_add_mesh": (_i, [_vp, _i, _vp, _i, _vp, _vp, _f, C.POINTER(_i)]),
     "ib_add_meshes": (_i, [_vp, _i, _i, _vp, _i, _vp, _vp, _f, C.POINTER(_i)]),
+    "ib_set_triangles": (_i, [_vp, _i, _i, _i, _vp, _vp, _f, _f, _f]),
     "ib_compute_membrane_forces": (_i, [_vp, _f, _u64, _u64]),
     "ib_spread": (_i, [_vp, _vp]),
     "ib_interpolate_advance": (_i, [_vp]),
@@ -167,6 +168,13 @@ def ib_add_meshes(h, xyz, edges, rest=None, k=0.0) -> int:
     return mid.value
 
 
+def ib_set_triangles(h, first_mesh_id, n_meshes, tris, ref_xyz=None, k_s=0.0, k_t=0.0, k_v=0.0):
+    tris = np.ascontiguousarray(tris, dtype=np.int32)
+    ref_xyz = None if ref_xyz is None else np.ascontiguousarray(ref_xyz, dtype=np.float64)
+    _check(lib().ib_set_triangles(h, int(first_mesh_id), int(n_meshes), tris.shape[0], _np_ptr(tris), _np_ptr(ref_xyz),
+                                  float(k_s), float(k_t), float(k_v)), "ib_set_triangles")
+
+
 def ib_compute_membrane_forces(h, noise_sigma=0.0, noise_seed=0, step=0):
     _check(lib().ib_compute_membrane_forces(h, float(noise_sigma), int(noise_seed), int(step)), "ib_compute_membrane_forces")
 
@@ -259,7 +267,9 @@ class Simulation:
         u = None if w.u0 is None else torch.as_tensor(w.u0, dtype=torch.float32).to(s.device).contiguous()
         s.set_equilibrium(None, u, w.noise_amp, w.noise_seed)
         if w.n_meshes:
-            s.add_meshes(w.mesh_xyz, w.edges, w.rest, w.k_spring)
+            first = s.add_meshes(w.mesh_xyz, w.edges, w.rest, w.k_spring)
+            if w.k_area_global or w.k_area_local or w.k_volume:
+                s.set_triangles(first, w.n_meshes, w.tris, w.ref_xyz, w.k_area_global, w.k_area_local, w.k_volume)
         return s
 
     def close(self):
@@ -298,6 +308,9 @@ class Simulation:
 
     def add_meshes(self, xyz, edges, rest=None, k=0.0):
         return ib_add_meshes(self.h, xyz, edges, rest, k)
+
+    def set_triangles(self, first_mesh_id, n_meshes, tris, ref_xyz=None, k_s=0.0, k_t=0.0, k_v=0.0):
+        ib_set_triangles(self.h, first_mesh_id, n_meshes, tris, ref_xyz, k_s, k_t, k_v)
 
     def compute_membrane_forces(self, sigma=0.0, seed=0, step=0):
         ib_compute_membrane_forces(self.h, sigma, seed, step)

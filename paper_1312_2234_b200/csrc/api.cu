@@ -53,7 +53,13 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     int2* edges = w.take<int2>((size_t)max_edges);
     float2* eprm = w.take<float2>((size_t)max_edges);
     int2* ranges = w.take<int2>((size_t)max_nodes);
+    // a closed genus-0 triangulated surface of N nodes has 2N - 4 triangles and at least 4 nodes
+    int4* tris = w.take<int4>((size_t)2 * max_nodes);
+    float* tri_S0 = w.take<float>((size_t)2 * max_nodes);
+    MeshConstraint* cons = w.take<MeshConstraint>((size_t)max_nodes / 4 + 1);
     if (c) {
+        c->tris = tris; c->tri_S0 = tri_S0; c->cons = cons;
+        c->cap_tris = 2 * max_nodes; c->cap_cons = max_nodes / 4 + 1;
         c->f[0] = f0; c->f[1] = f1;
         c->seg_mask = seg_mask; c->counters = counters;
         c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
@@ -93,6 +99,31 @@ static int sync_status(Ctx* c) {
     return PLB_OK;
 }
 
+}  // namespace plb
+
+// host-side geometry of one unstressed mesh: S_0 per triangle, S0_tot, V_0 (plain fp64; set-up only)
+namespace plb {
+void reference_area_volume(const double* x, int n_tris, const int* tris, float* S0, double* S0_tot, double* V0) {
+    double S = 0, V6 = 0;
+    for (int t = 0; t < n_tris; ++t) {
+        const double* a = x + 3 * tris[3 * t];
+        const double* b = x + 3 * tris[3 * t + 1];
+        const double* c = x + 3 * tris[3 * t + 2];
+        const double ab[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]}, ac[3] = {c[0] - a[0], c[1] - a[1], c[2] - a[2]};
+        const double n[3] = {ab[1] * ac[2] - ab[2] * ac[1], ab[2] * ac[0] - ab[0] * ac[2], ab[0] * ac[1] - ab[1] * ac[0]};
+        const double s = 0.5 * sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+        S0[t] = (float)s;
+        S += s;
+        // relative to the mesh's first node (V is translation invariant for a closed surface)
+        const double* o = x;
+        const double ra[3] = {a[0] - o[0], a[1] - o[1], a[2] - o[2]}, rb[3] = {b[0] - o[0], b[1] - o[1], b[2] - o[2]},
+                     rc[3] = {c[0] - o[0], c[1] - o[1], c[2] - o[2]};
+        V6 += ra[0] * (rb[1] * rc[2] - rb[2] * rc[1]) + ra[1] * (rb[2] * rc[0] - rb[0] * rc[2]) +
+              ra[2] * (rb[0] * rc[1] - rb[1] * rc[0]);
+    }
+    *S0_tot = S;
+    *V0 = V6 / 6.0;
+}
 }  // namespace plb
 
 using namespace plb;
@@ -174,6 +205,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->spread_current = false; c->forces_valid = false; c->populated = false;
     c->launches = 0;
     c->n_ranges = 0;
+    c->n_tris = 0; c->n_cons = 0;
     c->tile_cap = 512;
     c->sm_count = sms;
     c->mesh_node_off.push_back(0);
@@ -373,6 +405,7 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
         ctx->n_edges += n_edges;
         ctx->mesh_node_off.push_back(ctx->n_nodes);
         ctx->mesh_edge_off.push_back(ctx->n_edges);
+        ctx->mesh_constrained.push_back(0);
     }
     ctx->forces_valid = false;
     ctx->spread_current = false;
@@ -382,6 +415,80 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
 int ib_add_mesh(plb_ctx* ctx, int n_nodes, const double* h_xyz, int n_edges, const int* h_edges, const float* h_rest,
                 float k, int* out_mesh_id) {
     return ib_add_meshes(ctx, 1, n_nodes, h_xyz, n_edges, h_edges, h_rest, k, out_mesh_id);
+}
+
+int ib_set_triangles(plb_ctx* ctx, int first_mesh_id, int n_meshes, int n_tris, const int* h_tris,
+                     const double* h_ref_xyz, float k_s, float k_t, float k_v) {
+    REQUIRE_CTX(ctx);
+    const int total = (int)ctx->mesh_node_off.size() - 1;
+    if (first_mesh_id < 0 || n_meshes < 1 || first_mesh_id + n_meshes > total || n_tris < 1 || !h_tris ||
+        k_s < 0.f || k_t < 0.f || k_v < 0.f) {
+        set_error("ib_set_triangles: invalid argument");
+        return PLB_ERR_ARG;
+    }
+    const long nn = ctx->mesh_node_off[first_mesh_id + 1] - ctx->mesh_node_off[first_mesh_id];
+    for (int s = 0; s < n_meshes; ++s) {
+        if (ctx->mesh_node_off[first_mesh_id + s + 1] - ctx->mesh_node_off[first_mesh_id + s] != nn) {
+            set_error("ib_set_triangles: meshes %d..%d do not share one topology", first_mesh_id, first_mesh_id + n_meshes - 1);
+            return PLB_ERR_ARG;
+        }
+        if (ctx->mesh_constrained[first_mesh_id + s]) {
+            set_error("ib_set_triangles: mesh %d already has triangles", first_mesh_id + s);
+            return PLB_ERR_ORDER;
+        }
+    }
+    for (int t = 0; t < 3 * n_tris; ++t)
+        if (h_tris[t] < 0 || h_tris[t] >= nn) {
+            set_error("ib_set_triangles: triangle %d has a node index out of range", t / 3);
+            return PLB_ERR_ARG;
+        }
+    if (ctx->n_tris + (long)n_meshes * n_tris > ctx->cap_tris || ctx->n_cons + n_meshes > ctx->cap_cons) {
+        set_error("ib_set_triangles: capacity exceeded (%ld/%ld triangles)", ctx->n_tris + (long)n_meshes * n_tris, ctx->cap_tris);
+        return PLB_ERR_WORKSPACE;
+    }
+    // the unstressed shape: shared h_ref_xyz, or each mesh's current positions
+    std::vector<double> cur;
+    if (!h_ref_xyz) {
+        cur.resize((size_t)3 * ctx->n_nodes);
+        const int rc = ib_read_nodes(ctx, cur.data());
+        if (rc && rc != PLB_ERR_NODE_LEFT) return rc;
+    }
+    std::vector<int4> tg((size_t)n_meshes * n_tris);
+    std::vector<float> s0((size_t)n_meshes * n_tris);
+    std::vector<MeshConstraint> mc((size_t)n_meshes);
+    for (int s = 0; s < n_meshes; ++s) {
+        const long noff = ctx->mesh_node_off[first_mesh_id + s];
+        const double* ref = h_ref_xyz ? h_ref_xyz : cur.data() + 3 * noff;
+        MeshConstraint& m = mc[s];
+        reference_area_volume(ref, n_tris, h_tris, s0.data() + (size_t)s * n_tris, &m.S0_tot, &m.V0);
+        for (int t = 0; t < n_tris; ++t) {
+            if (!(s0[(size_t)s * n_tris + t] > 0.f)) {
+                set_error("ib_set_triangles: triangle %d of the unstressed shape has zero area", t);
+                return PLB_ERR_ARG;
+            }
+            tg[(size_t)s * n_tris + t] = make_int4((int)(noff + h_tris[3 * t]), (int)(noff + h_tris[3 * t + 1]),
+                                                   (int)(noff + h_tris[3 * t + 2]), 0);
+        }
+        if (!(m.V0 > 0.0)) {
+            set_error("ib_set_triangles: the surface is not closed or not oriented outwards (V_0 = %g)", m.V0);
+            return PLB_ERR_ARG;
+        }
+        m.tri_first = (int)(ctx->n_tris + (long)s * n_tris);
+        m.tri_count = n_tris;
+        m.node_first = (int)noff;
+        m.pad = 0; m.pad2 = 0.f;
+        m.k_s = k_s; m.k_t = k_t; m.k_v = k_v;
+    }
+    int rc = cuda_check(cudaMemcpyAsync(ctx->tris + ctx->n_tris, tg.data(), tg.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream), "upload triangles");
+    if (!rc) rc = cuda_check(cudaMemcpyAsync(ctx->tri_S0 + ctx->n_tris, s0.data(), s0.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream), "upload triangle areas");
+    if (!rc) rc = cuda_check(cudaMemcpyAsync(ctx->cons + ctx->n_cons, mc.data(), mc.size() * sizeof(MeshConstraint), cudaMemcpyHostToDevice, ctx->stream), "upload mesh constraints");
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    if (rc) return rc;
+    ctx->n_tris += (long)n_meshes * n_tris;
+    ctx->n_cons += n_meshes;
+    for (int s = 0; s < n_meshes; ++s) ctx->mesh_constrained[first_mesh_id + s] = 1;
+    ctx->forces_valid = false;
+    return PLB_OK;
 }
 
 int ib_compute_membrane_forces(plb_ctx* ctx, float noise_sigma, unsigned long long noise_seed, unsigned long long step) {

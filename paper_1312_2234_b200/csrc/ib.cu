@@ -56,6 +56,93 @@ __global__ void __launch_bounds__(256) edge_force_kernel(const double* __restric
 }
 
 // ---------------------------------------------------------------------------------------------
+// S1b: area and volume constraint forces, Eq. 4-5 (L101-108):
+//   H = k_s (S_tot - S0_tot)^2/(2 S0_tot) + sum_tri k_t (S - S_0)^2/(2 S_0) + k_v (V - V_0)^2/(2 V_0)
+//   S = |n|/2, n = (X_b - X_a) x (X_c - X_a);  V = (1/6) sum_tri X_a . (X_b x X_c)
+//   F_a -= [k_s (S_tot - S0_tot)/S0_tot + k_t (S - S_0)/S_0] (1/2) nhat x (X_c - X_b)
+//          + k_v (V - V_0)/V_0 (1/6) X_b x X_c                     (cyclic in a, b, c)
+// One thread block per constrained mesh: pass 1 reduces S_tot and V over the mesh's triangles in
+// a fixed order (deterministic), pass 2 scatters the forces (one vector atomic per corner).
+// Geometry in fp64 relative to the mesh's first node (positions reach ~1e3, S - S_0 ~ 1e-3 S;
+// V and its gradient summed over a closed surface do not depend on the origin).
+// ---------------------------------------------------------------------------------------------
+constexpr int CON_THREADS = 256;
+
+struct TriGeom {
+    double ax, ay, az, bx, by, bz, cx, cy, cz;   // corners relative to the reference node
+    double nx, ny, nz, len;                      // n = (b - a) x (c - a), |n|
+};
+
+__device__ __forceinline__ TriGeom tri_geom(const double* __restrict__ X, const double* __restrict__ Y,
+                                            const double* __restrict__ Z, const int4 t, const double ox,
+                                            const double oy, const double oz) {
+    TriGeom g;
+    g.ax = __ldg(X + t.x) - ox; g.ay = __ldg(Y + t.x) - oy; g.az = __ldg(Z + t.x) - oz;
+    g.bx = __ldg(X + t.y) - ox; g.by = __ldg(Y + t.y) - oy; g.bz = __ldg(Z + t.y) - oz;
+    g.cx = __ldg(X + t.z) - ox; g.cy = __ldg(Y + t.z) - oy; g.cz = __ldg(Z + t.z) - oz;
+    const double ux = g.bx - g.ax, uy = g.by - g.ay, uz = g.bz - g.az;
+    const double vx = g.cx - g.ax, vy = g.cy - g.ay, vz = g.cz - g.az;
+    g.nx = uy * vz - uz * vy; g.ny = uz * vx - ux * vz; g.nz = ux * vy - uy * vx;
+    g.len = sqrt(g.nx * g.nx + g.ny * g.ny + g.nz * g.nz);
+    return g;
+}
+
+__device__ __forceinline__ double block_sum(double v, double* scratch) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) scratch[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double tot = 0.0;
+#pragma unroll
+    for (int w = 0; w < CON_THREADS / 32; ++w) tot += scratch[w];
+    return tot;
+}
+
+__global__ void __launch_bounds__(CON_THREADS) constraint_force_kernel(
+    const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
+    const int4* __restrict__ tris, const float* __restrict__ tri_S0, const MeshConstraint* __restrict__ cons,
+    float4* __restrict__ F) {
+    __shared__ double scratch[CON_THREADS / 32];
+    const MeshConstraint m = cons[blockIdx.x];
+    const double ox = __ldg(X + m.node_first), oy = __ldg(Y + m.node_first), oz = __ldg(Z + m.node_first);
+    double S = 0.0, V6 = 0.0;
+    for (int t = threadIdx.x; t < m.tri_count; t += CON_THREADS) {
+        const TriGeom g = tri_geom(X, Y, Z, __ldg(tris + m.tri_first + t), ox, oy, oz);
+        S += 0.5 * g.len;
+        V6 += g.ax * (g.by * g.cz - g.bz * g.cy) + g.ay * (g.bz * g.cx - g.bx * g.cz) + g.az * (g.bx * g.cy - g.by * g.cx);
+    }
+    const double S_tot = block_sum(S, scratch);
+    const double V = block_sum(V6, scratch) * (1.0 / 6.0);
+    const double alpha = (double)m.k_s * (S_tot - m.S0_tot) / m.S0_tot;
+    const double beta6 = (double)m.k_v * (V - m.V0) / m.V0 * (1.0 / 6.0);
+    for (int t = threadIdx.x; t < m.tri_count; t += CON_THREADS) {
+        const int4 tv = __ldg(tris + m.tri_first + t);
+        const TriGeom g = tri_geom(X, Y, Z, tv, ox, oy, oz);
+        const double S0 = (double)__ldg(tri_S0 + m.tri_first + t);
+        const double inv = g.len > 0.0 ? 1.0 / g.len : 0.0;
+        const double hx = g.nx * inv, hy = g.ny * inv, hz = g.nz * inv;            // nhat
+        const double cS = 0.5 * (alpha + (double)m.k_t * (0.5 * g.len - S0) / S0);
+        // corner a: nhat x (c - b), b x c;  corner b: nhat x (a - c), c x a;  corner c: nhat x (b - a), a x b
+        double ex = g.cx - g.bx, ey = g.cy - g.by, ez = g.cz - g.bz;
+        atomicAdd(F + tv.x, make_float4(
+            (float)-(cS * (hy * ez - hz * ey) + beta6 * (g.by * g.cz - g.bz * g.cy)),
+            (float)-(cS * (hz * ex - hx * ez) + beta6 * (g.bz * g.cx - g.bx * g.cz)),
+            (float)-(cS * (hx * ey - hy * ex) + beta6 * (g.bx * g.cy - g.by * g.cx)), 0.f));
+        ex = g.ax - g.cx; ey = g.ay - g.cy; ez = g.az - g.cz;
+        atomicAdd(F + tv.y, make_float4(
+            (float)-(cS * (hy * ez - hz * ey) + beta6 * (g.cy * g.az - g.cz * g.ay)),
+            (float)-(cS * (hz * ex - hx * ez) + beta6 * (g.cz * g.ax - g.cx * g.az)),
+            (float)-(cS * (hx * ey - hy * ex) + beta6 * (g.cx * g.ay - g.cy * g.ax)), 0.f));
+        ex = g.bx - g.ax; ey = g.by - g.ay; ez = g.bz - g.az;
+        atomicAdd(F + tv.z, make_float4(
+            (float)-(cS * (hy * ez - hz * ey) + beta6 * (g.ay * g.bz - g.az * g.by)),
+            (float)-(cS * (hz * ex - hx * ez) + beta6 * (g.az * g.bx - g.ax * g.bz)),
+            (float)-(cS * (hx * ey - hy * ex) + beta6 * (g.ax * g.by - g.ay * g.bx)), 0.f));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // 4-point cosine delta (Eq. 36): for a node at X, base = floor(X) - 1, frac = X - floor(X),
 // the four weights at cells base + o are phi(frac + 1 - o):
 //     o=0: (1 - s)/4   o=1: (1 + c)/4   o=2: (1 + s)/4   o=3: (1 - c)/4,
@@ -479,7 +566,12 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
             c->X[0], c->X[1], c->X[2], c->edges, c->edge_prm, c->F, c->n_edges, c->counters);
         c->launches++;
     }
-    return cuda_check(cudaGetLastError(), "edge_force_kernel");
+    if (c->n_cons) {
+        constraint_force_kernel<<<(unsigned)c->n_cons, CON_THREADS, 0, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->tris, c->tri_S0, c->cons, c->F);
+        c->launches++;
+    }
+    return cuda_check(cudaGetLastError(), "membrane force kernels");
 }
 
 int launch_clear_spread(Ctx* c, float4* g) {

@@ -46,6 +46,14 @@ struct LbmParams {
     float uw[3][2][3];         // [axis][face] wall velocity (on-site velocity walls)
 };
 
+// one constrained mesh (Eq. 4-5): its triangles [tri_first, tri_first + tri_count), a reference
+// node for the fp64 relative coordinates, the unstressed totals and the three coefficients
+struct MeshConstraint {
+    int tri_first, tri_count, node_first, pad;
+    double S0_tot, V0;
+    float k_s, k_t, k_v, pad2;
+};
+
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 
 // status bits raised by kernels (sticky)
@@ -104,6 +112,13 @@ struct Ctx {
     int2* edges;               // global node index pairs
     float2* edge_prm;          // (rest length, k)
     std::vector<long> mesh_node_off, mesh_edge_off;
+    // area / volume constraints (Eq. 4-5): triangles of the constrained meshes, mesh by mesh
+    long cap_tris, n_tris;
+    int4* tris;                // (a, b, c, 0) global node indices, outward orientation
+    float* tri_S0;             // unstressed triangle area
+    MeshConstraint* cons;      // one entry per constrained mesh = one thread block of the kernel
+    long cap_cons, n_cons;
+    std::vector<char> mesh_constrained;
     int2* ranges;              // node ranges [first, last) served by one thread block of the IB kernels
     long n_ranges;
     int tile_cap;              // cells of the shared-memory lattice tile of the IB kernels
@@ -128,6 +143,8 @@ int launch_read_macros(Ctx* c, float* d_rho, float* d_u);
 int launch_read_populations(Ctx* c, float* d_f);
 int launch_write_populations(Ctx* c, const float* d_f);
 int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigned long long step);
+// host-side geometry of the unstressed shape (set-up, not on the timed path)
+void reference_area_volume(const double* xyz, int n_tris, const int* tris, float* S0, double* S0_tot, double* V0);
 int launch_clear_spread(Ctx* c, float4* g);
 int launch_spread(Ctx* c, float4* g);
 int launch_interpolate_advance(Ctx* c);

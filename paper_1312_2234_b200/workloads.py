@@ -33,7 +33,7 @@ WALL_HH = 2     # Hecht-Harting on-site velocity wall (the paper's own, Eq. 23-3
 # --------------------------------------------------------------------------------------
 def icosphere(subdiv: int):
     """Unit icosphere: 12-vertex icosahedron, each triangle split in four `subdiv` times, new
-    vertices normalised, vertices in creation order.  Returns (verts[n,3] f64, tris[m,3] i32,
+    vertices normalised, vertices in creation order, triangles oriented outwards.  Returns (verts[n,3] f64, tris[m,3] i32,
     edges[e,2] i32 sorted unique (low, high)).  n = 10*4^s + 2, e = 30*4^s, m = 20*4^s."""
     t = (1.0 + math.sqrt(5.0)) / 2.0
     verts = [(-1, t, 0), (1, t, 0), (-1, -t, 0), (1, -t, 0),
@@ -159,6 +159,11 @@ class Workload:
     edges: np.ndarray | None = None     # [n_edges, 2] i32, mesh-local, shared topology
     rest: np.ndarray | None = None      # [n_edges] f64, shared rest lengths
     k_spring: float = 0.0
+    tris: np.ndarray | None = None      # [n_tris, 3] i32, mesh-local, outward oriented (shared topology)
+    ref_xyz: np.ndarray | None = None   # [n_nodes, 3] f64 unstressed body-frame shape (defines S_0, S0_tot, V_0)
+    k_area_global: float = 0.0        # k_s of Eq. 4 (0 = area / volume constraints off: the BASELINE configs)
+    k_area_local: float = 0.0         # k_t of Eq. 4
+    k_volume: float = 0.0             # k_v of Eq. 5
     force_sigma: float = 0.0          # per-step Philox normal force noise (C5)
     force_seed: int = 0
     u_ref: float = 1.0                # velocity scale for the |du| <= 1e-4 u_ref tolerance (u_wall, or u0 for C2)
@@ -187,18 +192,28 @@ def _walls_y(u_wall):
     return (PERIODIC, WALL, PERIODIC), u_lo, u_hi
 
 
+class MeshSet:
+    def __init__(self, xyz, edges, rest, tris, ref_xyz):
+        self.xyz, self.edges, self.rest, self.tris, self.ref_xyz = xyz, edges, rest, tris, ref_xyz
+
+    def fields(self):
+        return dict(mesh_xyz=self.xyz, edges=self.edges, rest=self.rest, tris=self.tris, ref_xyz=self.ref_xyz)
+
+
 def ellipsoid_meshes(subdiv, semi_axes, rotations, centres, radial_scale=None):
     """Common mesh recipe: unit icosphere -> scale by semi-axes (a, a, c) along
     body (x, y, z) -> rest lengths from this shape -> [optional] multiply each node's radius
-    vector by radial_scale[m] -> rotate -> translate.  Returns (xyz[n_meshes,n,3], edges, rest)."""
-    v, _, e = icosphere(subdiv)
+    vector by radial_scale[m] -> rotate -> translate.  Returns a MeshSet: xyz[n_meshes,n,3],
+    edges, rest lengths, triangles and the unstressed body-frame shape ref_xyz[n,3]."""
+    v, tris, e = icosphere(subdiv)
     body = v * np.asarray(semi_axes, dtype=np.float64)[None, :]
+    ref = body.copy()
     rest = edge_lengths(body, e)
     if radial_scale is not None:
         body = body * np.asarray(radial_scale, dtype=np.float64)[:, None]
     xyz = np.einsum("mab,nb->mna", np.asarray(rotations, dtype=np.float64), body)
     xyz += np.asarray(centres, dtype=np.float64)[:, None, :]
-    return np.ascontiguousarray(xyz), e, rest
+    return MeshSet(np.ascontiguousarray(xyz), e, rest, tris, ref)
 
 
 def shear_channel(name, nx, ny, nz, tau, u_wall, n_meshes, subdiv, semi_axes, k_spring, y_range,
@@ -210,10 +225,10 @@ def shear_channel(name, nx, ny, nz, tau, u_wall, n_meshes, subdiv, semi_axes, k_
     centres = place_centres(rng, n_meshes, (0.0, y_range[0], 0.0), (float(nx), y_range[1], float(nz)),
                             min_dist, periodic_len=(float(nx), None, float(nz)))
     R = random_rotations(rng, n_meshes)
-    xyz, e, rest = ellipsoid_meshes(subdiv, semi_axes, R, centres)
+    ms = ellipsoid_meshes(subdiv, semi_axes, R, centres)
     return Workload(name=name, nx=nx, ny=ny, nz=nz, tau=tau, kind=kind, u_lo=u_lo, u_hi=u_hi, steps=steps,
-                    u0=shear_field(nx, ny, nz, u_wall), mesh_xyz=xyz, edges=e, rest=rest,
-                    k_spring=k_spring, u_ref=u_wall, notes=list(notes))
+                    u0=shear_field(nx, ny, nz, u_wall), k_spring=k_spring, u_ref=u_wall, notes=list(notes),
+                    **ms.fields())
 
 
 def config1(nx=32, ny=32, nz=64, steps=200, subdiv=2, seed=SEED_BASE + 1):
@@ -223,12 +238,12 @@ def config1(nx=32, ny=32, nz=64, steps=200, subdiv=2, seed=SEED_BASE + 1):
     theta = 0.5 * math.pi * rng.random()            # tilt about the world x axis, [0, pi/2)
     n_nodes = 10 * 4 ** subdiv + 2
     xi = rng.random(n_nodes)                         # 5 % seeded radial compression
-    xyz, e, rest = ellipsoid_meshes(subdiv, (4.0, 4.0, 1.0), rot_x(theta)[None], [(nx / 2, ny / 2, nz / 2)],
-                                    radial_scale=1.0 - 0.05 * xi)
+    ms = ellipsoid_meshes(subdiv, (4.0, 4.0, 1.0), rot_x(theta)[None], [(nx / 2, ny / 2, nz / 2)],
+                          radial_scale=1.0 - 0.05 * xi)
     return Workload(name="C1", nx=nx, ny=ny, nz=nz, tau=0.8, kind=kind, u_lo=u_lo, u_hi=u_hi, steps=steps,
                     u0=shear_field(nx, ny, nz, 0.05), noise_amp=1e-4, noise_seed=seed,
-                    mesh_xyz=xyz, edges=e, rest=rest, k_spring=0.01, u_ref=0.05,
-                    notes=["tilt = rotation about world x by (pi/2)*xi"])
+                    k_spring=0.01, u_ref=0.05,
+                    notes=["tilt = rotation about world x by (pi/2)*xi"], **ms.fields())
 
 
 def config2(n=256, steps=1000, u0=0.02):
@@ -262,9 +277,9 @@ def config5(n=256, grid_xz=64, layers=2, steps=200, subdiv=4, seed=SEED_BASE + 5
     centres = np.stack([pitch * (p.ravel() + 0.5), 8.0 + 8.0 * q.ravel(), pitch * (r.ravel() + 0.5)], axis=1)
     centres = centres + (rng.random(centres.shape) - 0.5)
     R = random_rotations(rng, centres.shape[0])
-    xyz, e, rest = ellipsoid_meshes(subdiv, (5.0, 5.0, 1.25), R, centres)
+    ms = ellipsoid_meshes(subdiv, (5.0, 5.0, 1.25), R, centres)
     return Workload(name="C5", nx=n, ny=n, nz=n, tau=0.7, kind=kind, u_lo=u_lo, u_hi=u_hi, steps=steps,
-                    u0=shear_field(n, n, n, 0.05), mesh_xyz=xyz, edges=e, rest=rest, k_spring=0.02,
+                    u0=shear_field(n, n, n, 0.05), k_spring=0.02, **ms.fields(),
                     force_sigma=1e-4, force_seed=seed, u_ref=0.05,
                     notes=["centres on a jittered %dx%dx%d lattice (spacing >= 3): the config's minimum centre "
                            "spacing of 11 cannot hold 8192 platelets in a 256x20x256 slab; meshes interpenetrate"
@@ -285,6 +300,21 @@ def with_onsite_walls(w: Workload) -> Workload:
     v.u0 = u.reshape(3, -1)
     v.name = w.name + "-onsite"
     v.notes = list(w.notes) + ["walls: Hecht-Harting on-site velocity condition (PAPER.md Eq. 23-30)"]
+    return v
+
+
+def with_area_volume_constraints(w: Workload, ratio=4.4) -> Workload:
+    """The same workload with the paper's area and volume constraints switched on (Eq. 4-5;
+    SURVEY.md NEXT-2).  Table 2 gives k_s = k_t = 6000 k_B T/l_0^2 = 4.4e-3 N/m against the spring
+    stiffness k = 2 E dx/5 = 1e-3 N/m (L94), i.e. k_s/k = k_t/k = 4.4; k_v (an energy per volume)
+    is taken as k_s per lattice spacing."""
+    import copy
+    v = copy.copy(w)
+    assert w.tris is not None
+    v.k_area_global = v.k_area_local = ratio * w.k_spring
+    v.k_volume = ratio * w.k_spring
+    v.name = w.name + "-constrained"
+    v.notes = list(w.notes) + ["area / volume constraints on (PAPER.md Eq. 4-5): k_s = k_t = k_v = %.3g" % v.k_volume]
     return v
 
 
