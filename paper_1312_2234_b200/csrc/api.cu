@@ -44,6 +44,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     float* f1 = w.take<float>((size_t)Q * cells);
     unsigned* seg_mask = w.take<unsigned>((size_t)(n_segs + 31) / 32);
     int* counters = w.take<int>(64);
+    int* seg_list = w.take<int>((size_t)n_segs);
     double* X0 = w.take<double>((size_t)max_nodes);
     double* X1 = w.take<double>((size_t)max_nodes);
     double* X2 = w.take<double>((size_t)max_nodes);
@@ -61,7 +62,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
         c->tris = tris; c->tri_S0 = tri_S0; c->cons = cons;
         c->cap_tris = 2 * max_nodes; c->cap_cons = max_nodes / 4 + 1;
         c->f[0] = f0; c->f[1] = f1;
-        c->seg_mask = seg_mask; c->counters = counters;
+        c->seg_mask = seg_mask; c->counters = counters; c->seg_list = seg_list;
         c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
         c->edges = edges; c->edge_prm = eprm; c->ranges = ranges;
     }
@@ -206,6 +207,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->launches = 0;
     c->n_ranges = 0;
     c->n_tris = 0; c->n_cons = 0;
+    c->list_parity = 0;
     c->tile_cap = 512;
     c->sm_count = sms;
     c->mesh_node_off.push_back(0);

@@ -148,22 +148,6 @@ __global__ void __launch_bounds__(CON_THREADS) constraint_force_kernel(
 //     o=0: (1 - s)/4   o=1: (1 + c)/4   o=2: (1 + s)/4   o=3: (1 - c)/4,
 // s = sin(pi frac/2), c = cos(pi frac/2)   (cos(a + pi/2) = -sin a, cos(a - pi) = -cos a).
 // ---------------------------------------------------------------------------------------------
-struct Axis {
-    int base;      // floor(X) - 1 (unwrapped)
-    float s, c;
-};
-
-__device__ __forceinline__ Axis axis_of(const double x) {
-    const double fl = floor(x);
-    Axis a;
-    a.base = (int)fl - 1;
-    sincospif(0.5f * (float)(x - fl), &a.s, &a.c);
-    return a;
-}
-__device__ __forceinline__ float weight_of(const Axis& a, const int o) {
-    const float t = (o == 0) ? -a.s : (o == 1) ? a.c : (o == 2) ? a.s : -a.c;
-    return 0.25f + 0.25f * t;
-}
 // wrapped index on a periodic axis; -1 if dropped on a wall axis
 __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
     if (q >= 0 && q < n) return q;
@@ -187,29 +171,36 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
 //                 the 19 pulled populations (no velocity field in HBM) -> nodes gather from the tile.
 // A range whose bounding box does not fit the tile (a non-compact "mesh") takes the direct path:
 // global REDs per (node, cell) and on-the-fly cell moments.  Both paths compute the same sums.
-// Within a block 16 lanes serve one node: lane = (ox, oy), loop over oz.
+// Within a block FOUR lanes serve one node: lane = ox (the x offset of the stencil column), each
+// lane walks the 4 x 4 (oy, oz) cells of its column; the lanes also share the per-node set-up
+// (lane a < 3 does floor / sincospi of axis a) and finish with a 4-lane shuffle reduction.
 // ---------------------------------------------------------------------------------------------
 constexpr int IB_THREADS = 512;
-constexpr int IB_CHUNK = 256;                      // nodes whose stencil records are staged at a time
-constexpr int LANES_PER_NODE = 16;
-constexpr int IB_GROUPS = IB_THREADS / LANES_PER_NODE;
+constexpr int NODE_LANES = 4;
+constexpr int IB_GROUPS = IB_THREADS / NODE_LANES;
 
 struct MeshTile {
     int o[3];            // unwrapped lattice coordinate of tile cell (0,0,0)
     int e[3];            // extent in cells
     int lo[3], hi[3];    // tile coordinates [lo, hi) that exist on the lattice (wall axes clip)
     int enabled;
+    int clipped;         // some [lo, hi) is smaller than the extent: stencils need the range check
+    int interior;        // every tile cell and its 18 neighbours lie inside the grid: no wrap, no wall
     int mn[3], mx[3];    // reduction scratch: min / max of floor(X)
     unsigned fmax_bits;  // reduction scratch: largest |F| component (non-negative float bits)
     int n_need;          // interpolate: number of tile cells some node needs
 };
 
-// set the activity bit of the 8-cell segment of a cell
-__device__ __forceinline__ void mark_segment(const int cell, unsigned* __restrict__ seg_mask) {
+// set the activity bit of the 8-cell segment of a cell; the thread that sets it first also appends
+// the segment to the list the next ib_spread clears from
+__device__ __forceinline__ void mark_segment(const int cell, unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
+                                             int* __restrict__ seg_count) {
     const int seg = cell >> SEG_SHIFT;
     const unsigned bit = 1u << (seg & 31);
     unsigned* word = seg_mask + (seg >> 5);
-    if ((*(volatile unsigned*)word & bit) == 0u) atomicOr(word, bit);
+    if ((*(volatile unsigned*)word & bit) == 0u) {
+        if ((atomicOr(word, bit) & bit) == 0u) seg_list[atomicAdd(seg_count, 1)] = seg;
+    }
 }
 
 // bounding box of the supports of nodes [n0, n1) -> tile geometry (all threads of the block);
@@ -249,7 +240,7 @@ __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict
     if (threadIdx.x == 0) {
         const int n[3] = {p.nx, p.ny, p.nz};
         long long vol = 1;
-        bool ok = n1 > n0;
+        bool ok = n1 > n0, clipped = false, interior = true;
         for (int a = 0; a < 3; ++a) {
             const long long ext = (long long)T.mx[a] - (long long)T.mn[a] + 4;
             ok = ok && ext <= (long long)cap;
@@ -264,8 +255,12 @@ __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict
             } else {
                 T.lo[a] = 0; T.hi[a] = T.e[a];
             }
+            clipped = clipped || T.lo[a] != 0 || T.hi[a] != T.e[a];
+            interior = interior && (long long)T.o[a] >= 1 && (long long)T.o[a] + ext <= (long long)n[a] - 1;
         }
         T.enabled = ok ? 1 : 0;
+        T.clipped = clipped ? 1 : 0;
+        T.interior = (ok && interior) ? 1 : 0;
     }
     __syncthreads();
 }
@@ -281,95 +276,119 @@ __device__ __forceinline__ Cell tile_cell(const MeshTile& T, const int t, const 
     return c;
 }
 
-// per-node stencil records of one chunk of nodes, in shared memory
-struct Chunk {
-    int* b;        // [3][IB_CHUNK] base = floor(X) - 1, tile-relative if the tile is enabled
-    float* sc;     // [6][IB_CHUNK] sin / cos of pi frac / 2 per axis
+// The stencil of one node as its four lanes see it: lane `sub` owns the column ox = sub.
+struct NodeStencil {
+    int bx, by, bz;        // base = floor(X) - 1 per axis, minus `origin`
+    float wx;              // weight of this lane's ox
+    float wy[4], wz[4];    // weights of oy, oz = 0..3
 };
 
-__device__ __forceinline__ void chunk_record(const Chunk& ch, const MeshTile& T, const bool tiled, const int r,
-                                             const double x, const double y, const double z) {
-    const Axis ax = axis_of(x), ay = axis_of(y), az = axis_of(z);
-    ch.b[r] = tiled ? ax.base - T.o[0] : ax.base;
-    ch.b[IB_CHUNK + r] = tiled ? ay.base - T.o[1] : ay.base;
-    ch.b[2 * IB_CHUNK + r] = tiled ? az.base - T.o[2] : az.base;
-    ch.sc[r] = ax.s; ch.sc[IB_CHUNK + r] = ax.c;
-    ch.sc[2 * IB_CHUNK + r] = ay.s; ch.sc[3 * IB_CHUNK + r] = ay.c;
-    ch.sc[4 * IB_CHUNK + r] = az.s; ch.sc[5 * IB_CHUNK + r] = az.c;
+// phi(frac + 1 - o), o = 0..3, from s = sin(pi frac/2), c = cos(pi frac/2)  (see weight_of)
+__device__ __forceinline__ void weights4(const float s, const float c, float (&w)[4]) {
+    w[0] = fmaf(-0.25f, s, 0.25f); w[1] = fmaf(0.25f, c, 0.25f);
+    w[2] = fmaf(0.25f, s, 0.25f);  w[3] = fmaf(-0.25f, c, 0.25f);
 }
-__device__ __forceinline__ Axis chunk_axis(const Chunk& ch, const int a, const int r) {
-    Axis ax;
-    ax.base = ch.b[a * IB_CHUNK + r];
-    ax.s = ch.sc[2 * a * IB_CHUNK + r];
-    ax.c = ch.sc[(2 * a + 1) * IB_CHUNK + r];
-    return ax;
+
+// All 32 lanes call this (m clamped by the caller); lane a < 3 of each 4-lane group evaluates
+// axis a (fp64 floor, sincospi of the fraction), then the group exchanges by shuffle.
+template <bool WEIGHTS>
+__device__ __forceinline__ NodeStencil node_stencil(const double* X, const double* Y, const double* Z, const int m, const int sub,
+                                                    const int o0, const int o1, const int o2) {
+    const double* P = sub == 1 ? Y : (sub == 2 ? Z : X);
+    const double x = P[m];
+    const double fl = floor(x);
+    const int base = (int)fl - 1 - (sub == 1 ? o1 : (sub == 2 ? o2 : o0));
+    float s = 0.f, c = 0.f;
+    if (WEIGHTS) sincospif(0.5f * (float)(x - fl), &s, &c);
+    NodeStencil st;
+    st.bx = __shfl_sync(0xffffffffu, base, 0, NODE_LANES);
+    st.by = __shfl_sync(0xffffffffu, base, 1, NODE_LANES);
+    st.bz = __shfl_sync(0xffffffffu, base, 2, NODE_LANES);
+    if (WEIGHTS) {
+        const float sx = __shfl_sync(0xffffffffu, s, 0, NODE_LANES), cx = __shfl_sync(0xffffffffu, c, 0, NODE_LANES);
+        const float sy = __shfl_sync(0xffffffffu, s, 1, NODE_LANES), cy = __shfl_sync(0xffffffffu, c, 1, NODE_LANES);
+        const float sz = __shfl_sync(0xffffffffu, s, 2, NODE_LANES), cz = __shfl_sync(0xffffffffu, c, 2, NODE_LANES);
+        const float t = (sub & 1) ? cx : sx;                       // o = 0: -s, 1: +c, 2: +s, 3: -c
+        st.wx = fmaf((sub == 0 || sub == 3) ? -0.25f : 0.25f, t, 0.25f);
+        weights4(sy, cy, st.wy);
+        weights4(sz, cz, st.wz);
+    }
+    return st;
+}
+
+// one lane's column of the spread into the shared fixed-point tile
+template <bool CHECK>
+__device__ __forceinline__ void spread_column(int* __restrict__ tile, const int cap, const MeshTile& T,
+                                              const NodeStencil& st, const int tx, const float fx, const float fy,
+                                              const float fz) {
+    const int e0 = T.e[0], e10 = T.e[0] * T.e[1];
+    if (CHECK && (tx < T.lo[0] || tx >= T.hi[0])) return;
+    const int t0 = (st.bz * T.e[1] + st.by) * e0 + tx;
+#pragma unroll
+    for (int oz = 0; oz < 4; ++oz) {
+        if (CHECK && (st.bz + oz < T.lo[2] || st.bz + oz >= T.hi[2])) continue;
+#pragma unroll
+        for (int oy = 0; oy < 4; ++oy) {
+            if (CHECK && (st.by + oy < T.lo[1] || st.by + oy >= T.hi[1])) continue;
+            const float W = st.wy[oy] * st.wz[oz];
+            const int t = t0 + oz * e10 + oy * e0;
+            atomicAdd(tile + t, __float2int_rn(W * fx));
+            atomicAdd(tile + cap + t, __float2int_rn(W * fy));
+            atomicAdd(tile + 2 * cap + t, __float2int_rn(W * fz));
+        }
+    }
 }
 
 // S2: g_ijk += F_m phi phi phi (Eq. 34).  Also sets the activity bits of the touched segments.
 __global__ void __launch_bounds__(IB_THREADS) spread_mesh_kernel(
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
-    unsigned* __restrict__ seg_mask, const LbmParams p, const int cap) {
+    unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
+    const int cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
     int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point
-    Chunk ch;
-    ch.b = tile + 3 * (size_t)cap;
-    ch.sc = reinterpret_cast<float*>(ch.b + 3 * IB_CHUNK);
-    float* rF = ch.sc + 6 * IB_CHUNK;                                  // [3][IB_CHUNK]
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
     tile_setup(T, X, Y, Z, F, n0, n1, p, cap);
     const float fmax = __uint_as_float(T.fmax_bits);
     if (!(fmax > 0.f)) return;                                         // nothing to spread
     const bool tiled = T.enabled != 0 && fmax < 3.0e38f;
-    const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
+    const int ncell = tiled ? T.e[0] * T.e[1] * T.e[2] : 0;
     // |tile value| <= n_nodes * max W * max|F| = bound; scale = 2^k with bound * scale < 2^30
     const int k = max(-100, min(100, 29 - ilogbf(0.125f * (float)(n1 - n0) * fmax)));
     const float scale = tiled ? ldexpf(1.0f, k) : 1.0f, inv_scale = ldexpf(1.0f, -k);
     for (int t = tid; t < ncell; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
-    const int sub = tid & (LANES_PER_NODE - 1), ox = sub & 3, oy = sub >> 2;
-    for (int c0 = n0; c0 < n1; c0 += IB_CHUNK) {
-        __syncthreads();
-        if (tid < IB_CHUNK && c0 + tid < n1) {
-            const int m = c0 + tid;
-            chunk_record(ch, T, tiled, tid, __ldg(X + m), __ldg(Y + m), __ldg(Z + m));
-            const float4 Fm = __ldg(F + m);
-            rF[tid] = Fm.x * scale; rF[IB_CHUNK + tid] = Fm.y * scale; rF[2 * IB_CHUNK + tid] = Fm.z * scale;
-        }
-        __syncthreads();
-        const int cnt = min(IB_CHUNK, n1 - c0);
-        for (int r = tid / LANES_PER_NODE; r < cnt; r += IB_GROUPS) {
-            const Axis ax = chunk_axis(ch, 0, r), ay = chunk_axis(ch, 1, r), az = chunk_axis(ch, 2, r);
-            const float Fx = rF[r], Fy = rF[IB_CHUNK + r], Fz = rF[2 * IB_CHUNK + r];
-            const float wxy = weight_of(ax, ox) * weight_of(ay, oy);
-            if (tiled) {
-                const int tx = ax.base + ox, ty = ay.base + oy;
-                if (tx < T.lo[0] || tx >= T.hi[0] || ty < T.lo[1] || ty >= T.hi[1]) continue;
+    __syncthreads();
+    const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
+    const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
+    for (int mb = n0; mb < n1; mb += IB_GROUPS) {                      // warp-uniform trip count
+        const bool valid = mb + group < n1;
+        const int m = valid ? mb + group : n1 - 1;
+        const NodeStencil st = node_stencil<true>(X, Y, Z, m, sub, o0, o1, o2);
+        const float4 Fm = __ldg(F + m);
+        if (!valid) continue;
+        const float fx = Fm.x * scale * st.wx, fy = Fm.y * scale * st.wx, fz = Fm.z * scale * st.wx;
+        if (tiled) {
+            if (T.clipped) spread_column<true>(tile, cap, T, st, st.bx + sub, fx, fy, fz);
+            else           spread_column<false>(tile, cap, T, st, st.bx + sub, fx, fy, fz);
+        } else {
+            const int qx = wrap_index(st.bx + sub, p.nx, p.wall[0]);
+            if (qx < 0) continue;
 #pragma unroll
-                for (int oz = 0; oz < 4; ++oz) {
-                    const int tz = az.base + oz;
-                    if (tz < T.lo[2] || tz >= T.hi[2]) continue;
-                    const float W = wxy * weight_of(az, oz);
-                    const int t = (tz * e1 + ty) * e0 + tx;
-                    atomicAdd(tile + t, __float2int_rn(W * Fx));
-                    atomicAdd(tile + cap + t, __float2int_rn(W * Fy));
-                    atomicAdd(tile + 2 * cap + t, __float2int_rn(W * Fz));
-                }
-            } else {
-                const int qx = wrap_index(ax.base + ox, p.nx, p.wall[0]);
-                const int qy = wrap_index(ay.base + oy, p.ny, p.wall[1]);
-                if (qx < 0 || qy < 0) continue;
+            for (int oz = 0; oz < 4; ++oz) {
+                const int qz = wrap_index(st.bz + oz, p.nz, p.wall[2]);
+                if (qz < 0) continue;
 #pragma unroll
-                for (int oz = 0; oz < 4; ++oz) {
-                    const int qz = wrap_index(az.base + oz, p.nz, p.wall[2]);
-                    if (qz < 0) continue;
-                    const float W = wxy * weight_of(az, oz);
+                for (int oy = 0; oy < 4; ++oy) {
+                    const int qy = wrap_index(st.by + oy, p.ny, p.wall[1]);
+                    if (qy < 0) continue;
+                    const float W = st.wy[oy] * st.wz[oz];
                     const int cell = qx + p.nx * (qy + p.ny * qz);
-                    atomicAdd(g + cell, make_float4(W * Fx, W * Fy, W * Fz, 0.f));
-                    mark_segment(cell, seg_mask);
+                    atomicAdd(g + cell, make_float4(W * fx, W * fy, W * fz, 0.f));
+                    mark_segment(cell, seg_mask, seg_list, seg_count);
                 }
             }
         }
@@ -382,67 +401,86 @@ __global__ void __launch_bounds__(IB_THREADS) spread_mesh_kernel(
             const Cell c = tile_cell(T, t, p);
             const int cell = c.i + p.nx * (c.j + p.ny * c.k);
             atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
-            mark_segment(cell, seg_mask);
+            mark_segment(cell, seg_mask, seg_list, seg_count);
         }
     }
 }
 
-// zero the cells of the segments the previous spread touched, and drop their activity bits:
-// one thread per segment (a 128-byte line of the forcing field), one warp per mask word
+// zero the cells of the segments the previous spread touched (its list), and drop their activity
+// bits: 8 lanes per segment, one float4 each = one 128-byte line per segment.  Also resets the
+// counter the coming spread will append to (the two counters alternate).
 __global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ g, unsigned* __restrict__ seg_mask,
-                                                           const int n_segs, const int cells) {
-    const int seg = blockIdx.x * 256 + threadIdx.x;
-    const int word = seg >> 5;
-    const unsigned m = (seg < n_segs) ? seg_mask[word] : 0u;
-    if (__ballot_sync(0xffffffffu, m != 0u) == 0u) return;
-    if ((m >> (seg & 31)) & 1u) {
-        const int c0 = seg * SEG;
-#pragma unroll
-        for (int c = 0; c < SEG; ++c)
-            if (c0 + c < cells) g[c0 + c] = make_float4(0.f, 0.f, 0.f, 0.f);
+                                                           const int* __restrict__ seg_list, const int* __restrict__ count_done,
+                                                           int* __restrict__ count_next, const int cells) {
+    const int n = *count_done;
+    const int lane8 = threadIdx.x & (SEG - 1);
+    const int stride = gridDim.x * (256 / SEG);
+    for (int e = blockIdx.x * (256 / SEG) + (threadIdx.x >> SEG_SHIFT); e < n; e += stride) {
+        const int seg = __ldg(seg_list + e);
+        const int c = seg * SEG + lane8;
+        if (c < cells) g[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (lane8 == 0) seg_mask[seg >> 5] = 0u;          // every set bit of the word is in the list
     }
-    __syncwarp();
-    if ((seg & 31) == 0 && m != 0u) seg_mask[word] = 0u;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *count_next = 0;
+}
+
+// one lane's column of the gather from the shared velocity tile
+template <bool CHECK>
+__device__ __forceinline__ void gather_column(const float4* __restrict__ tile, const MeshTile& T, const NodeStencil& st,
+                                              const int tx, float& ux, float& uy, float& uz) {
+    const int e0 = T.e[0], e10 = T.e[0] * T.e[1];
+    if (CHECK && (tx < T.lo[0] || tx >= T.hi[0])) return;
+    const float4* col = tile + ((st.bz * T.e[1] + st.by) * e0 + tx);
+#pragma unroll
+    for (int oz = 0; oz < 4; ++oz) {
+        if (CHECK && (st.bz + oz < T.lo[2] || st.bz + oz >= T.hi[2])) continue;
+#pragma unroll
+        for (int oy = 0; oy < 4; ++oy) {
+            if (CHECK && (st.by + oy < T.lo[1] || st.by + oy >= T.hi[1])) continue;
+            const float W = st.wy[oy] * st.wz[oz];
+            const float4 v = col[oz * e10 + oy * e0];
+            ux = fmaf(W, v.x, ux);
+            uy = fmaf(W, v.y, uy);
+            uz = fmaf(W, v.z, uz);
+        }
+    }
 }
 
 // S4 + S5: U_m = sum v phi phi phi (Eq. 33) with v = (sum c_i f_i + g/2)/rho of the state after
-// lbm_step (G11), by a 16-lane shuffle reduction over the 4x4x4 stencil, then
-// X_m += U_m in fp64.
+// lbm_step (G11), each of a node's four lanes summing its stencil column, then a 4-lane
+// shuffle reduction, then X_m += U_m in fp64.
 __global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
     double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z, float4* __restrict__ U,
     const int2* __restrict__ ranges, const float* __restrict__ src, const float4* __restrict__ g,
     int* __restrict__ counters, const LbmParams p, const int cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
-    float* tile = reinterpret_cast<float*>(smem_raw);                  // [3][cap] velocity
-    Chunk ch;
-    ch.b = reinterpret_cast<int*>(tile + 3 * (size_t)cap);
-    ch.sc = reinterpret_cast<float*>(ch.b + 3 * IB_CHUNK);
-    unsigned short* list = reinterpret_cast<unsigned short*>(ch.sc + 6 * IB_CHUNK);   // [cap] needed tile cells
+    float4* tile = reinterpret_cast<float4*>(smem_raw);                // [cap] (vx, vy, vz, rho)
+    unsigned short* list = reinterpret_cast<unsigned short*>(tile + cap);   // [cap] needed tile cells
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
     tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap);
     const bool tiled = T.enabled != 0;
     const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
+    const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
+    const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
     if (tiled) {
-        unsigned* need = reinterpret_cast<unsigned*>(tile);           // marks live in the x plane of the tile
+        unsigned* need = reinterpret_cast<unsigned*>(smem_raw);       // marks alias the (not yet filled) tile
         for (int t = tid; t < ncell; t += IB_THREADS) need[t] = 0u;
         __syncthreads();
-        for (int m = n0 + tid; m < n1; m += IB_THREADS) {             // the 4^3 cells each node needs
-            const int bx = (int)floor(X[m]) - 1 - T.o[0], by = (int)floor(Y[m]) - 1 - T.o[1],
-                      bz = (int)floor(Z[m]) - 1 - T.o[2];
-            for (int oz = 0; oz < 4; ++oz) {
-                const int tz = bz + oz;
-                if (tz < T.lo[2] || tz >= T.hi[2]) continue;
-                for (int oy = 0; oy < 4; ++oy) {
-                    const int ty = by + oy;
-                    if (ty < T.lo[1] || ty >= T.hi[1]) continue;
-                    const int row = (tz * e1 + ty) * e0;
+        for (int mb = n0; mb < n1; mb += IB_GROUPS) {                  // the 4^3 cells each node needs
+            const bool valid = mb + group < n1;
+            const NodeStencil st = node_stencil<false>(X, Y, Z, valid ? mb + group : n1 - 1, sub, o0, o1, o2);
+            const int tx = st.bx + sub;
+            if (!valid || tx < T.lo[0] || tx >= T.hi[0]) continue;
 #pragma unroll
-                    for (int ox = 0; ox < 4; ++ox) {
-                        const int tx = bx + ox;
-                        if (tx >= T.lo[0] && tx < T.hi[0]) need[row + tx] = 1u;
-                    }
+            for (int oz = 0; oz < 4; ++oz) {
+                const int tz = st.bz + oz;
+                if (tz < T.lo[2] || tz >= T.hi[2]) continue;
+#pragma unroll
+                for (int oy = 0; oy < 4; ++oy) {
+                    const int ty = st.by + oy;
+                    if (ty >= T.lo[1] && ty < T.hi[1]) need[(tz * e1 + ty) * e0 + tx] = 1u;
                 }
             }
         }
@@ -459,48 +497,43 @@ __global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
         }
         __syncthreads();
         const int n_need = T.n_need;
-        for (int e = tid; e < n_need; e += IB_THREADS) {
-            const int t = list[e];
-            const float4 v = cell_macros(src, g, p, tile_cell(T, t, p));
-            tile[t] = v.x; tile[cap + t] = v.y; tile[2 * cap + t] = v.z;
+        if (T.interior) {
+            const int sy = p.nx, sz = p.nx * p.ny;
+            const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
+            for (int e = tid; e < n_need; e += IB_THREADS) {
+                const int t = list[e];
+                const int x = t % e0, r = t / e0;
+                const int y = r % e1, z = r / e1;
+                tile[t] = cell_macros_interior(src, g, p, origin + x + sy * y + sz * z);
+            }
+        } else {
+            for (int e = tid; e < n_need; e += IB_THREADS) {
+                const int t = list[e];
+                tile[t] = cell_macros(src, g, p, tile_cell(T, t, p));
+            }
         }
+        __syncthreads();
     }
-    const int sub = tid & (LANES_PER_NODE - 1), ox = sub & 3, oy = sub >> 2;
-    for (int c0 = n0; c0 < n1; c0 += IB_CHUNK) {
-        __syncthreads();
-        if (tid < IB_CHUNK && c0 + tid < n1) {
-            const int m = c0 + tid;
-            chunk_record(ch, T, tiled, tid, X[m], Y[m], Z[m]);
-        }
-        __syncthreads();
-        const int cnt = min(IB_CHUNK, n1 - c0);
-        // the 16 lanes of a node iterate together: r is the same for a whole half-warp
-        for (int r = tid / LANES_PER_NODE; r < cnt; r += IB_GROUPS) {
-            const Axis ax = chunk_axis(ch, 0, r), ay = chunk_axis(ch, 1, r), az = chunk_axis(ch, 2, r);
-            const float wxy = weight_of(ax, ox) * weight_of(ay, oy);
-            float ux = 0.f, uy = 0.f, uz = 0.f;
-            if (tiled) {
-                const int tx = ax.base + ox, ty = ay.base + oy;
-                if (tx >= T.lo[0] && tx < T.hi[0] && ty >= T.lo[1] && ty < T.hi[1]) {
+    for (int mb = n0; mb < n1; mb += IB_GROUPS) {
+        const bool valid = mb + group < n1;
+        const int m = valid ? mb + group : n1 - 1;
+        const NodeStencil st = node_stencil<true>(X, Y, Z, m, sub, o0, o1, o2);
+        float ux = 0.f, uy = 0.f, uz = 0.f;
+        if (tiled) {
+            if (T.clipped) gather_column<true>(tile, T, st, st.bx + sub, ux, uy, uz);
+            else           gather_column<false>(tile, T, st, st.bx + sub, ux, uy, uz);
+        } else {
+            const int qx = wrap_index(st.bx + sub, p.nx, p.wall[0]);
+            if (qx >= 0) {
 #pragma unroll
-                    for (int oz = 0; oz < 4; ++oz) {
-                        const int tz = az.base + oz;
-                        if (tz < T.lo[2] || tz >= T.hi[2]) continue;
-                        const float W = wxy * weight_of(az, oz);
-                        const int t = (tz * e1 + ty) * e0 + tx;
-                        ux = fmaf(W, tile[t], ux);
-                        uy = fmaf(W, tile[cap + t], uy);
-                        uz = fmaf(W, tile[2 * cap + t], uz);
-                    }
-                }
-            } else {
-                const int qx = wrap_index(ax.base + ox, p.nx, p.wall[0]);
-                const int qy = wrap_index(ay.base + oy, p.ny, p.wall[1]);
-                if (qx >= 0 && qy >= 0) {
-                    for (int oz = 0; oz < 4; ++oz) {
-                        const int qz = wrap_index(az.base + oz, p.nz, p.wall[2]);
-                        if (qz < 0) continue;
-                        const float W = wxy * weight_of(az, oz);
+                for (int oz = 0; oz < 4; ++oz) {
+                    const int qz = wrap_index(st.bz + oz, p.nz, p.wall[2]);
+                    if (qz < 0) continue;
+#pragma unroll
+                    for (int oy = 0; oy < 4; ++oy) {
+                        const int qy = wrap_index(st.by + oy, p.ny, p.wall[1]);
+                        if (qy < 0) continue;
+                        const float W = st.wy[oy] * st.wz[oz];
                         Cell c;
                         c.i = qx; c.j = qy; c.k = qz;
                         const float4 v = cell_macros(src, g, p, c);
@@ -510,26 +543,27 @@ __global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
                     }
                 }
             }
-            const unsigned half = 0xffffu << (threadIdx.x & 16);
+        }
+        ux *= st.wx; uy *= st.wx; uz *= st.wx;
 #pragma unroll
-            for (int o = LANES_PER_NODE / 2; o > 0; o >>= 1) {
-                ux += __shfl_xor_sync(half, ux, o);
-                uy += __shfl_xor_sync(half, uy, o);
-                uz += __shfl_xor_sync(half, uz, o);
-            }
-            if (sub == 0) {
-                const int m = c0 + r;
-                U[m] = make_float4(ux, uy, uz, 0.f);
-                const double xn = X[m] + (double)ux, yn = Y[m] + (double)uy, zn = Z[m] + (double)uz;
-                X[m] = xn; Y[m] = yn; Z[m] = zn;
-                // halfway bounce-back walls lie at -1/2 and n - 1/2, on-site velocity walls at 0 and n - 1
-                const double m0 = p.wall[0] == PLB_WALL_HH ? 0.0 : 0.5, m1 = p.wall[1] == PLB_WALL_HH ? 0.0 : 0.5,
-                             m2 = p.wall[2] == PLB_WALL_HH ? 0.0 : 0.5;
-                const bool left = (p.wall[0] && (xn < -m0 || xn > (double)(p.nx - 1) + m0)) ||
-                                  (p.wall[1] && (yn < -m1 || yn > (double)(p.ny - 1) + m1)) ||
-                                  (p.wall[2] && (zn < -m2 || zn > (double)(p.nz - 1) + m2));
-                if (left) atomicOr(counters + 1, STATUS_NODE_LEFT);
-            }
+        for (int o = NODE_LANES / 2; o > 0; o >>= 1) {
+            ux += __shfl_xor_sync(0xffffffffu, ux, o);
+            uy += __shfl_xor_sync(0xffffffffu, uy, o);
+            uz += __shfl_xor_sync(0xffffffffu, uz, o);
+        }
+        // all reads of this sweep's positions are done before any lane of the warp writes (the
+        // shuffles above are warp-synchronous and every lane's loads feed them)
+        if (valid && sub == 0) {
+            U[m] = make_float4(ux, uy, uz, 0.f);
+            const double xn = X[m] + (double)ux, yn = Y[m] + (double)uy, zn = Z[m] + (double)uz;
+            X[m] = xn; Y[m] = yn; Z[m] = zn;
+            // halfway bounce-back walls lie at -1/2 and n - 1/2, on-site velocity walls at 0 and n - 1
+            const double m0 = p.wall[0] == PLB_WALL_HH ? 0.0 : 0.5, m1 = p.wall[1] == PLB_WALL_HH ? 0.0 : 0.5,
+                         m2 = p.wall[2] == PLB_WALL_HH ? 0.0 : 0.5;
+            const bool left = (p.wall[0] && (xn < -m0 || xn > (double)(p.nx - 1) + m0)) ||
+                              (p.wall[1] && (yn < -m1 || yn > (double)(p.ny - 1) + m1)) ||
+                              (p.wall[2] && (zn < -m2 || zn > (double)(p.nz - 1) + m2));
+            if (left) atomicOr(counters + 1, STATUS_NODE_LEFT);
         }
     }
 }
@@ -574,21 +608,26 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
     return cuda_check(cudaGetLastError(), "membrane force kernels");
 }
 
+// counters[2 + parity] = number of segments listed by the spread of that parity
 int launch_clear_spread(Ctx* c, float4* g) {
-    clear_spread_kernel<<<(unsigned)((c->n_segs + 255) / 256), 256, 0, c->stream>>>(g, c->seg_mask, (int)c->n_segs,
-                                                                                  c->prm.cells);
+    const int done = c->list_parity, next = done ^ 1;
+    const long want = (c->n_segs + 31) / 32;
+    const unsigned grid = (unsigned)(want < (long)c->sm_count * 8 ? (want > 0 ? want : 1) : (long)c->sm_count * 8);
+    clear_spread_kernel<<<grid, 256, 0, c->stream>>>(g, c->seg_mask, c->seg_list, c->counters + 2 + done,
+                                                     c->counters + 2 + next, c->prm.cells);
+    c->list_parity = next;
     c->launches++;
     return cuda_check(cudaGetLastError(), "clear_spread_kernel");
 }
 
-static size_t spread_smem(int cap) { return (size_t)cap * 12 + (size_t)IB_CHUNK * 48; }
-static size_t interp_smem(int cap) { return (size_t)cap * 12 + (size_t)IB_CHUNK * 36 + (((size_t)cap * 2 + 15) & ~(size_t)15); }
+static size_t spread_smem(int cap) { return (size_t)cap * 12; }
+static size_t interp_smem(int cap) { return (size_t)cap * 16 + (((size_t)cap * 2 + 15) & ~(size_t)15); }
 
 // Largest tile (in cells) both kernels can hold with at least one block per SM; a tile cell index
 // must also fit the 16-bit entries of the interpolation's compact list.
 int ib_max_tile_cap() {
     const size_t budget = 200 * 1024;
-    const size_t cap = (budget - (size_t)IB_CHUNK * 48 - 64) / 14;
+    const size_t cap = (budget - 64) / 18;
     return (int)(cap < 65535 ? cap : 65535);
 }
 
@@ -599,7 +638,8 @@ int launch_spread(Ctx* c, float4* g) {
                         "cudaFuncSetAttribute(spread_mesh_kernel)");
     if (rc) return rc;
     spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->prm, c->tile_cap);
+        c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, c->counters + 2 + c->list_parity, c->prm,
+        c->tile_cap);
     c->launches++;
     return cuda_check(cudaGetLastError(), "spread_mesh_kernel");
 }

@@ -118,6 +118,16 @@ __device__ __forceinline__ void pull19(const float* __restrict__ src, const LbmP
     if (hz) hecht_harting_close<2, V, COL>(h, hz, p.uw[2][hz < 0]);
 }
 
+// The same pull for a cell whose 18 neighbours all lie inside the grid (no wrap, no wall): the
+// source offsets are compile-time multiples of the strides.
+template <int V, int COL>
+__device__ __forceinline__ void pull19_interior(const float* __restrict__ src, const size_t N, const int idx,
+                                                const int sy, const int sz, float (&h)[Q][V]) {
+#pragma unroll
+    for (int d = 0; d < Q; ++d)
+        h[d][COL] = __ldg(src + (size_t)d * N + (idx - CX(d) - CY(d) * sy - CZ(d) * sz));
+}
+
 // delta rho = sum h_d, j = sum c_d h_d (Eq. 17-18; sum_d w_d c_d = 0 so the shift drops out of j)
 template <int V, int COL>
 __device__ __forceinline__ void moments(const float (&h)[Q][V], float& drho, float& jx, float& jy, float& jz) {
@@ -142,6 +152,19 @@ __device__ __forceinline__ float4 cell_macros(const float* __restrict__ src, con
     const int idx = c.i + p.nx * (c.j + p.ny * c.k);
     float h[Q][1];
     pull19<1, 0>(src, p, c, idx, h);
+    float drho, jx, jy, jz;
+    moments<1, 0>(h, drho, jx, jy, jz);
+    float4 g4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (g) g4 = __ldg(g + idx);
+    const float rho = 1.0f + drho, inv = 1.0f / rho;
+    return make_float4((jx + 0.5f * g4.x) * inv, (jy + 0.5f * g4.y) * inv, (jz + 0.5f * g4.z) * inv, rho);
+}
+
+// the same for an interior cell (see pull19_interior)
+__device__ __forceinline__ float4 cell_macros_interior(const float* __restrict__ src, const float4* __restrict__ g,
+                                                       const LbmParams& p, const int idx) {
+    float h[Q][1];
+    pull19_interior<1, 0>(src, (size_t)p.cells, idx, p.nx, p.nx * p.ny, h);
     float drho, jx, jy, jz;
     moments<1, 0>(h, drho, jx, jy, jz);
     float4 g4 = make_float4(0.f, 0.f, 0.f, 0.f);

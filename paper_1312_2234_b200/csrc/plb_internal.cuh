@@ -102,7 +102,9 @@ struct Ctx {
     float* f[2];
     int cur;
     unsigned* seg_mask;        // one bit per segment, (n_segs + 31) / 32 words
-    int* counters;             // [1] status bits
+    int* counters;             // [1] status bits, [2], [3] lengths of the segment list (alternating)
+    int* seg_list;             // segments the last spread marked (n_segs entries)
+    int list_parity;           // which counter the next spread appends to
     // meshes
     long cap_nodes, cap_edges, n_nodes, n_edges;
     double* X[3];              // SoA fp64 unwrapped positions
