@@ -166,6 +166,7 @@ class Workload:
     k_volume: float = 0.0             # k_v of Eq. 5
     force_sigma: float = 0.0          # per-step Philox normal force noise (C5)
     force_seed: int = 0
+    shear_rate: float = 0.0           # du_x/dy of the initial flow (flipping workload)
     u_ref: float = 1.0                # velocity scale for the |du| <= 1e-4 u_ref tolerance (u_wall, or u0 for C2)
     notes: list = field(default_factory=list)
 
@@ -316,6 +317,62 @@ def with_area_volume_constraints(w: Workload, ratio=4.4) -> Workload:
     v.name = w.name + "-constrained"
     v.notes = list(w.notes) + ["area / volume constraints on (PAPER.md Eq. 4-5): k_s = k_t = k_v = %.3g" % v.k_volume]
     return v
+
+
+def rot_z(theta: float) -> np.ndarray:
+    c, s = math.cos(theta), math.sin(theta)
+    return np.array([[c, -s, 0], [s, c, 0], [0, 0, 1]], dtype=np.float64)
+
+
+def flipping_platelet(nx=64, ny=200, nz=64, a=5.0, lam=0.25, height=None, u_wall=0.1, tau=1.379, k_spring=0.1,
+                      subdiv=3, theta0=0.0, steps=1000, constraints=4.4):
+    """SURVEY.md NEXT-3, the paper's validation case (section 4.1, Fig. 5-6): ONE
+    stiff platelet, oblate spheroid of major radius `a` cells and aspect ratio `lam` (L81), tau =
+    1.379 (L215), flipping in a linear shear flow.
+      height=None : far from any wall ("H/a > 20", the Jeffery-orbit case): the two walls move in
+                    opposite directions (-u_wall, +u_wall) so the centre, at mid-height, does not
+                    drift; shear rate 2 u_wall/ny.
+      height=H    : near-wall case (the paper's H = 2.4 a): bottom wall at rest, top wall at u_wall,
+                    centre H above the bottom WALL (which lies at y = -1/2); shear rate u_wall/ny.
+    The symmetry axis of the disc starts in the shear plane (x-y), `theta0` away from the gradient
+    direction y towards the flow direction x.  The membrane is the hot path's springs plus the
+    area / volume constraints of NEXT-2 (`constraints` = k_s/k, 0 = off); no seed: nothing is random."""
+    kind = (PERIODIC, WALL, PERIODIC)
+    u_lo = np.zeros((3, 3)); u_hi = np.zeros((3, 3))
+    j = np.arange(ny, dtype=np.float64)
+    if height is None:
+        u_lo[1, 0], u_hi[1, 0] = -u_wall, u_wall
+        prof = u_wall * (2.0 * (j + 0.5) / ny - 1.0)
+        centre = (nx / 2.0, (ny - 1) / 2.0, nz / 2.0)
+        shear = 2.0 * u_wall / ny
+        name = "flip-far"
+    else:
+        u_hi[1, 0] = u_wall
+        prof = u_wall * (j + 0.5) / ny
+        centre = (nx / 2.0, height - 0.5, nz / 2.0)
+        shear = u_wall / ny
+        name = "flip-wall"
+    u = np.zeros((3, nz, ny, nx), dtype=np.float64)
+    u[0] = prof[None, :, None]
+    # body z (the short axis) -> world y, then tilt by theta0 about world z towards +x
+    R = rot_z(-theta0) @ rot_x(-0.5 * math.pi)
+    ms = ellipsoid_meshes(subdiv, (a, a, lam * a), R[None], [centre])
+    w = Workload(name=name, nx=nx, ny=ny, nz=nz, tau=tau, kind=kind, u_lo=u_lo, u_hi=u_hi, steps=steps,
+                 u0=u.reshape(3, -1), k_spring=k_spring, u_ref=u_wall,
+                 notes=["one platelet a=%g lambda=%g, shear rate %.4g per step, Jeffery period %.0f steps"
+                        % (a, lam, shear, 2 * math.pi * (lam + 1.0 / lam) / shear)], shear_rate=shear,
+                 **ms.fields())
+    if constraints:
+        w = with_area_volume_constraints(w, ratio=constraints)
+    return w
+
+
+def disc_axis(xyz: np.ndarray) -> np.ndarray:
+    """Unit symmetry axis of a disc-like node cloud [n,3]: the eigenvector of the smallest
+    eigenvalue of the gyration tensor (measurement helper for the flipping workload)."""
+    d = xyz - xyz.mean(axis=0)
+    w, v = np.linalg.eigh(d.T @ d)
+    return v[:, 0]
 
 
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
