@@ -67,6 +67,12 @@ struct orc_ctx {
     real *tri_S0;                      /* unstressed triangle area S_0 */
     real *S0_tot, *V0, *k_s, *k_t, *k_v;   /* per mesh (k = 0 and no triangles until orc_set_triangles) */
     int forces_valid;
+    /* NEXT-4 (section 3.2, 3.4.1): receptors, bonds to the vWF sites of one wall, wall repulsion */
+    int n_rec;
+    int *rec_node;                     /* global node each receptor sits on */
+    int *bond;                         /* per receptor: (bound 0/1, site s0, site s1), sites unwrapped */
+    int *site_count;                   /* bonds per vWF site, n[t0] * n[t1] */
+    orc_adhesion adh;
 };
 
 void orc_lattice(int* c_out, double* w_out) {
@@ -172,6 +178,7 @@ int orc_destroy(orc_ctx* c) {
     free(c->X); free(c->F); free(c->U); free(c->edge); free(c->rest); free(c->kspring);
     free(c->mesh_off); free(c->tri); free(c->tri_mesh); free(c->tri_S0);
     free(c->S0_tot); free(c->V0); free(c->k_s); free(c->k_t); free(c->k_v);
+    free(c->rec_node); free(c->bond); free(c->site_count);
     free(c);
     return 0;
 }
@@ -558,6 +565,8 @@ static void area_volume_forces(orc_ctx* c) {
     free(alpha); free(beta);
 }
 
+static int adhesion_forces(orc_ctx* c);   /* NEXT-4, below */
+
 /* O-5: F <- 0; for each edge (a,b): R = X_b - X_a, l = |R|, e = k (l - L) R / l; F_a += e,
  * F_b -= e.  Eq. 2-3 (L92-99) with the sign read per G1: the force on point i is -grad_{X_i} of
  * Eq. 2, i.e. +k(|R|-L)R/|R| with R = X_j - X_i (attracting when stretched).  If sigma > 0,
@@ -581,6 +590,8 @@ int orc_compute_membrane_forces(orc_ctx* c, double sigma, uint64_t seed, uint64_
         }
     }
     area_volume_forces(c);
+    int rc = adhesion_forces(c);
+    if (rc) return rc;
     if (sigma > 0)
         for (int m = 0; m < c->n_nodes; ++m) {
             double z[3];
@@ -743,4 +754,185 @@ int orc_read_node_velocities(orc_ctx* c, double* U) {
     if (!c || !U) return -1;
     for (int m = 0; m < 3 * c->n_nodes; ++m) U[m] = (double)c->U[m];
     return 0;
+}
+
+/* =============================================================================================
+ * NEXT-4: stochastic dynamic adhesion model (section 3.2) + wall repulsion (section 3.4.1).
+ * Decision arithmetic (probabilities, capture distance) is fp64 in BOTH builds and on the GPU:
+ * a Monte-Carlo decision is an integer outcome, so both sides take it in the same precision.
+ * ============================================================================================= */
+static void tangential_axes(int a, int* t0, int* t1) {
+    *t0 = a == 0 ? 1 : 0;
+    *t1 = a == 2 ? 1 : 2;
+}
+static double wall_plane(const orc_ctx* c, int a) { return c->kind[a] == ORC_WALL_HH ? 0.0 : -0.5; }
+
+int orc_set_receptors(orc_ctx* c, int n_rec, const int* node, const orc_adhesion* prm) {
+    if (!c || n_rec < 0 || (n_rec && !node) || !prm) return -1;
+    const int a = prm->wall_axis;
+    if (a < 0 || a > 2 || c->kind[a] == ORC_PERIODIC || prm->max_per_site < 1) return -1;
+    if (!(prm->l_max > 0) || prm->k_on0 < 0 || prm->k_off0 < 0) return -1;
+    for (int r = 0; r < n_rec; ++r)
+        if (node[r] < 0 || node[r] >= c->n_nodes) return -1;
+    int t0, t1;
+    tangential_axes(a, &t0, &t1);
+    free(c->rec_node); free(c->bond); free(c->site_count);
+    c->n_rec = n_rec;
+    c->rec_node = (int*)malloc(sizeof(int) * (size_t)(n_rec > 0 ? n_rec : 1));
+    c->bond = (int*)calloc((size_t)3 * (size_t)(n_rec > 0 ? n_rec : 1), sizeof(int));
+    c->site_count = (int*)calloc((size_t)c->n[t0] * (size_t)c->n[t1], sizeof(int));
+    for (int r = 0; r < n_rec; ++r) c->rec_node[r] = node[r];
+    c->adh = *prm;
+    c->forces_valid = 0;
+    return 0;
+}
+
+/* linear index of site (s0, s1) for the per-site bond count, -1 if the site does not exist
+ * (outside a non-periodic tangential axis) */
+static long site_index(const orc_ctx* c, int t0, int t1, long s0, long s1) {
+    long s[2] = {s0, s1};
+    const int t[2] = {t0, t1};
+    for (int e = 0; e < 2; ++e) {
+        const long n = c->n[t[e]];
+        if (c->kind[t[e]] == ORC_PERIODIC) {
+            s[e] %= n;
+            if (s[e] < 0) s[e] += n;
+        } else if (s[e] < 0 || s[e] >= n) {
+            return -1;
+        }
+    }
+    return s[0] + (long)c->n[t0] * s[1];
+}
+
+/* distance between the receptor at X and the site (s0, s1) on the wall plane */
+static double bond_length(const orc_ctx* c, const real* X, int a, int t0, int t1, long s0, long s1, double R[3]) {
+    R[a] = wall_plane(c, a) - (double)X[a];
+    R[t0] = (double)s0 - (double)X[t0];
+    R[t1] = (double)s1 - (double)X[t1];
+    return sqrt(R[0] * R[0] + R[1] * R[1] + R[2] * R[2]);
+}
+
+void orc_adhesion_probabilities(const orc_adhesion* p, double x_b, double* P_f, double* P_r) {
+    const double d = fabs(x_b - p->l_b);
+    const double k_on = p->k_on0 * exp(p->s * d * (p->gamma - 0.5 * d));   /* Eq. 13 */
+    const double k_off = p->k_off0 * exp(p->gamma * p->s * d);             /* Eq. 12, F_b = sigma d */
+    if (P_f) *P_f = 1.0 - exp(-k_on);                                      /* L151, dt = 1 */
+    if (P_r) *P_r = 1.0 - exp(-k_off);
+}
+
+int orc_adhesion_update(orc_ctx* c, uint64_t seed, uint64_t step) {
+    if (!c || !c->rec_node) return -4;
+    const orc_adhesion* p = &c->adh;
+    const int a = p->wall_axis;
+    int t0, t1;
+    tangential_axes(a, &t0, &t1);
+    /* 1) break the already formed bonds (L276) */
+    for (int r = 0; r < c->n_rec; ++r) {
+        int* b = c->bond + 3 * r;
+        if (!b[0]) continue;
+        double R[3], xi[4], P_r;
+        const double x_b = bond_length(c, c->X + 3 * c->rec_node[r], a, t0, t1, b[1], b[2], R);
+        orc_adhesion_probabilities(p, x_b, NULL, &P_r);
+        orc_noise_uniform(seed, (uint64_t)r, (uint32_t)step, 3u, xi);
+        if (xi[0] < P_r) {
+            b[0] = 0;
+            c->site_count[site_index(c, t0, t1, b[1], b[2])] -= 1;
+        }
+    }
+    /* 2) generate new bonds from unbound receptors and sites with a free place (L147-149, L276):
+     * receptor order = index order, so the lowest indices take the free places of a site */
+    for (int r = 0; r < c->n_rec; ++r) {
+        int* b = c->bond + 3 * r;
+        if (b[0]) continue;                                          /* rule 1: one vWF per receptor */
+        const real* X = c->X + 3 * c->rec_node[r];
+        const long s0 = (long)floor((double)X[t0] + 0.5), s1 = (long)floor((double)X[t1] + 0.5);   /* nearest site */
+        const long si = site_index(c, t0, t1, s0, s1);
+        if (si < 0) continue;
+        double R[3], xi[4], P_f;
+        const double x_b = bond_length(c, X, a, t0, t1, s0, s1, R);
+        if (!(x_b < p->l_max)) continue;                             /* L149: closer than the bond length */
+        if (c->site_count[si] >= p->max_per_site) continue;          /* rule 2: at most 4 receptors per vWF */
+        orc_adhesion_probabilities(p, x_b, &P_f, NULL);
+        orc_noise_uniform(seed, (uint64_t)r, (uint32_t)step, 3u, xi);
+        if (xi[1] < P_f) {
+            b[0] = 1; b[1] = (int)s0; b[2] = (int)s1;
+            c->site_count[si] += 1;
+        }
+    }
+    c->forces_valid = 0;
+    return 0;
+}
+
+int orc_read_bonds(orc_ctx* c, int* bonds) {
+    if (!c || !bonds) return -1;
+    for (int i = 0; i < 3 * c->n_rec; ++i) bonds[i] = c->bond[i];
+    return 0;
+}
+
+int orc_write_bonds(orc_ctx* c, const int* bonds) {
+    if (!c || !bonds || !c->rec_node) return -1;
+    int t0, t1;
+    tangential_axes(c->adh.wall_axis, &t0, &t1);
+    const long n_sites = (long)c->n[t0] * c->n[t1];
+    for (long i = 0; i < n_sites; ++i) c->site_count[i] = 0;
+    for (int r = 0; r < c->n_rec; ++r) {
+        int* b = c->bond + 3 * r;
+        b[0] = bonds[3 * r] ? 1 : 0; b[1] = b[0] ? bonds[3 * r + 1] : 0; b[2] = b[0] ? bonds[3 * r + 2] : 0;
+        if (b[0]) {
+            const long si = site_index(c, t0, t1, b[1], b[2]);
+            if (si < 0) return -1;
+            c->site_count[si] += 1;
+        }
+    }
+    c->forces_valid = 0;
+    return 0;
+}
+
+/* Eq. 14 read as the restoring spring force of the bond on its node (magnitude sigma |x_b - l_b|,
+ * towards the site when stretched), plus F_rep of L246 on every node along the inward normal. */
+static int adhesion_forces(orc_ctx* c) {
+    if (!c->rec_node) return 0;
+    const orc_adhesion* p = &c->adh;
+    const int a = p->wall_axis;
+    int t0, t1;
+    tangential_axes(a, &t0, &t1);
+    for (int r = 0; r < c->n_rec; ++r) {
+        const int* b = c->bond + 3 * r;
+        if (!b[0]) continue;
+        const int m = c->rec_node[r];
+        double R[3];
+        const double x_b = bond_length(c, c->X + 3 * m, a, t0, t1, b[1], b[2], R);
+        if (!(x_b > 0)) continue;
+        for (int d = 0; d < 3; ++d) c->F[3 * m + d] += (real)(p->sigma * (x_b - p->l_b) * R[d] / x_b);
+    }
+    if (p->F0 > 0)
+        for (int m = 0; m < c->n_nodes; ++m) {
+            const double eps = (double)c->X[3 * m + a] - wall_plane(c, a);
+            if (!(eps > 0)) return -5;
+            const double e = exp(-p->tau_rep * eps);
+            c->F[3 * m + a] += (real)(p->F0 * p->tau_rep * e / (1.0 - e));
+        }
+    return 0;
+}
+
+double orc_adhesion_energy(orc_ctx* c) {
+    if (!c || !c->rec_node) return 0.0;
+    const orc_adhesion* p = &c->adh;
+    const int a = p->wall_axis;
+    int t0, t1;
+    tangential_axes(a, &t0, &t1);
+    double H = 0;
+    for (int r = 0; r < c->n_rec; ++r) {
+        const int* b = c->bond + 3 * r;
+        if (!b[0]) continue;
+        double R[3];
+        const double x_b = bond_length(c, c->X + 3 * c->rec_node[r], a, t0, t1, b[1], b[2], R);
+        H += 0.5 * p->sigma * (x_b - p->l_b) * (x_b - p->l_b);
+    }
+    if (p->F0 > 0)
+        for (int m = 0; m < c->n_nodes; ++m) {
+            const double eps = (double)c->X[3 * m + a] - wall_plane(c, a);
+            H -= p->F0 * log(1.0 - exp(-p->tau_rep * eps));
+        }
+    return H;
 }

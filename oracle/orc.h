@@ -79,6 +79,43 @@ double orc_spring_energy(orc_ctx*);
  * no advance (used for the adjointness pin) */
 int orc_interpolate_field(orc_ctx*, const double* w, double* U /*AoS*/);
 
+/* ---- NEXT-4: stochastic dynamic adhesion model (section 3.2, Eq. 12-14, rules L147-149)
+ * and short-range wall repulsion (section 3.4.1).  DESIGN.md readings A-1 .. A-9.
+ * All quantities in lattice units (h = dt = 1); rates are per time step.
+ *   receptors : receptor r sits on global node node[r] ("located at ith node", Eq. 14)
+ *   vWF sites : on the LOW face of wall axis `wall_axis`, one per lattice point of that plane
+ *               (25 per um^2 = one per h^2 at h = 0.2 um, L145/L173); the plane lies at -1/2
+ *               (ORC_WALL) or 0 (ORC_WALL_HH); a site is named by its two tangential integer
+ *               coordinates (s0, s1), the tangential axes in x, y, z order, kept unwrapped
+ *   k_on  = k_on0  exp( s d (gamma - d/2) ),  d = |x_b - l_b|,  s = sigma/(k_B T)     (Eq. 13)
+ *   k_off = k_off0 exp( gamma s d )             (Eq. 12 with F_b = sigma d)
+ *   P_f = 1 - exp(-k_on), P_r = 1 - exp(-k_off) (L151)
+ *   bond force on the node: sigma (x_b - l_b) (S - X)/x_b                         (Eq. 14)
+ *   repulsion on every node: F0 tau exp(-tau eps)/(1 - exp(-tau eps)) along the inward wall normal,
+ *               eps = distance of the node from the wall plane                    (L246)     */
+typedef struct {
+    int    wall_axis;
+    int    max_per_site;       /* rule 2 (L148): 4 */
+    double k_on0, k_off0;
+    double s;                  /* sigma / k_B T */
+    double gamma;              /* reactive compliance (a length) */
+    double sigma;              /* bond spring constant */
+    double l_b, l_max;         /* equilibrium bond length; capture distance (128 nm, L149) */
+    double F0, tau_rep;        /* repulsion (0 = off) */
+} orc_adhesion;
+int orc_set_receptors(orc_ctx*, int n_receptors, const int* node, const orc_adhesion* prm);
+/* one Monte-Carlo update at the current node positions: first every existing bond is tested for
+ * breakage, then every unbound receptor for formation (order of L276); random numbers from
+ * Philox keyed on (seed; receptor, step, tag 3): word 0 breaks, word 1 forms. */
+int orc_adhesion_update(orc_ctx*, uint64_t seed, uint64_t step);
+int orc_read_bonds(orc_ctx*, int* bonds /*3 per receptor: bound, s0, s1*/);
+int orc_write_bonds(orc_ctx*, const int* bonds);
+/* sum over bonds sigma/2 (x_b - l_b)^2  -  F0 sum over nodes ln(1 - exp(-tau eps)): the potential
+ * whose negative gradient the adhesion + repulsion forces are (for the finite-difference pin) */
+double orc_adhesion_energy(orc_ctx*);
+/* P_f and P_r at bond length x_b (the closed forms above) */
+void orc_adhesion_probabilities(const orc_adhesion* prm, double x_b, double* P_f, double* P_r);
+
 #ifdef __cplusplus
 }
 #endif

@@ -13,6 +13,27 @@ from . import build as _build
 _libs = {}
 
 
+class Adhesion(C.Structure):
+    """orc_adhesion of orc.h (NEXT-4: PAPER.md section 3.2 / 3.4.1), lattice units, rates per step"""
+    _fields_ = [("wall_axis", C.c_int), ("max_per_site", C.c_int), ("k_on0", C.c_double), ("k_off0", C.c_double),
+                ("s", C.c_double), ("gamma", C.c_double), ("sigma", C.c_double), ("l_b", C.c_double),
+                ("l_max", C.c_double), ("F0", C.c_double), ("tau_rep", C.c_double)]
+
+    @classmethod
+    def from_dict(cls, d):
+        return cls(int(d.get("wall_axis", 1)), int(d.get("max_per_site", 4)), float(d["k_on0"]), float(d["k_off0"]),
+                   float(d["s"]), float(d["gamma"]), float(d["sigma"]), float(d["l_b"]), float(d["l_max"]),
+                   float(d.get("F0", 0.0)), float(d.get("tau_rep", 0.0)))
+
+
+def adhesion_probabilities(prm: dict, x_b: float):
+    """(P_f, P_r) of Eq. 12-13 / L151 at bond length x_b"""
+    a = Adhesion.from_dict(prm)
+    pf, pr = C.c_double(), C.c_double()
+    lib().orc_adhesion_probabilities(C.byref(a), float(x_b), C.byref(pf), C.byref(pr))
+    return pf.value, pr.value
+
+
 def lib(fp32: bool = False):
     if fp32 not in _libs:
         _build.build()
@@ -52,6 +73,12 @@ def lib(fp32: bool = False):
             "orc_read_node_velocities": (C.c_int, [vp, dp]),
             "orc_spring_energy": (C.c_double, [vp]),
             "orc_interpolate_field": (C.c_int, [vp, dp, dp]),
+            "orc_set_receptors": (C.c_int, [vp, C.c_int, ip, C.POINTER(Adhesion)]),
+            "orc_adhesion_update": (C.c_int, [vp, u64, u64]),
+            "orc_read_bonds": (C.c_int, [vp, ip]),
+            "orc_write_bonds": (C.c_int, [vp, ip]),
+            "orc_adhesion_energy": (C.c_double, [vp]),
+            "orc_adhesion_probabilities": (None, [C.POINTER(Adhesion), C.c_double, dp, dp]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -136,6 +163,9 @@ class Oracle:
             o.add_mesh(w.mesh_xyz[m], w.edges, w.rest, w.k_spring)
             if w.k_area_global or w.k_area_local or w.k_volume:
                 o.set_triangles(m, w.tris, w.ref_xyz, w.k_area_global, w.k_area_local, w.k_volume)
+        if getattr(w, "receptor_node", None) is not None:
+            o.set_receptors(w.receptor_node, w.adhesion)
+            o.adhesion_seed = w.adhesion_seed
         return o
 
     def _chk(self, rc, what):
@@ -253,6 +283,30 @@ class Oracle:
     def spring_energy(self):
         return self.L.orc_spring_energy(self.h)
 
+    # ---- NEXT-4: adhesion (section 3.2) and wall repulsion (section 3.4.1)
+    def set_receptors(self, node, prm: dict):
+        node = np.ascontiguousarray(node, dtype=np.int32)
+        self.n_rec = node.shape[0]
+        self.adhesion_seed = getattr(self, "adhesion_seed", 0)
+        a = Adhesion.from_dict(prm)
+        self._chk(self.L.orc_set_receptors(self.h, node.shape[0], _ip(node), C.byref(a)), "orc_set_receptors")
+
+    def adhesion_update(self, seed=0, step=0):
+        self._chk(self.L.orc_adhesion_update(self.h, int(seed), int(step)), "orc_adhesion_update")
+
+    def read_bonds(self):
+        b = np.empty((self.n_rec, 3), dtype=np.int32)
+        self._chk(self.L.orc_read_bonds(self.h, _ip(b)), "orc_read_bonds")
+        return b
+
+    def write_bonds(self, bonds):
+        b = np.ascontiguousarray(bonds, dtype=np.int32)
+        assert b.shape == (self.n_rec, 3)
+        self._chk(self.L.orc_write_bonds(self.h, _ip(b)), "orc_write_bonds")
+
+    def adhesion_energy(self):
+        return self.L.orc_adhesion_energy(self.h)
+
     def coupled_step(self, sigma=0.0, seed=0, step=0):
         """forces -> spread -> LBM step -> interpolate + advance (Fig. 1)."""
         if self.n_nodes:
@@ -260,5 +314,7 @@ class Oracle:
             g = self.spread()
             self.step(g)
             self.interpolate_advance()
+            if getattr(self, "n_rec", 0):          # L276: "Finally, the MC computations are performed"
+                self.adhesion_update(self.adhesion_seed, step)
         else:
             self.step(None)

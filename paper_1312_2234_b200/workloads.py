@@ -166,6 +166,9 @@ class Workload:
     k_volume: float = 0.0             # k_v of Eq. 5
     force_sigma: float = 0.0          # per-step Philox normal force noise (C5)
     force_seed: int = 0
+    receptor_node: np.ndarray | None = None   # [n_receptors] i32 global node of each receptor (NEXT-4)
+    adhesion: dict | None = None      # DAM + wall-repulsion parameters (include/plb.h plb_adhesion), lattice units
+    adhesion_seed: int = 0
     shear_rate: float = 0.0           # du_x/dy of the initial flow (flipping workload)
     u_ref: float = 1.0                # velocity scale for the |du| <= 1e-4 u_ref tolerance (u_wall, or u0 for C2)
     notes: list = field(default_factory=list)
@@ -365,6 +368,38 @@ def flipping_platelet(nx=64, ny=200, nz=64, a=5.0, lam=0.25, height=None, u_wall
     if constraints:
         w = with_area_volume_constraints(w, ratio=constraints)
     return w
+
+
+def adhering_platelets(nx=48, ny=32, nz=48, n_side=1, a=5.0, lam=0.25, gap=0.25, u_wall=0.04, tau=1.0, k_spring=0.05,
+                       subdiv=3, receptors_per_platelet=5344, steps=200, seed=SEED_BASE + 14, adhesion=None):
+    """SURVEY.md NEXT-4 workload: n_side x n_side platelets lying flat just above the resting bottom
+    wall (lowest point `gap` above the wall plane y = -1/2) under a shear flow, each carrying
+    `receptors_per_platelet` receptor points (5344 per platelet) assigned to uniformly
+    drawn nodes of its mesh.  vWF sites are the lattice points of the wall plane (one per h^2 =
+    25 per um^2 at h = 0.2 um, L145/L173).  The DAM parameters sigma, gamma, l_b are not in Table 2;
+    the defaults below are synthetic values in lattice units chosen so that bonds form, stretch and
+    break within a few hundred steps (capture distance 128 nm = 0.64 h is the paper's, L149)."""
+    rng = np.random.default_rng(np.random.PCG64(seed))
+    kind, u_lo, u_hi = _walls_y(u_wall)
+    c = lam * a
+    px, pz = nx / n_side, nz / n_side
+    p, r = np.meshgrid(np.arange(n_side), np.arange(n_side), indexing="ij")
+    centres = np.stack([px * (p.ravel() + 0.5), np.full(p.size, -0.5 + gap + c), pz * (r.ravel() + 0.5)], axis=1)
+    centres[:, [0, 2]] += rng.random((p.size, 2)) - 0.5
+    R = np.repeat(rot_x(-0.5 * math.pi)[None], p.size, axis=0)          # body z (short axis) -> world y
+    ms = ellipsoid_meshes(subdiv, (a, a, c), R, centres)
+    n_nodes = ms.xyz.shape[1]
+    rec = (rng.integers(0, n_nodes, size=(p.size, receptors_per_platelet)) + n_nodes * np.arange(p.size)[:, None])
+    prm = dict(wall_axis=1, max_per_site=4, k_on0=0.1, k_off0=0.002, s=4.0, gamma=0.2, sigma=0.05, l_b=0.3,
+               l_max=0.64, F0=2e-5, tau_rep=4.0)
+    if adhesion:
+        prm.update(adhesion)
+    w = Workload(name="adhesion", nx=nx, ny=ny, nz=nz, tau=tau, kind=kind, u_lo=u_lo, u_hi=u_hi, steps=steps,
+                 u0=shear_field(nx, ny, nz, u_wall), k_spring=k_spring, u_ref=u_wall,
+                 receptor_node=np.ascontiguousarray(rec.ravel(), dtype=np.int32), adhesion=prm, adhesion_seed=seed,
+                 notes=["%d platelets flat on the bottom wall, %d receptors each; DAM parameters synthetic (not in Table 2)"
+                        % (p.size, receptors_per_platelet)], **ms.fields())
+    return with_area_volume_constraints(w)
 
 
 def disc_axis(xyz: np.ndarray) -> np.ndarray:
