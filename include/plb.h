@@ -146,6 +146,54 @@ PLB_API int ib_spread(plb_ctx* ctx, float* d_forcing);
  * ib_read_nodes report as PLB_ERR_NODE_LEFT. */
 PLB_API int ib_interpolate_advance(plb_ctx* ctx);
 
+/* ---- stochastic dynamic adhesion model (section 3.2, Eq. 12-14, rules
+ * L147-149, P_f / P_r L151) and short-range wall repulsion (section 3.4.1); the step
+ * after S5 in the paper's loop (L276).  Readings A-1 .. A-9 in DESIGN.md.  Lattice units, rates
+ * per time step.
+ *   receptors : receptor r sits on global node h_node[r] (Eq. 14: "bond located at ith node");
+ *   vWF sites : on the LOW face of wall axis `wall_axis` (the paper's "bottom plane"), one per
+ *               lattice point of that plane (25 per um^2 = one per h^2 at h = 0.2 um, L145, L173).
+ *               The plane lies at -1/2 (PLB_WALL_BB) or 0 (PLB_WALL_HH).  A site is named by its two
+ *               tangential integer coordinates (s0, s1), tangential axes in x, y, z order, kept
+ *               unwrapped like the node positions;
+ *   k_on  = k_on0  exp( s d (gamma - d/2) ),  d = |x_b - l_b|,  s = sigma / k_B T        (Eq. 13)
+ *   k_off = k_off0 exp( gamma s d )            (Eq. 12, Bell, with F_b = sigma d)
+ *   P_f = 1 - exp(-k_on),  P_r = 1 - exp(-k_off)                                        (L151)
+ *   bond force on its node : sigma (x_b - l_b) (S - X)/x_b   (Eq. 14 read as the restoring force)
+ *   repulsion on every node: F0 tau exp(-tau eps)/(1 - exp(-tau eps)) along the inward normal,
+ *               eps = distance of the node from the wall plane (L246); eps <= 0 raises the
+ *               PLB_ERR_NODE_LEFT flag.                                                         */
+typedef struct {
+    int   wall_axis;      /* 0, 1, 2: must be a wall axis of the context */
+    int   max_per_site;   /* rule 2 (L148): 4; at most 32 */
+    float k_on0, k_off0;
+    float s;              /* sigma / k_B T */
+    float gamma;          /* reactive compliance (a length) */
+    float sigma;          /* bond spring constant */
+    float l_b, l_max;     /* equilibrium bond length; capture distance (128 nm = 0.64 h, L149) */
+    float F0, tau_rep;    /* repulsion; F0 = 0 switches it off */
+} plb_adhesion;
+
+/* Device bytes ib_set_receptors needs for n_receptors receptors on this grid and wall axis. */
+PLB_API int ib_adhesion_workspace_bytes(const plb_grid* grid, int wall_axis, long n_receptors, size_t* out_bytes);
+/* Attach the receptors (all meshes must have been added).  d_workspace: caller-owned, 256-byte
+ * aligned, ib_adhesion_workspace_bytes() bytes, valid until lbm_destroy.  All bonds start open.
+ * From then on ib_compute_membrane_forces adds the bond and repulsion forces. */
+PLB_API int ib_set_receptors(plb_ctx* ctx, long n_receptors, const int* h_node, const plb_adhesion* prm,
+                     void* d_workspace, size_t workspace_bytes);
+/* One Monte-Carlo update at the current node positions (call it after ib_interpolate_advance):
+ * every existing bond is tested for breakage, then every unbound receptor whose nearest vWF site
+ * is closer than l_max is tested for formation (order of L276).  Uniforms from Philox keyed on
+ * (seed; receptor, step, tag 3): word 0 breaks (u < P_r), word 1 forms (u < P_f).  Probabilities
+ * are evaluated in fp64.  When more receptors pass the formation test for one site than it has
+ * free places, the lowest receptor indices take them.  More than 32 same-step candidates for one
+ * site raise a sticky error that plb_status reports as PLB_ERR_WORKSPACE. */
+PLB_API int ib_adhesion_update(plb_ctx* ctx, unsigned long long seed, unsigned long long step);
+PLB_API int ib_n_receptors(plb_ctx* ctx, long* out);
+/* h_bonds: 3 ints per receptor = (bound 0/1, s0, s1) */
+PLB_API int ib_read_bonds(plb_ctx* ctx, int* h_bonds);
+PLB_API int ib_write_bonds(plb_ctx* ctx, const int* h_bonds);   /* also rebuilds the per-site counts */
+
 /* ---- auxiliary, off the timed path (tests, checkpoints, end-to-end I/O) ---- */
 PLB_API int ib_n_nodes(plb_ctx* ctx, long* out);
 PLB_API int ib_read_nodes(plb_ctx* ctx, double* h_xyz);            /* n x 3 AoS */

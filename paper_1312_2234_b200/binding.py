@@ -42,6 +42,12 @@ SYMBOLS = {
     "ib_read_node_velocities": (_i, [_vp, _vp]),
     "lbm_read_populations": (_i, [_vp, _vp]),
     "lbm_write_populations": (_i, [_vp, _vp]),
+    "ib_adhesion_workspace_bytes": (_i, [_vp, _i, _l, C.POINTER(_sz)]),
+    "ib_set_receptors": (_i, [_vp, _l, _vp, _vp, _vp, _sz]),
+    "ib_adhesion_update": (_i, [_vp, _u64, _u64]),
+    "ib_n_receptors": (_i, [_vp, C.POINTER(_l)]),
+    "ib_read_bonds": (_i, [_vp, _vp]),
+    "ib_write_bonds": (_i, [_vp, _vp]),
     "plb_status": (_i, [_vp]),
     "plb_launch_count": (_i, [_vp, C.POINTER(_l)]),
     "plb_philox4x32_10": (_i, [_vp, _l, _vp, _vp, _vp]),
@@ -54,6 +60,18 @@ class PlbGrid(C.Structure):
 
 class PlbBoundary(C.Structure):
     _fields_ = [("kind", _i * 3), ("u_lo", (_f * 3) * 3), ("u_hi", (_f * 3) * 3)]
+
+
+class PlbAdhesion(C.Structure):
+    """plb_adhesion of include/plb.h (NEXT-4), lattice units, rates per step"""
+    _fields_ = [("wall_axis", _i), ("max_per_site", _i), ("k_on0", _f), ("k_off0", _f), ("s", _f), ("gamma", _f),
+                ("sigma", _f), ("l_b", _f), ("l_max", _f), ("F0", _f), ("tau_rep", _f)]
+
+    @classmethod
+    def from_dict(cls, d):
+        return cls(int(d.get("wall_axis", 1)), int(d.get("max_per_site", 4)), float(d["k_on0"]), float(d["k_off0"]),
+                   float(d["s"]), float(d["gamma"]), float(d["sigma"]), float(d["l_b"]), float(d["l_max"]),
+                   float(d.get("F0", 0.0)), float(d.get("tau_rep", 0.0)))
 
 
 class PlbError(RuntimeError):
@@ -224,6 +242,43 @@ def ib_read_node_velocities(h):
     return out
 
 
+def ib_adhesion_workspace_bytes(nx, ny, nz, wall_axis, n_receptors) -> int:
+    g = PlbGrid(nx, ny, nz)
+    out = _sz(0)
+    _check(lib().ib_adhesion_workspace_bytes(C.addressof(g), int(wall_axis), int(n_receptors), C.byref(out)),
+           "ib_adhesion_workspace_bytes")
+    return out.value
+
+
+def ib_set_receptors(h, node, prm: dict, workspace):
+    node = np.ascontiguousarray(node, dtype=np.int32)
+    a = PlbAdhesion.from_dict(prm)
+    _check(lib().ib_set_receptors(h, node.shape[0], _np_ptr(node), C.addressof(a), workspace.data_ptr(),
+                                  workspace.numel() * workspace.element_size()), "ib_set_receptors")
+
+
+def ib_adhesion_update(h, seed=0, step=0):
+    _check(lib().ib_adhesion_update(h, int(seed), int(step)), "ib_adhesion_update")
+
+
+def ib_n_receptors(h) -> int:
+    out = _l(0)
+    _check(lib().ib_n_receptors(h, C.byref(out)), "ib_n_receptors")
+    return out.value
+
+
+def ib_read_bonds(h):
+    out = np.empty((ib_n_receptors(h), 3), dtype=np.int32)
+    _check(lib().ib_read_bonds(h, _np_ptr(out)), "ib_read_bonds")
+    return out
+
+
+def ib_write_bonds(h, bonds):
+    b = np.ascontiguousarray(bonds, dtype=np.int32)
+    assert b.shape == (ib_n_receptors(h), 3)
+    _check(lib().ib_write_bonds(h, _np_ptr(b)), "ib_write_bonds")
+
+
 def plb_status(h):
     _check(lib().plb_status(h), "plb_status")
 
@@ -270,6 +325,9 @@ class Simulation:
             first = s.add_meshes(w.mesh_xyz, w.edges, w.rest, w.k_spring)
             if w.k_area_global or w.k_area_local or w.k_volume:
                 s.set_triangles(first, w.n_meshes, w.tris, w.ref_xyz, w.k_area_global, w.k_area_local, w.k_volume)
+        if getattr(w, "receptor_node", None) is not None:
+            s.set_receptors(w.receptor_node, w.adhesion)
+            s.adhesion_seed = w.adhesion_seed
         return s
 
     def close(self):
@@ -315,6 +373,23 @@ class Simulation:
     def compute_membrane_forces(self, sigma=0.0, seed=0, step=0):
         ib_compute_membrane_forces(self.h, sigma, seed, step)
 
+    def set_receptors(self, node, prm: dict):
+        node = np.ascontiguousarray(node, dtype=np.int32)
+        nbytes = ib_adhesion_workspace_bytes(self.nx, self.ny, self.nz, int(prm.get("wall_axis", 1)), node.shape[0])
+        self.adhesion_workspace = self.torch.empty(nbytes, dtype=self.torch.uint8, device=self.device)
+        ib_set_receptors(self.h, node, prm, self.adhesion_workspace)
+        self.n_rec = node.shape[0]
+        self.adhesion_seed = getattr(self, "adhesion_seed", 0)
+
+    def adhesion_update(self, seed=0, step=0):
+        ib_adhesion_update(self.h, seed, step)
+
+    def read_bonds(self):
+        return ib_read_bonds(self.h)
+
+    def write_bonds(self, bonds):
+        ib_write_bonds(self.h, bonds)
+
     def spread(self, d_forcing=None):
         ib_spread(self.h, self.forcing if d_forcing is None else d_forcing)
 
@@ -327,6 +402,8 @@ class Simulation:
         ib_spread(self.h, self.forcing)
         lbm_step(self.h, self.forcing)
         ib_interpolate_advance(self.h)
+        if getattr(self, "n_rec", 0):               # L276: "Finally, the MC computations are performed"
+            ib_adhesion_update(self.h, self.adhesion_seed, step)
 
     @property
     def n_nodes(self):

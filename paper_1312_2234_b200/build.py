@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libplb.so")
-SOURCES = ["api.cu", "lbm.cu", "ib.cu"]
+SOURCES = ["api.cu", "lbm.cu", "ib.cu", "adhesion.cu"]
 HEADERS = ["plb_internal.cuh", os.path.join("..", "..", "include", "plb.h")]
 
 NVCC_FLAGS = [

@@ -93,6 +93,14 @@ static int sync_status(Ctx* c) {
         set_error("a mesh edge has zero length");
         return PLB_ERR_ARG;
     }
+    if (h[1] & STATUS_ADH_OVERFLOW) {
+        set_error("more than %d same-step bond candidates for one vWF site", ADH_MAX_CAND);
+        return PLB_ERR_WORKSPACE;
+    }
+    if (h[1] & STATUS_ADH_BAD_SITE) {
+        set_error("ib_write_bonds: a bond names a site outside a non-periodic tangential axis");
+        return PLB_ERR_ARG;
+    }
     if (h[1] & STATUS_NODE_LEFT) {
         set_error("a node left the channel through a wall axis");
         return PLB_ERR_NODE_LEFT;
@@ -207,6 +215,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->launches = 0;
     c->n_ranges = 0;
     c->n_tris = 0; c->n_cons = 0;
+    c->adh_on = false; c->n_rec = 0;
     c->list_parity = 0;
     c->tile_cap = 512;
     c->sm_count = sms;
@@ -532,6 +541,151 @@ int ib_interpolate_advance(plb_ctx* ctx) {
     }
     const int rc = launch_interpolate_advance(ctx);
     ctx->spread_current = false;
+    ctx->forces_valid = false;
+    return rc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-4: adhesion.  The receptors, bonds and per-site tables live in their own caller-owned workspace.
+static size_t carve_adhesion(Ctx* c, char* base, long n_sites, long n_rec) {
+    Carve w{base, 0};
+    int* rec_node = w.take<int>((size_t)n_rec);
+    int4* bond = w.take<int4>((size_t)n_rec);
+    int* site_count = w.take<int>((size_t)n_sites);
+    int* cand_n = w.take<int>((size_t)n_sites);
+    int* cand = w.take<int>((size_t)n_sites * ADH_MAX_CAND);
+    if (c) {
+        c->rec_node = rec_node; c->bond = bond; c->site_count = site_count; c->cand_n = cand_n; c->cand = cand;
+    }
+    return w.off;
+}
+
+static void tangential_axes(int a, int* t0, int* t1) {
+    *t0 = a == 0 ? 1 : 0;
+    *t1 = a == 2 ? 1 : 2;
+}
+
+int ib_adhesion_workspace_bytes(const plb_grid* grid, int wall_axis, long n_receptors, size_t* out_bytes) {
+    long cells;
+    int rc = check_grid(grid, &cells);
+    if (rc) return rc;
+    if (!out_bytes || wall_axis < 0 || wall_axis > 2 || n_receptors < 0) {
+        set_error("ib_adhesion_workspace_bytes: invalid argument");
+        return PLB_ERR_ARG;
+    }
+    const int n[3] = {grid->nx, grid->ny, grid->nz};
+    int t0, t1;
+    tangential_axes(wall_axis, &t0, &t1);
+    *out_bytes = carve_adhesion(nullptr, nullptr, (long)n[t0] * n[t1], n_receptors);
+    return PLB_OK;
+}
+
+int ib_set_receptors(plb_ctx* ctx, long n_receptors, const int* h_node, const plb_adhesion* prm, void* d_workspace,
+                     size_t workspace_bytes) {
+    REQUIRE_CTX(ctx);
+    if (n_receptors < 0 || (n_receptors > 0 && !h_node) || !prm || !d_workspace || ((uintptr_t)d_workspace & 255) != 0) {
+        set_error("ib_set_receptors: invalid argument (the workspace must be non-null and 256-byte aligned)");
+        return PLB_ERR_ARG;
+    }
+    const int a = prm->wall_axis;
+    if (a < 0 || a > 2 || ctx->bnd.kind[a] == PLB_PERIODIC) {
+        set_error("ib_set_receptors: wall_axis %d is not a wall axis of this context", a);
+        return PLB_ERR_ARG;
+    }
+    if (prm->max_per_site < 1 || prm->max_per_site > ADH_MAX_CAND || !(prm->l_max > 0.f) || prm->k_on0 < 0.f ||
+        prm->k_off0 < 0.f || prm->F0 < 0.f || prm->tau_rep < 0.f) {
+        set_error("ib_set_receptors: invalid parameters (1 <= max_per_site <= %d, l_max > 0, rates, F0, tau_rep >= 0)", ADH_MAX_CAND);
+        return PLB_ERR_ARG;
+    }
+    if (n_receptors >= (1L << 31)) {
+        set_error("ib_set_receptors: more than 2^31 receptors");
+        return PLB_ERR_ARG;
+    }
+    for (long r = 0; r < n_receptors; ++r)
+        if (h_node[r] < 0 || h_node[r] >= ctx->n_nodes) {
+            set_error("ib_set_receptors: receptor %ld sits on node %d, out of range", r, h_node[r]);
+            return PLB_ERR_ARG;
+        }
+    const int n[3] = {ctx->grid.nx, ctx->grid.ny, ctx->grid.nz};
+    int t0, t1;
+    tangential_axes(a, &t0, &t1);
+    const long n_sites = (long)n[t0] * n[t1];
+    const size_t need = carve_adhesion(nullptr, nullptr, n_sites, n_receptors);
+    if (workspace_bytes < need) {
+        set_error("ib_set_receptors: workspace of %zu bytes is smaller than the %zu needed", workspace_bytes, need);
+        return PLB_ERR_WORKSPACE;
+    }
+    carve_adhesion(ctx, (char*)d_workspace, n_sites, n_receptors);
+    AdhParams& p = ctx->adh;
+    p.a = a; p.t0 = t0; p.t1 = t1; p.n0 = n[t0]; p.n1 = n[t1];
+    p.per0 = ctx->bnd.kind[t0] == PLB_PERIODIC; p.per1 = ctx->bnd.kind[t1] == PLB_PERIODIC;
+    p.max_per_site = prm->max_per_site;
+    p.plane = ctx->bnd.kind[a] == PLB_WALL_HH ? 0.0 : -0.5;
+    p.k_on0 = prm->k_on0; p.k_off0 = prm->k_off0; p.s = prm->s; p.gamma = prm->gamma; p.sigma = prm->sigma;
+    p.l_b = prm->l_b; p.l_max = prm->l_max; p.F0 = prm->F0; p.tau_rep = prm->tau_rep;
+    ctx->n_rec = n_receptors;
+    ctx->adh_on = true;
+    int rc = cuda_check(cudaMemsetAsync(d_workspace, 0, need, ctx->stream), "clear adhesion workspace");
+    if (!rc && n_receptors)
+        rc = cuda_check(cudaMemcpyAsync(ctx->rec_node, h_node, (size_t)n_receptors * sizeof(int), cudaMemcpyHostToDevice,
+                                        ctx->stream), "upload receptor nodes");
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    ctx->forces_valid = false;
+    return rc;
+}
+
+int ib_adhesion_update(plb_ctx* ctx, unsigned long long seed, unsigned long long step) {
+    REQUIRE_CTX(ctx);
+    if (!ctx->adh_on) {
+        set_error("ib_adhesion_update before ib_set_receptors");
+        return PLB_ERR_ORDER;
+    }
+    ctx->forces_valid = false;
+    return launch_adhesion_update(ctx, seed, step);
+}
+
+int ib_n_receptors(plb_ctx* ctx, long* out) {
+    REQUIRE_CTX(ctx);
+    if (!out) return PLB_ERR_ARG;
+    *out = ctx->adh_on ? ctx->n_rec : 0;
+    return PLB_OK;
+}
+
+int ib_read_bonds(plb_ctx* ctx, int* h_bonds) {
+    REQUIRE_CTX(ctx);
+    if (!h_bonds || !ctx->adh_on) {
+        set_error("ib_read_bonds: null output or no receptors set");
+        return h_bonds ? PLB_ERR_ORDER : PLB_ERR_ARG;
+    }
+    const long n = ctx->n_rec;
+    std::vector<int4> tmp((size_t)n);
+    int rc = PLB_OK;
+    if (n) rc = cuda_check(cudaMemcpyAsync(tmp.data(), ctx->bond, (size_t)n * sizeof(int4), cudaMemcpyDeviceToHost, ctx->stream),
+                           "download bonds");
+    if (!rc) rc = sync_status(ctx);
+    for (long r = 0; r < n; ++r) {
+        h_bonds[3 * r] = tmp[r].x; h_bonds[3 * r + 1] = tmp[r].y; h_bonds[3 * r + 2] = tmp[r].z;
+    }
+    return rc;
+}
+
+int ib_write_bonds(plb_ctx* ctx, const int* h_bonds) {
+    REQUIRE_CTX(ctx);
+    if (!h_bonds || !ctx->adh_on) {
+        set_error("ib_write_bonds: null input or no receptors set");
+        return h_bonds ? PLB_ERR_ORDER : PLB_ERR_ARG;
+    }
+    const long n = ctx->n_rec;
+    std::vector<int4> tmp((size_t)n);
+    for (long r = 0; r < n; ++r) {
+        const int on = h_bonds[3 * r] ? 1 : 0;
+        tmp[r] = make_int4(on, on ? h_bonds[3 * r + 1] : 0, on ? h_bonds[3 * r + 2] : 0, -1);
+    }
+    int rc = PLB_OK;
+    if (n) rc = cuda_check(cudaMemcpyAsync(ctx->bond, tmp.data(), (size_t)n * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream),
+                           "upload bonds");
+    if (!rc) rc = launch_adhesion_recount(ctx);
+    if (!rc) rc = sync_status(ctx);
     ctx->forces_valid = false;
     return rc;
 }

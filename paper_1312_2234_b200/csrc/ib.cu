@@ -605,6 +605,8 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
             c->X[0], c->X[1], c->X[2], c->tris, c->tri_S0, c->cons, c->F);
         c->launches++;
     }
+    const int rc = launch_adhesion_forces(c);
+    if (rc) return rc;
     return cuda_check(cudaGetLastError(), "membrane force kernels");
 }
 

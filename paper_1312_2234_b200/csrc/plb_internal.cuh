@@ -57,7 +57,16 @@ struct MeshConstraint {
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 
 // status bits raised by kernels (sticky)
-enum { STATUS_NODE_LEFT = 1, STATUS_ZERO_EDGE = 2 };
+enum { STATUS_NODE_LEFT = 1, STATUS_ZERO_EDGE = 2, STATUS_ADH_OVERFLOW = 4, STATUS_ADH_BAD_SITE = 8 };
+
+// NEXT-4 (section 3.2 / 3.4.1): adhesion parameters as the kernels take them.  a = wall
+// axis, (t0, t1) the tangential axes in x, y, z order, (n0, n1) their sizes = the vWF site grid,
+// plane = position of the wall plane on axis a.  Decision arithmetic is fp64 (adhesion.cu).
+constexpr int ADH_MAX_CAND = 32;   // same-step formation candidates one site can list
+struct AdhParams {
+    int a, t0, t1, n0, n1, per0, per1, max_per_site;
+    double plane, k_on0, k_off0, s, gamma, sigma, l_b, l_max, F0, tau_rep;
+};
 
 __device__ __forceinline__ bool seg_active(const unsigned* __restrict__ seg_mask, const int cell) {
     return (__ldg(seg_mask + (cell >> (SEG_SHIFT + 5))) >> ((cell >> SEG_SHIFT) & 31)) & 1u;
@@ -124,6 +133,15 @@ struct Ctx {
     int2* ranges;              // node ranges [first, last) served by one thread block of the IB kernels
     long n_ranges;
     int tile_cap;              // cells of the shared-memory lattice tile of the IB kernels
+    // NEXT-4: receptors and bonds (carved from the caller's adhesion workspace)
+    bool adh_on;
+    AdhParams adh;
+    long n_rec;
+    int* rec_node;             // global node of each receptor
+    int4* bond;                // (bound, s0, s1, candidate site of the running update or -1)
+    int* site_count;           // bonds per vWF site, n0 * n1
+    int* cand_n;               // same-step formation candidates per site
+    int* cand;                 // their receptor indices, ADH_MAX_CAND per site
     // bookkeeping
     const float4* g_last;
     int g_last_mode;           // ForceMode used by the last lbm_step
@@ -152,6 +170,9 @@ int launch_spread(Ctx* c, float4* g);
 int launch_interpolate_advance(Ctx* c);
 int ib_max_tile_cap();
 int launch_nodes_transpose(Ctx* c, bool to_aos);
+int launch_adhesion_forces(Ctx* c);
+int launch_adhesion_update(Ctx* c, unsigned long long seed, unsigned long long step);
+int launch_adhesion_recount(Ctx* c);
 int launch_philox(cudaStream_t s, long n, const unsigned* ctr, const unsigned* key, unsigned* out);
 
 }  // namespace plb
