@@ -175,7 +175,10 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
 // lane walks the 4 x 4 (oy, oz) cells of its column; the lanes also share the per-node set-up
 // (lane a < 3 does floor / sincospi of axis a) and finish with a 4-lane shuffle reduction.
 // ---------------------------------------------------------------------------------------------
-constexpr int IB_THREADS = 512;
+#ifndef PLB_IB_THREADS
+#define PLB_IB_THREADS 512
+#endif
+constexpr int IB_THREADS = PLB_IB_THREADS;
 constexpr int NODE_LANES = 4;
 constexpr int IB_GROUPS = IB_THREADS / NODE_LANES;
 
@@ -289,13 +292,17 @@ __device__ __forceinline__ void weights4(const float s, const float c, float (&w
     w[2] = fmaf(0.25f, s, 0.25f);  w[3] = fmaf(-0.25f, c, 0.25f);
 }
 
-// All 32 lanes call this (m clamped by the caller); lane a < 3 of each 4-lane group evaluates
-// axis a (fp64 floor, sincospi of the fraction), then the group exchanges by shuffle.
-template <bool WEIGHTS>
-__device__ __forceinline__ NodeStencil node_stencil(const double* X, const double* Y, const double* Z, const int m, const int sub,
-                                                    const int o0, const int o1, const int o2) {
+// All 32 lanes call this; lane a < 3 of each 4-lane group holds x = coordinate a of the node (lane
+// 3 a copy of X) and evaluates that axis (fp64 floor, sincospi of the fraction), then the group
+// exchanges by shuffle.  The caller loads x one sweep ahead (node_coord) so that the global-load
+// latency hides behind the previous sweep's shared-memory work.
+__device__ __forceinline__ double node_coord(const double* X, const double* Y, const double* Z, const int m, const int sub) {
     const double* P = sub == 1 ? Y : (sub == 2 ? Z : X);
-    const double x = P[m];
+    return P[m];
+}
+
+template <bool WEIGHTS>
+__device__ __forceinline__ NodeStencil node_stencil(const double x, const int sub, const int o0, const int o1, const int o2) {
     const double fl = floor(x);
     const int base = (int)fl - 1 - (sub == 1 ? o1 : (sub == 2 ? o2 : o0));
     float s = 0.f, c = 0.f;
@@ -340,7 +347,7 @@ __device__ __forceinline__ void spread_column(int* __restrict__ tile, const int 
 }
 
 // S2: g_ijk += F_m phi phi phi (Eq. 34).  Also sets the activity bits of the touched segments.
-__global__ void __launch_bounds__(IB_THREADS) spread_mesh_kernel(
+__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_kernel(
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
@@ -364,11 +371,16 @@ __global__ void __launch_bounds__(IB_THREADS) spread_mesh_kernel(
     __syncthreads();
     const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
     const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
+    double x_next = node_coord(X, Y, Z, min(n0 + group, n1 - 1), sub);
+    float4 F_next = __ldg(F + min(n0 + group, n1 - 1));
     for (int mb = n0; mb < n1; mb += IB_GROUPS) {                      // warp-uniform trip count
         const bool valid = mb + group < n1;
-        const int m = valid ? mb + group : n1 - 1;
-        const NodeStencil st = node_stencil<true>(X, Y, Z, m, sub, o0, o1, o2);
-        const float4 Fm = __ldg(F + m);
+        const double x = x_next;
+        const float4 Fm = F_next;
+        const int m_next = min(mb + IB_GROUPS + group, n1 - 1);        // one sweep ahead
+        x_next = node_coord(X, Y, Z, m_next, sub);
+        F_next = __ldg(F + m_next);
+        const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
         if (!valid) continue;
         const float fx = Fm.x * scale * st.wx, fy = Fm.y * scale * st.wx, fz = Fm.z * scale * st.wx;
         if (tiled) {
@@ -449,7 +461,7 @@ __device__ __forceinline__ void gather_column(const float4* __restrict__ tile, c
 // S4 + S5: U_m = sum v phi phi phi (Eq. 33) with v = (sum c_i f_i + g/2)/rho of the state after
 // lbm_step (G11), each of a node's four lanes summing its stencil column, then a 4-lane
 // shuffle reduction, then X_m += U_m in fp64.
-__global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
+__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mesh_kernel(
     double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z, float4* __restrict__ U,
     const int2* __restrict__ ranges, const float* __restrict__ src, const float4* __restrict__ g,
     int* __restrict__ counters, const LbmParams p, const int cap) {
@@ -468,9 +480,12 @@ __global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
         unsigned* need = reinterpret_cast<unsigned*>(smem_raw);       // marks alias the (not yet filled) tile
         for (int t = tid; t < ncell; t += IB_THREADS) need[t] = 0u;
         __syncthreads();
+        double x_next = node_coord(X, Y, Z, min(n0 + group, n1 - 1), sub);
         for (int mb = n0; mb < n1; mb += IB_GROUPS) {                  // the 4^3 cells each node needs
             const bool valid = mb + group < n1;
-            const NodeStencil st = node_stencil<false>(X, Y, Z, valid ? mb + group : n1 - 1, sub, o0, o1, o2);
+            const double x = x_next;
+            x_next = node_coord(X, Y, Z, min(mb + IB_GROUPS + group, n1 - 1), sub);
+            const NodeStencil st = node_stencil<false>(x, sub, o0, o1, o2);
             const int tx = st.bx + sub;
             if (!valid || tx < T.lo[0] || tx >= T.hi[0]) continue;
 #pragma unroll
@@ -514,10 +529,15 @@ __global__ void __launch_bounds__(IB_THREADS) interpolate_mesh_kernel(
         }
         __syncthreads();
     }
+    // positions one sweep ahead: sweep i + 1 reads nodes that sweep i does not write (a clamped tail
+    // lane may re-read node n1 - 1 after it moved, but such a lane is not valid and its value unused)
+    double x_next = node_coord(X, Y, Z, min(n0 + group, n1 - 1), sub);
     for (int mb = n0; mb < n1; mb += IB_GROUPS) {
         const bool valid = mb + group < n1;
         const int m = valid ? mb + group : n1 - 1;
-        const NodeStencil st = node_stencil<true>(X, Y, Z, m, sub, o0, o1, o2);
+        const double x = x_next;
+        x_next = node_coord(X, Y, Z, min(mb + IB_GROUPS + group, n1 - 1), sub);
+        const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
         float ux = 0.f, uy = 0.f, uz = 0.f;
         if (tiled) {
             if (T.clipped) gather_column<true>(tile, T, st, st.bx + sub, ux, uy, uz);
