@@ -218,6 +218,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->adh_on = false; c->n_rec = 0;
     c->list_parity = 0;
     c->tile_cap = 512;
+    c->spread_cap = 1024;
     c->sm_count = sms;
     c->mesh_node_off.push_back(0);
     c->mesh_edge_off.push_back(0);
@@ -372,7 +373,7 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
     // capacity their initial bounding boxes ask for (two cells of slack per axis for deformation)
     constexpr int IB_RANGE_NODES = 4096;
     std::vector<int2> rg;
-    int cap = ctx->tile_cap;
+    int cap = ctx->tile_cap, scap = ctx->spread_cap;
     for (int s = 0; s < n_meshes; ++s) {
         const long noff = ctx->n_nodes + (long)s * n_nodes;
         const double* x = h_xyz + (size_t)3 * s * n_nodes;
@@ -380,6 +381,7 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
             const int b = a + IB_RANGE_NODES < n_nodes ? a + IB_RANGE_NODES : n_nodes;
             rg.push_back(make_int2((int)(noff + a), (int)(noff + b)));
             double vol = 1.0;
+            int ext[3];
             for (int d = 0; d < 3; ++d) {
                 double lo = floor(x[3 * a + d]), hi = lo;
                 for (int m = a + 1; m < b; ++m) {
@@ -388,11 +390,29 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
                     hi = f > hi ? f : hi;
                 }
                 vol *= hi - lo + 4.0 + 2.0;
+                ext[d] = hi - lo < 1e6 ? (int)(hi - lo) + 6 : 1 << 20;
             }
-            if (vol <= (double)ib_max_tile_cap() && (int)vol > cap) cap = (int)vol;
+            // a mesh may turn (a flipping platelet): size for the cube of its largest extent when that
+            // fits, else for the initial box; the spread tile is padded (tile_row_pitch / tile_plane_pitch)
+            const int emax = ext[0] > ext[1] ? (ext[0] > ext[2] ? ext[0] : ext[2]) : (ext[1] > ext[2] ? ext[1] : ext[2]);
+            const double cube = (double)emax * emax * emax;
+            int box[3] = {ext[0], ext[1], ext[2]};
+            if (cube <= 6144.0 && cube <= (double)ib_max_tile_cap() &&      // 6144 cells: two blocks per SM stay resident
+                tile_plane_pitch(tile_row_pitch(emax), emax) * emax <= ib_max_spread_cap()) {
+                vol = cube;
+                box[0] = box[1] = box[2] = emax;
+            }
+            if (vol <= (double)ib_max_tile_cap()) {
+                const int padded = tile_plane_pitch(tile_row_pitch(box[0]), box[1]) * box[2];
+                if (padded <= ib_max_spread_cap()) {
+                    if ((int)vol > cap) cap = (int)vol;
+                    if (padded > scap) scap = padded;
+                }
+            }
         }
     }
     ctx->tile_cap = cap;
+    ctx->spread_cap = scap;
     int rc = cuda_check(cudaMemcpyAsync(ctx->ranges + ctx->n_ranges, rg.data(), rg.size() * sizeof(int2),
                                         cudaMemcpyHostToDevice, ctx->stream), "upload node ranges");
     for (int d = 0; d < 3 && !rc; ++d)

@@ -185,6 +185,7 @@ constexpr int IB_GROUPS = IB_THREADS / NODE_LANES;
 struct MeshTile {
     int o[3];            // unwrapped lattice coordinate of tile cell (0,0,0)
     int e[3];            // extent in cells
+    int p0, pp;          // row and plane pitch of the stored tile (= e[0], e[0] * e[1] unless padded)
     int lo[3], hi[3];    // tile coordinates [lo, hi) that exist on the lattice (wall axes clip)
     int enabled;
     int clipped;         // some [lo, hi) is smaller than the extent: stencils need the range check
@@ -210,7 +211,7 @@ __device__ __forceinline__ void mark_segment(const int cell, unsigned* __restric
 // with F != nullptr also the largest force component of the range
 __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict__ X, const double* __restrict__ Y,
                                            const double* __restrict__ Z, const float4* __restrict__ F, const int n0,
-                                           const int n1, const LbmParams& p, const int cap) {
+                                           const int n1, const LbmParams& p, const int cap, const bool padded) {
     if (threadIdx.x == 0) {
         for (int a = 0; a < 3; ++a) { T.mn[a] = INT_MAX; T.mx[a] = INT_MIN; }
         T.fmax_bits = 0u;
@@ -261,6 +262,9 @@ __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict
             clipped = clipped || T.lo[a] != 0 || T.hi[a] != T.e[a];
             interior = interior && (long long)T.o[a] >= 1 && (long long)T.o[a] + ext <= (long long)n[a] - 1;
         }
+        T.p0 = padded ? tile_row_pitch(T.e[0]) : T.e[0];
+        T.pp = padded ? tile_plane_pitch(T.p0, T.e[1]) : T.e[0] * T.e[1];
+        ok = ok && (long long)T.pp * T.e[2] <= (long long)cap;
         T.enabled = ok ? 1 : 0;
         T.clipped = clipped ? 1 : 0;
         T.interior = (ok && interior) ? 1 : 0;
@@ -323,30 +327,39 @@ __device__ __forceinline__ NodeStencil node_stencil(const double x, const int su
     return st;
 }
 
-// one lane's column of the spread into the shared fixed-point tile
+// S2: g_ijk += F_m phi phi phi (Eq. 34).  Also sets the activity bits of the touched segments.
+// One WARP per node: lane = (ox, oy, oz & 1) covers the 4 x 4 x 2 cells of half the stencil, two
+// instructions per force component cover all 64.  The tile is stored with a row pitch = 4 (mod 8)
+// and a plane pitch = 16 (mod 32) words, so the 32 addresses of one instruction fall into 32
+// different banks: no replays inside a warp, whatever the node's position, and no two lanes of a
+// warp ever hit the same word (which is what serialises a one-lane-per-node scatter when many
+// nodes share a cell, config 5).  Lanes 0-2 evaluate the three axes (fp64 floor, sincospi) of the
+// node, loaded one node ahead, and the warp exchanges by shuffle.
 template <bool CHECK>
-__device__ __forceinline__ void spread_column(int* __restrict__ tile, const int cap, const MeshTile& T,
-                                              const NodeStencil& st, const int tx, const float fx, const float fy,
-                                              const float fz) {
-    const int e0 = T.e[0], e10 = T.e[0] * T.e[1];
-    if (CHECK && (tx < T.lo[0] || tx >= T.hi[0])) return;
-    const int t0 = (st.bz * T.e[1] + st.by) * e0 + tx;
-#pragma unroll
-    for (int oz = 0; oz < 4; ++oz) {
-        if (CHECK && (st.bz + oz < T.lo[2] || st.bz + oz >= T.hi[2])) continue;
-#pragma unroll
-        for (int oy = 0; oy < 4; ++oy) {
-            if (CHECK && (st.by + oy < T.lo[1] || st.by + oy >= T.hi[1])) continue;
-            const float W = st.wy[oy] * st.wz[oz];
-            const int t = t0 + oz * e10 + oy * e0;
-            atomicAdd(tile + t, __float2int_rn(W * fx));
-            atomicAdd(tile + cap + t, __float2int_rn(W * fy));
-            atomicAdd(tile + 2 * cap + t, __float2int_rn(W * fz));
-        }
+__device__ __forceinline__ void spread_node(int* __restrict__ tile, const int cap, const MeshTile& T, const int tx,
+                                            const int ty, const int tz0, const float w0, const float w1, const float fx,
+                                            const float fy, const float fz) {
+    if (CHECK && (tx < T.lo[0] || tx >= T.hi[0] || ty < T.lo[1] || ty >= T.hi[1])) return;
+    const int t0 = tz0 * T.pp + ty * T.p0 + tx;
+    if (!CHECK || (tz0 >= T.lo[2] && tz0 < T.hi[2])) {
+        atomicAdd(tile + t0, __float2int_rn(w0 * fx));
+        atomicAdd(tile + cap + t0, __float2int_rn(w0 * fy));
+        atomicAdd(tile + 2 * cap + t0, __float2int_rn(w0 * fz));
+    }
+    if (!CHECK || (tz0 + 2 >= T.lo[2] && tz0 + 2 < T.hi[2])) {
+        const int t1 = t0 + 2 * T.pp;
+        atomicAdd(tile + t1, __float2int_rn(w1 * fx));
+        atomicAdd(tile + cap + t1, __float2int_rn(w1 * fy));
+        atomicAdd(tile + 2 * cap + t1, __float2int_rn(w1 * fz));
     }
 }
 
-// S2: g_ijk += F_m phi phi phi (Eq. 34).  Also sets the activity bits of the touched segments.
+// phi(frac + 1 - o) from s = sin(pi frac/2), c = cos(pi frac/2): o = 0: (1 - s)/4, 1: (1 + c)/4,
+// 2: (1 + s)/4, 3: (1 - c)/4
+__device__ __forceinline__ float weight_o(const float s, const float c, const int o) {
+    return fmaf((o == 0 || o == 3) ? -0.25f : 0.25f, (o & 1) ? c : s, 0.25f);
+}
+
 __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_kernel(
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
@@ -354,61 +367,71 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     const int cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
-    int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point
+    int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point, padded pitches
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, F, n0, n1, p, cap);
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true);
     const float fmax = __uint_as_float(T.fmax_bits);
     if (!(fmax > 0.f)) return;                                         // nothing to spread
     const bool tiled = T.enabled != 0 && fmax < 3.0e38f;
-    const int ncell = tiled ? T.e[0] * T.e[1] * T.e[2] : 0;
+    const int nword = tiled ? T.pp * T.e[2] : 0;
     // |tile value| <= n_nodes * max W * max|F| = bound; scale = 2^k with bound * scale < 2^30
     const int k = max(-100, min(100, 29 - ilogbf(0.125f * (float)(n1 - n0) * fmax)));
     const float scale = tiled ? ldexpf(1.0f, k) : 1.0f, inv_scale = ldexpf(1.0f, -k);
-    for (int t = tid; t < ncell; t += IB_THREADS) {
+    for (int t = tid; t < nword; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
     __syncthreads();
-    const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int ox = lane & 3, oy = (lane >> 2) & 3, oz = lane >> 4;       // this lane's cells: (ox, oy, oz) and (ox, oy, oz + 2)
     const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
-    double x_next = node_coord(X, Y, Z, min(n0 + group, n1 - 1), sub);
-    float4 F_next = __ldg(F + min(n0 + group, n1 - 1));
-    for (int mb = n0; mb < n1; mb += IB_GROUPS) {                      // warp-uniform trip count
-        const bool valid = mb + group < n1;
+    const int axis = lane < 3 ? lane : 0;                              // lanes 0-2 evaluate x, y, z
+    const double* P = axis == 1 ? Y : (axis == 2 ? Z : X);
+    const int origin = axis == 1 ? o1 : (axis == 2 ? o2 : o0);
+    double x_next = n0 + warp < n1 ? P[n0 + warp] : 0.0;
+    float4 F_next = n0 + warp < n1 ? __ldg(F + n0 + warp) : make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int m = n0 + warp; m < n1; m += IB_THREADS / 32) {
         const double x = x_next;
         const float4 Fm = F_next;
-        const int m_next = min(mb + IB_GROUPS + group, n1 - 1);        // one sweep ahead
-        x_next = node_coord(X, Y, Z, m_next, sub);
-        F_next = __ldg(F + m_next);
-        const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
-        if (!valid) continue;
-        const float fx = Fm.x * scale * st.wx, fy = Fm.y * scale * st.wx, fz = Fm.z * scale * st.wx;
+        const int m_next = m + IB_THREADS / 32;                        // one node ahead
+        if (m_next < n1) { x_next = P[m_next]; F_next = __ldg(F + m_next); }
+        const double fl = floor(x);
+        const int base = (int)fl - 1 - origin;
+        float s, c;
+        sincospif(0.5f * (float)(x - fl), &s, &c);
+        const int bx = __shfl_sync(0xffffffffu, base, 0), by = __shfl_sync(0xffffffffu, base, 1),
+                  bz = __shfl_sync(0xffffffffu, base, 2);
+        const float sx = __shfl_sync(0xffffffffu, s, 0), cx = __shfl_sync(0xffffffffu, c, 0);
+        const float sy = __shfl_sync(0xffffffffu, s, 1), cy = __shfl_sync(0xffffffffu, c, 1);
+        const float sz = __shfl_sync(0xffffffffu, s, 2), cz = __shfl_sync(0xffffffffu, c, 2);
+        const float wxy = weight_o(sx, cx, ox) * weight_o(sy, cy, oy);
+        const float w0 = wxy * weight_o(sz, cz, oz), w1 = wxy * weight_o(sz, cz, oz + 2);
+        const float fx = Fm.x * scale, fy = Fm.y * scale, fz = Fm.z * scale;
         if (tiled) {
-            if (T.clipped) spread_column<true>(tile, cap, T, st, st.bx + sub, fx, fy, fz);
-            else           spread_column<false>(tile, cap, T, st, st.bx + sub, fx, fy, fz);
+            if (T.clipped) spread_node<true>(tile, cap, T, bx + ox, by + oy, bz + oz, w0, w1, fx, fy, fz);
+            else           spread_node<false>(tile, cap, T, bx + ox, by + oy, bz + oz, w0, w1, fx, fy, fz);
         } else {
-            const int qx = wrap_index(st.bx + sub, p.nx, p.wall[0]);
-            if (qx < 0) continue;
+            const int qx = wrap_index(bx + ox, p.nx, p.wall[0]), qy = wrap_index(by + oy, p.ny, p.wall[1]);
+            if (qx < 0 || qy < 0) continue;
 #pragma unroll
-            for (int oz = 0; oz < 4; ++oz) {
-                const int qz = wrap_index(st.bz + oz, p.nz, p.wall[2]);
+            for (int h = 0; h < 2; ++h) {
+                const int qz = wrap_index(bz + oz + 2 * h, p.nz, p.wall[2]);
                 if (qz < 0) continue;
-#pragma unroll
-                for (int oy = 0; oy < 4; ++oy) {
-                    const int qy = wrap_index(st.by + oy, p.ny, p.wall[1]);
-                    if (qy < 0) continue;
-                    const float W = st.wy[oy] * st.wz[oz];
-                    const int cell = qx + p.nx * (qy + p.ny * qz);
-                    atomicAdd(g + cell, make_float4(W * fx, W * fy, W * fz, 0.f));
-                    mark_segment(cell, seg_mask, seg_list, seg_count);
-                }
+                const float W = h ? w1 : w0;
+                const int cell = qx + p.nx * (qy + p.ny * qz);
+                atomicAdd(g + cell, make_float4(W * fx, W * fy, W * fz, 0.f));
+                mark_segment(cell, seg_mask, seg_list, seg_count);
             }
         }
     }
     if (!tiled) return;
     __syncthreads();
+    const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
     for (int t = tid; t < ncell; t += IB_THREADS) {
-        const int qx = tile[t], qy = tile[cap + t], qz = tile[2 * cap + t];
+        const int x = t % e0, r = t / e0;
+        const int y = r % e1, z = r / e1;
+        const int w = z * T.pp + y * T.p0 + x;
+        const int qx = tile[w], qy = tile[cap + w], qz = tile[2 * cap + w];
         if ((qx | qy | qz) != 0) {
             const Cell c = tile_cell(T, t, p);
             const int cell = c.i + p.nx * (c.j + p.ny * c.k);
@@ -471,7 +494,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
     unsigned short* list = reinterpret_cast<unsigned short*>(tile + cap);   // [cap] needed tile cells
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap);
+    tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, false);
     const bool tiled = T.enabled != 0;
     const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
     const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
@@ -653,15 +676,18 @@ int ib_max_tile_cap() {
     return (int)(cap < 65535 ? cap : 65535);
 }
 
+// words per component of the padded spread tile: two blocks of 110 KB per SM
+int ib_max_spread_cap() { return (int)((110 * 1024) / 12); }
+
 int launch_spread(Ctx* c, float4* g) {
     if (c->n_nodes == 0) return PLB_OK;
-    const size_t smem = spread_smem(c->tile_cap);
+    const size_t smem = spread_smem(c->spread_cap);
     int rc = cuda_check(cudaFuncSetAttribute(spread_mesh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                         "cudaFuncSetAttribute(spread_mesh_kernel)");
     if (rc) return rc;
     spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
         c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, c->counters + 2 + c->list_parity, c->prm,
-        c->tile_cap);
+        c->spread_cap);
     c->launches++;
     return cuda_check(cudaGetLastError(), "spread_mesh_kernel");
 }

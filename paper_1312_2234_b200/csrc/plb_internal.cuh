@@ -54,6 +54,15 @@ struct MeshConstraint {
     float k_s, k_t, k_v, pad2;
 };
 
+// Pitches of the spread kernel's shared-memory tile (ib.cu): a row pitch = 4 (mod 8) and a plane
+// pitch = 16 (mod 32) put the 4 x 4 x 2 cells one warp instruction touches (4 consecutive x, 4 rows,
+// 2 planes) into 32 different banks.
+__host__ __device__ inline int tile_row_pitch(const int e0) { return e0 + ((4 - (e0 & 7)) & 7); }
+__host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e1) {
+    const int v = row_pitch * e1;
+    return v + ((16 - (v & 31)) & 31);
+}
+
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 
 // status bits raised by kernels (sticky)
@@ -132,7 +141,8 @@ struct Ctx {
     std::vector<char> mesh_constrained;
     int2* ranges;              // node ranges [first, last) served by one thread block of the IB kernels
     long n_ranges;
-    int tile_cap;              // cells of the shared-memory lattice tile of the IB kernels
+    int tile_cap;              // cells of the shared-memory lattice tile of the interpolation kernel
+    int spread_cap;            // words per component of the (padded, bank-conflict-free) spread tile
     // NEXT-4: receptors and bonds (carved from the caller's adhesion workspace)
     bool adh_on;
     AdhParams adh;
@@ -169,6 +179,7 @@ int launch_clear_spread(Ctx* c, float4* g);
 int launch_spread(Ctx* c, float4* g);
 int launch_interpolate_advance(Ctx* c);
 int ib_max_tile_cap();
+int ib_max_spread_cap();
 int launch_nodes_transpose(Ctx* c, bool to_aos);
 int launch_adhesion_forces(Ctx* c);
 int launch_adhesion_update(Ctx* c, unsigned long long seed, unsigned long long step);
