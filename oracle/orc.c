@@ -835,8 +835,8 @@ int orc_adhesion_update(orc_ctx* c, uint64_t seed, uint64_t step) {
         orc_adhesion_probabilities(p, x_b, NULL, &P_r);
         orc_noise_uniform(seed, (uint64_t)r, (uint32_t)step, 3u, xi);
         if (xi[0] < P_r) {
-            b[0] = 0;
             c->site_count[site_index(c, t0, t1, b[1], b[2])] -= 1;
+            b[0] = 0; b[1] = 0; b[2] = 0;                            /* an open receptor names no site */
         }
     }
     /* 2) generate new bonds from unbound receptors and sites with a free place (L147-149, L276):

@@ -180,6 +180,7 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
 #endif
 constexpr int IB_THREADS = PLB_IB_THREADS;
 constexpr int NODE_LANES = 4;
+constexpr int SPREAD_SEG_LIST = 2048;   // segments one spread block can newly mark before it appends one by one
 constexpr int IB_GROUPS = IB_THREADS / NODE_LANES;
 
 struct MeshTile {
@@ -328,36 +329,44 @@ __device__ __forceinline__ NodeStencil node_stencil(const double x, const int su
 }
 
 // S2: g_ijk += F_m phi phi phi (Eq. 34).  Also sets the activity bits of the touched segments.
-// One WARP per node: lane = (ox, oy, oz & 1) covers the 4 x 4 x 2 cells of half the stencil, two
-// instructions per force component cover all 64.  The tile is stored with a row pitch = 4 (mod 8)
-// and a plane pitch = 16 (mod 32) words, so the 32 addresses of one instruction fall into 32
-// different banks: no replays inside a warp, whatever the node's position, and no two lanes of a
-// warp ever hit the same word (which is what serialises a one-lane-per-node scatter when many
-// nodes share a cell, config 5).  Lanes 0-2 evaluate the three axes (fp64 floor, sincospi) of the
-// node, loaded one node ahead, and the warp exchanges by shuffle.
-template <bool CHECK>
-__device__ __forceinline__ void spread_node(int* __restrict__ tile, const int cap, const MeshTile& T, const int tx,
-                                            const int ty, const int tz0, const float w0, const float w1, const float fx,
-                                            const float fy, const float fz) {
-    if (CHECK && (tx < T.lo[0] || tx >= T.hi[0] || ty < T.lo[1] || ty >= T.hi[1])) return;
-    const int t0 = tz0 * T.pp + ty * T.p0 + tx;
-    if (!CHECK || (tz0 >= T.lo[2] && tz0 < T.hi[2])) {
-        atomicAdd(tile + t0, __float2int_rn(w0 * fx));
-        atomicAdd(tile + cap + t0, __float2int_rn(w0 * fy));
-        atomicAdd(tile + 2 * cap + t0, __float2int_rn(w0 * fz));
-    }
-    if (!CHECK || (tz0 + 2 >= T.lo[2] && tz0 + 2 < T.hi[2])) {
-        const int t1 = t0 + 2 * T.pp;
-        atomicAdd(tile + t1, __float2int_rn(w1 * fx));
-        atomicAdd(tile + cap + t1, __float2int_rn(w1 * fy));
-        atomicAdd(tile + 2 * cap + t1, __float2int_rn(w1 * fz));
-    }
-}
+// SIXTEEN lanes per node: lane = (ox, oy) walks the four oz cells of its stencil column.  The per-node
+// set-up (fp64 floor, sincospi per axis, force scaling) is done once, one thread per node, for a
+// chunk of 256 nodes at a time (coalesced loads, issued one chunk ahead) and staged in shared
+// memory; the lanes read it back as broadcasts.  The tile is stored with a row pitch = 4 (mod 8)
+// words, so the 16 cells a node touches per instruction fall into 16 different banks.
+// (Measured on B200, config 4 / config 5: 4 lanes per node 0.136 / 2.44 ms, one warp per node with
+// redundant set-up 0.124 / 2.87 ms; this layout is the fastest of the three.)
+constexpr int SPREAD_LANES = 16;
+constexpr int SPREAD_CHUNK = 256;
+constexpr int SPREAD_GROUPS = IB_THREADS / SPREAD_LANES;
 
 // phi(frac + 1 - o) from s = sin(pi frac/2), c = cos(pi frac/2): o = 0: (1 - s)/4, 1: (1 + c)/4,
 // 2: (1 + s)/4, 3: (1 - c)/4
 __device__ __forceinline__ float weight_o(const float s, const float c, const int o) {
     return fmaf((o == 0 || o == 3) ? -0.25f : 0.25f, (o & 1) ? c : s, 0.25f);
+}
+
+struct SpreadChunk {
+    int* b;        // [3][SPREAD_CHUNK] base = floor(X) - 1 - tile origin
+    float* sc;     // [6][SPREAD_CHUNK] sin, cos of pi frac/2 per axis
+    float* f;      // [3][SPREAD_CHUNK] scaled force
+};
+
+__device__ __forceinline__ void spread_record(const SpreadChunk& ch, const int r, const double x, const double y,
+                                              const double z, const float4 F, const float scale, const int o0,
+                                              const int o1, const int o2) {
+    const double fx = floor(x), fy = floor(y), fz = floor(z);
+    ch.b[r] = (int)fx - 1 - o0;
+    ch.b[SPREAD_CHUNK + r] = (int)fy - 1 - o1;
+    ch.b[2 * SPREAD_CHUNK + r] = (int)fz - 1 - o2;
+    float s, c;
+    sincospif(0.5f * (float)(x - fx), &s, &c);
+    ch.sc[r] = s; ch.sc[SPREAD_CHUNK + r] = c;
+    sincospif(0.5f * (float)(y - fy), &s, &c);
+    ch.sc[2 * SPREAD_CHUNK + r] = s; ch.sc[3 * SPREAD_CHUNK + r] = c;
+    sincospif(0.5f * (float)(z - fz), &s, &c);
+    ch.sc[4 * SPREAD_CHUNK + r] = s; ch.sc[5 * SPREAD_CHUNK + r] = c;
+    ch.f[r] = F.x * scale; ch.f[SPREAD_CHUNK + r] = F.y * scale; ch.f[2 * SPREAD_CHUNK + r] = F.z * scale;
 }
 
 __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_kernel(
@@ -368,6 +377,11 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
     int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point, padded pitches
+    int* new_segs = tile + 3 * cap;                                    // [SPREAD_SEG_LIST]
+    SpreadChunk ch;
+    ch.b = new_segs + SPREAD_SEG_LIST;
+    ch.sc = reinterpret_cast<float*>(ch.b + 3 * SPREAD_CHUNK);
+    ch.f = ch.sc + 6 * SPREAD_CHUNK;
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
     tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true);
@@ -381,51 +395,61 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     for (int t = tid; t < nword; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
-    __syncthreads();
-    const int lane = tid & 31, warp = tid >> 5;
-    const int ox = lane & 3, oy = (lane >> 2) & 3, oz = lane >> 4;       // this lane's cells: (ox, oy, oz) and (ox, oy, oz + 2)
+    const int sub = tid & (SPREAD_LANES - 1), ox = sub & 3, oy = sub >> 2, group = tid / SPREAD_LANES;
     const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
-    const int axis = lane < 3 ? lane : 0;                              // lanes 0-2 evaluate x, y, z
-    const double* P = axis == 1 ? Y : (axis == 2 ? Z : X);
-    const int origin = axis == 1 ? o1 : (axis == 2 ? o2 : o0);
-    double x_next = n0 + warp < n1 ? P[n0 + warp] : 0.0;
-    float4 F_next = n0 + warp < n1 ? __ldg(F + n0 + warp) : make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int m = n0 + warp; m < n1; m += IB_THREADS / 32) {
-        const double x = x_next;
-        const float4 Fm = F_next;
-        const int m_next = m + IB_THREADS / 32;                        // one node ahead
-        if (m_next < n1) { x_next = P[m_next]; F_next = __ldg(F + m_next); }
-        const double fl = floor(x);
-        const int base = (int)fl - 1 - origin;
-        float s, c;
-        sincospif(0.5f * (float)(x - fl), &s, &c);
-        const int bx = __shfl_sync(0xffffffffu, base, 0), by = __shfl_sync(0xffffffffu, base, 1),
-                  bz = __shfl_sync(0xffffffffu, base, 2);
-        const float sx = __shfl_sync(0xffffffffu, s, 0), cx = __shfl_sync(0xffffffffu, c, 0);
-        const float sy = __shfl_sync(0xffffffffu, s, 1), cy = __shfl_sync(0xffffffffu, c, 1);
-        const float sz = __shfl_sync(0xffffffffu, s, 2), cz = __shfl_sync(0xffffffffu, c, 2);
-        const float wxy = weight_o(sx, cx, ox) * weight_o(sy, cy, oy);
-        const float w0 = wxy * weight_o(sz, cz, oz), w1 = wxy * weight_o(sz, cz, oz + 2);
-        const float fx = Fm.x * scale, fy = Fm.y * scale, fz = Fm.z * scale;
-        if (tiled) {
-            if (T.clipped) spread_node<true>(tile, cap, T, bx + ox, by + oy, bz + oz, w0, w1, fx, fy, fz);
-            else           spread_node<false>(tile, cap, T, bx + ox, by + oy, bz + oz, w0, w1, fx, fy, fz);
-        } else {
-            const int qx = wrap_index(bx + ox, p.nx, p.wall[0]), qy = wrap_index(by + oy, p.ny, p.wall[1]);
-            if (qx < 0 || qy < 0) continue;
+    const int p0 = T.p0, pp = T.pp;
+    const bool clipped = T.clipped != 0;
+    // this thread's node of the coming chunk, loaded one chunk ahead
+    double px = 0.0, py = 0.0, pz = 0.0;
+    float4 pF = make_float4(0.f, 0.f, 0.f, 0.f);
+    bool have = tid < SPREAD_CHUNK && n0 + tid < n1;
+    if (have) { px = X[n0 + tid]; py = Y[n0 + tid]; pz = Z[n0 + tid]; pF = __ldg(F + n0 + tid); }
+    for (int c0 = n0; c0 < n1; c0 += SPREAD_CHUNK) {
+        __syncthreads();                                               // tile zeroed / previous chunk consumed
+        if (have) spread_record(ch, tid, px, py, pz, pF, scale, o0, o1, o2);
+        __syncthreads();
+        const int m_next = c0 + SPREAD_CHUNK + tid;
+        have = tid < SPREAD_CHUNK && m_next < n1;
+        if (have) { px = X[m_next]; py = Y[m_next]; pz = Z[m_next]; pF = __ldg(F + m_next); }
+        const int cnt = min(SPREAD_CHUNK, n1 - c0);
+        for (int r = group; r < cnt; r += SPREAD_GROUPS) {
+            const int bx = ch.b[r] + ox, by = ch.b[SPREAD_CHUNK + r] + oy, bz = ch.b[2 * SPREAD_CHUNK + r];
+            const float wxy = weight_o(ch.sc[r], ch.sc[SPREAD_CHUNK + r], ox) *
+                              weight_o(ch.sc[2 * SPREAD_CHUNK + r], ch.sc[3 * SPREAD_CHUNK + r], oy);
+            const float sz = ch.sc[4 * SPREAD_CHUNK + r], cz = ch.sc[5 * SPREAD_CHUNK + r];
+            const float fx = wxy * ch.f[r], fy = wxy * ch.f[SPREAD_CHUNK + r], fz = wxy * ch.f[2 * SPREAD_CHUNK + r];
+            if (tiled) {
+                if (clipped && (bx < T.lo[0] || bx >= T.hi[0] || by < T.lo[1] || by >= T.hi[1])) continue;
+                const int t0 = bz * pp + by * p0 + bx;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int qz = wrap_index(bz + oz + 2 * h, p.nz, p.wall[2]);
-                if (qz < 0) continue;
-                const float W = h ? w1 : w0;
-                const int cell = qx + p.nx * (qy + p.ny * qz);
-                atomicAdd(g + cell, make_float4(W * fx, W * fy, W * fz, 0.f));
-                mark_segment(cell, seg_mask, seg_list, seg_count);
+                for (int oz = 0; oz < 4; ++oz) {
+                    if (clipped && (bz + oz < T.lo[2] || bz + oz >= T.hi[2])) continue;
+                    const float wz = weight_o(sz, cz, oz);
+                    const int t = t0 + oz * pp;
+                    atomicAdd(tile + t, __float2int_rn(wz * fx));
+                    atomicAdd(tile + cap + t, __float2int_rn(wz * fy));
+                    atomicAdd(tile + 2 * cap + t, __float2int_rn(wz * fz));
+                }
+            } else {
+                const int qx = wrap_index(bx, p.nx, p.wall[0]), qy = wrap_index(by, p.ny, p.wall[1]);
+                if (qx < 0 || qy < 0) continue;
+#pragma unroll
+                for (int oz = 0; oz < 4; ++oz) {
+                    const int qz = wrap_index(bz + oz, p.nz, p.wall[2]);
+                    if (qz < 0) continue;
+                    const float wz = weight_o(sz, cz, oz);
+                    const int cell = qx + p.nx * (qy + p.ny * qz);
+                    atomicAdd(g + cell, make_float4(wz * fx, wz * fy, wz * fz, 0.f));
+                    mark_segment(cell, seg_mask, seg_list, seg_count);
+                }
             }
         }
     }
     if (!tiled) return;
     __syncthreads();
+    // flush: one vector RED per non-zero tile cell.  The segments this block is the first to mark are
+    // collected in shared memory and appended to the global list with ONE atomicAdd per block (a
+    // returning atomic per segment on the single list counter was 58 % of this kernel's stall samples).
     const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
     for (int t = tid; t < ncell; t += IB_THREADS) {
         const int x = t % e0, r = t / e0;
@@ -436,9 +460,23 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
             const Cell c = tile_cell(T, t, p);
             const int cell = c.i + p.nx * (c.j + p.ny * c.k);
             atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
-            mark_segment(cell, seg_mask, seg_list, seg_count);
+            const int seg = cell >> SEG_SHIFT;
+            const unsigned bit = 1u << (seg & 31);
+            unsigned* word = seg_mask + (seg >> 5);
+            if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u) {
+                const int slot = atomicAdd(&T.n_need, 1);               // n_need doubles as the block's list length
+                if (slot < SPREAD_SEG_LIST) new_segs[slot] = seg;
+                else seg_list[atomicAdd(seg_count, 1)] = seg;          // list full: append directly
+            }
         }
     }
+    __syncthreads();
+    const int n_new = min(T.n_need, SPREAD_SEG_LIST);
+    if (n_new == 0) return;
+    if (tid == 0) T.mn[0] = atomicAdd(seg_count, n_new);
+    __syncthreads();
+    const int first = T.mn[0];
+    for (int i = tid; i < n_new; i += IB_THREADS) seg_list[first + i] = new_segs[i];
 }
 
 // zero the cells of the segments the previous spread touched (its list), and drop their activity
@@ -503,11 +541,9 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
         unsigned* need = reinterpret_cast<unsigned*>(smem_raw);       // marks alias the (not yet filled) tile
         for (int t = tid; t < ncell; t += IB_THREADS) need[t] = 0u;
         __syncthreads();
-        double x_next = node_coord(X, Y, Z, min(n0 + group, n1 - 1), sub);
         for (int mb = n0; mb < n1; mb += IB_GROUPS) {                  // the 4^3 cells each node needs
             const bool valid = mb + group < n1;
-            const double x = x_next;
-            x_next = node_coord(X, Y, Z, min(mb + IB_GROUPS + group, n1 - 1), sub);
+            const double x = node_coord(X, Y, Z, min(mb + group, n1 - 1), sub);
             const NodeStencil st = node_stencil<false>(x, sub, o0, o1, o2);
             const int tx = st.bx + sub;
             if (!valid || tx < T.lo[0] || tx >= T.hi[0]) continue;
@@ -552,14 +588,10 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
         }
         __syncthreads();
     }
-    // positions one sweep ahead: sweep i + 1 reads nodes that sweep i does not write (a clamped tail
-    // lane may re-read node n1 - 1 after it moved, but such a lane is not valid and its value unused)
-    double x_next = node_coord(X, Y, Z, min(n0 + group, n1 - 1), sub);
     for (int mb = n0; mb < n1; mb += IB_GROUPS) {
         const bool valid = mb + group < n1;
         const int m = valid ? mb + group : n1 - 1;
-        const double x = x_next;
-        x_next = node_coord(X, Y, Z, min(mb + IB_GROUPS + group, n1 - 1), sub);
+        const double x = node_coord(X, Y, Z, m, sub);
         const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
         float ux = 0.f, uy = 0.f, uz = 0.f;
         if (tiled) {
@@ -665,7 +697,7 @@ int launch_clear_spread(Ctx* c, float4* g) {
     return cuda_check(cudaGetLastError(), "clear_spread_kernel");
 }
 
-static size_t spread_smem(int cap) { return (size_t)cap * 12; }
+static size_t spread_smem(int cap) { return (size_t)cap * 12 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)SPREAD_CHUNK * 48; }
 static size_t interp_smem(int cap) { return (size_t)cap * 16 + (((size_t)cap * 2 + 15) & ~(size_t)15); }
 
 // Largest tile (in cells) both kernels can hold with at least one block per SM; a tile cell index
@@ -677,7 +709,7 @@ int ib_max_tile_cap() {
 }
 
 // words per component of the padded spread tile: two blocks of 110 KB per SM
-int ib_max_spread_cap() { return (int)((110 * 1024) / 12); }
+int ib_max_spread_cap() { return (int)((90 * 1024) / 12); }
 
 int launch_spread(Ctx* c, float4* g) {
     if (c->n_nodes == 0) return PLB_OK;

@@ -54,14 +54,10 @@ struct MeshConstraint {
     float k_s, k_t, k_v, pad2;
 };
 
-// Pitches of the spread kernel's shared-memory tile (ib.cu): a row pitch = 4 (mod 8) and a plane
-// pitch = 16 (mod 32) put the 4 x 4 x 2 cells one warp instruction touches (4 consecutive x, 4 rows,
-// 2 planes) into 32 different banks.
+// Pitches of the spread kernel's shared-memory tile (ib.cu): a row pitch = 4 (mod 8) words puts the
+// 4 x 4 cells one node touches per instruction (4 consecutive x in 4 rows) into 16 different banks.
 __host__ __device__ inline int tile_row_pitch(const int e0) { return e0 + ((4 - (e0 & 7)) & 7); }
-__host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e1) {
-    const int v = row_pitch * e1;
-    return v + ((16 - (v & 31)) & 31);
-}
+__host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e1) { return row_pitch * e1; }
 
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 

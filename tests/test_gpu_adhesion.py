@@ -38,13 +38,13 @@ def near_wall_cloud(rng, n, nx, nz, plane=-0.5):
 
 @pytest.mark.parametrize("kind,plane", [((0, 1, 0), -0.5), ((0, 2, 0), 0.0)])
 def test_bond_tables_are_bit_exact_over_many_updates(kind, plane):
-    """3000 nodes jittering near the wall (some across the periodic seams), 20000 receptors, 30
+    """3000 nodes jittering near the wall (some across the periodic seams), 8000 receptors, 30
     updates with the same positions on both sides: break, form, contention for the 4 places"""
     rng = np.random.default_rng(41)
     nx, nz = 24, 20
     xyz = near_wall_cloud(rng, 3000, nx, nz, plane)
     sim, ora = pair(xyz, nx=nx, nz=nz, kind=kind)
-    rec = rng.integers(0, 3000, size=20000)
+    rec = rng.integers(0, 3000, size=8000)
     sim.set_receptors(rec, PRM); ora.set_receptors(rec, PRM)
     total = 0
     for step in range(30):
@@ -56,7 +56,7 @@ def test_bond_tables_are_bit_exact_over_many_updates(kind, plane):
         xyz[:, 1] = np.clip(xyz[:, 1], plane + 0.01, None)
         sim.write_nodes(xyz); ora.write_nodes(xyz)
     on = bo[bo[:, 0] == 1]
-    assert total > 20000 and len(on) > 500                              # plenty of bonds formed and broke
+    assert total > 8000 and len(on) > 300                              # plenty of bonds formed and broke
     _, counts = np.unique((on[:, 1] % nx) + nx * (on[:, 2] % nz), return_counts=True)
     assert counts.max() == 4                                            # rule 2 was binding somewhere
     sim.close(); ora.close()
