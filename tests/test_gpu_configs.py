@@ -160,6 +160,15 @@ def record(name, w, out):
             fh.write(line + "\n")
 
 
+def full_steps(cfg, configured):
+    """PLB_FULL_STEPS="4:250,5:25" caps the full-size runs of those configs (the plain oracle spreads
+    config 5's 21 M nodes serially, about a minute per step); default = the configured length"""
+    for item in os.environ.get("PLB_FULL_STEPS", "").split(","):
+        if ":" in item and int(item.split(":")[0]) == cfg:
+            return min(configured, int(item.split(":")[1]))
+    return configured
+
+
 @pytest.mark.slow
 @pytest.mark.skipif(not FULL, reason="full-length, full-size oracle runs take minutes to an hour of CPU time (PLB_FULL=1)")
 @pytest.mark.parametrize("cfg", [3, 5, 4])
@@ -167,4 +176,5 @@ def test_config_full_length_full_size(cfg):
     """the whole configured run (C3: 2000 steps, C5: 200, C4: 500) at full size against the fp64
     oracle, at the north_star tolerances (C4 needs ~25 GB of host memory for the oracle)"""
     w = wl.config(cfg)
+    w.steps = full_steps(cfg, w.steps)
     record("C%d full" % cfg, w, run_and_compare(w))
