@@ -7,7 +7,11 @@
  *
  * PARITY UNPINNED (conventions fixed in DESIGN.md, not by the paper): which velocity is
  * interpolated (G11, reading A), the wall density rho_w = 1 (G9), dropped stencil cells at a
- * wall (G15), the corner rule for links leaving through two wall faces at once.
+ * wall (G15), the corner rule for links leaving through two wall faces at once, closing the
+ * on-site wall layers at initialisation (G25); for the adhesion model (NEXT-4): break-before-form
+ * order within one update (A-5), lowest-receptor-index-first arbitration of the places of a vWF
+ * site (A-7), nearest-site candidate (A-3), receptors sitting on mesh nodes (A-1); for the flipping
+ * platelet (NEXT-3) the near-wall orbit (the paper's 2.65 % refers to a curve printed as an image).
  */
 #include "orc.h"
 #include <math.h>
