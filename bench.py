@@ -254,6 +254,18 @@ def time_oracle(config, steps, warmup):
             "sample": "%s; %d coupled steps (%d cells, %d nodes) in %.2f s" % (what, steps, w.cells, w.n_nodes, dt)}, dt, w
 
 
+def oracle_single_thread(config, steps=5):
+    """the oracle timed once with ONE thread too (a child process: the OpenMP team
+    size is read when the library loads).  Returns MLUPS or None."""
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, os.path.abspath(__file__), "--impl", "reference", "--config", str(config),
+                              "--steps", str(steps), "--warmup", "1"], env=env, capture_output=True, text=True, timeout=600)
+        return float(json.loads(out.stdout.strip().splitlines()[-1])["value"])
+    except Exception:
+        return None
+
+
 def run_reference(args):
     rank, world, _ = dist_env()
     if rank != 0:
@@ -396,6 +408,7 @@ def run_ours(args):
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cb, _, _ = time_oracle(args.config, 100 if args.config == 4 else 20, 2)
+        cb["value_1_thread"] = oracle_single_thread(args.config)
         line["cpu_baseline"] = cb
     elif rank == 0:
         line["cpu_baseline"] = None

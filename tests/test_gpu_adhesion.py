@@ -109,6 +109,25 @@ def test_bond_and_repulsion_forces_match_oracle():
     sim.close(); ora.close()
 
 
+def test_wall_on_the_z_axis():
+    """wall axis 2: sites on the (x, y) lattice of the low z face"""
+    rng = np.random.default_rng(47)
+    n = 1500
+    xyz = np.stack([-2 + 20 * rng.random(n), -2 + 16 * rng.random(n), -0.5 + 0.02 + 0.8 * rng.random(n)], axis=1)
+    sim, ora = pair(xyz, nx=16, ny=12, nz=8, kind=(0, 0, 1))
+    rec = rng.integers(0, n, size=4000)
+    prm = dict(PRM, wall_axis=2)
+    sim.set_receptors(rec, prm); ora.set_receptors(rec, prm)
+    for step in range(8):
+        sim.adhesion_update(77, step); ora.adhesion_update(77, step)
+        assert (sim.read_bonds() == ora.read_bonds()).all(), step
+    sim.compute_membrane_forces(); ora.compute_membrane_forces()
+    Fg, Fo = sim.read_forces().astype(np.float64), ora.read_forces()
+    assert ora.read_bonds()[:, 0].sum() > 200
+    assert np.abs(Fg - Fo).max() <= 2e-6 * np.abs(Fo).max()
+    sim.close(); ora.close()
+
+
 def test_node_through_the_wall_is_reported():
     sim, ora = pair([[3.0, -0.6, 3.0]])
     sim.set_receptors([0], PRM)

@@ -224,3 +224,29 @@ def test_coupled_platelet_adheres_and_bonds_slow_it_down():
     assert ymin_b > -0.5 and ymin_f > -0.5                         # repulsion keeps the membrane off the wall
     drift_b, drift_f = c_b[0] - w.mesh_xyz[0].mean(axis=0)[0], c_f[0] - free.mesh_xyz[0].mean(axis=0)[0]
     assert 0 <= drift_b < 0.8 * drift_f, (drift_b, drift_f)
+
+
+def test_wall_axis_relabelling_gives_the_same_bonds():
+    """the same receptor cloud over a wall on axis y, and with y and z exchanged over a wall on axis
+    z: identical bond table (tangential axes in x, y, z order: (x, z) becomes (x, y)) and forces
+    with the two components exchanged"""
+    rng = np.random.default_rng(5)
+    p = dict(PRM, F0=1e-4, tau_rep=3.0, k_on0=0.4)
+    n = 400
+    xyz = np.stack([12 * rng.random(n), -0.5 + 0.05 + 0.7 * rng.random(n), 10 * rng.random(n)], axis=1)
+    rec = rng.integers(0, n, size=1500)
+    tables, forces = [], []
+    for axis in (1, 2):
+        pts = xyz if axis == 1 else xyz[:, [0, 2, 1]]
+        dims = dict(nx=12, ny=8, nz=10) if axis == 1 else dict(nx=12, ny=10, nz=8)
+        kind = (0, 1, 0) if axis == 1 else (0, 0, 1)
+        o = cloud(n, pts, kind=kind, **dims)
+        o.set_receptors(rec, dict(p, wall_axis=axis))
+        for step in range(6):
+            o.adhesion_update(seed=9, step=step)
+        o.compute_membrane_forces()
+        tables.append(o.read_bonds()); forces.append(o.read_forces())
+        o.close()
+    assert tables[0][:, 0].sum() > 100
+    assert (tables[0] == tables[1]).all()
+    assert np.allclose(forces[0], forces[1][:, [0, 2, 1]], rtol=1e-13, atol=1e-18)
