@@ -88,3 +88,16 @@ def test_product_does_not_import_oracle():
                 assert "orc.h" not in txt and "liboracle" not in txt, f
     orc_c = open(os.path.join(ROOT, "oracle", "orc.c")).read()
     assert "plb" not in orc_c.replace("PLB", "").lower().replace("paper_1312", "")
+
+
+def test_adhesion_workspace_bytes_host_only(plb):
+    n = plb.ib_adhesion_workspace_bytes(64, 32, 48, 1, 10000)       # wall axis y: 64 x 48 vWF sites
+    sites = 64 * 48
+    assert n >= 10000 * (4 + 16) + sites * (4 + 4 + 32 * 4) and n % 256 == 0
+    assert plb.ib_adhesion_workspace_bytes(64, 32, 48, 2, 0) >= 64 * 32 * (4 + 4 + 32 * 4)
+    with pytest.raises(plb.PlbError) as e:
+        plb.ib_adhesion_workspace_bytes(64, 32, 48, 3, 10)
+    assert e.value.code == plb.PLB_ERR_ARG
+    L = plb.lib()
+    assert L.ib_adhesion_update(None, 0, 0) == plb.PLB_ERR_ARG
+    assert L.ib_set_receptors(None, 0, None, None, None, 0) == plb.PLB_ERR_ARG
