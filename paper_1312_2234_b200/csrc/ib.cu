@@ -542,11 +542,37 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
         // A densely sampled tile (config 5: 2562 nodes on ~2700 cells, every cell inside ~1000
         // stencils) needs all of its cells: skip the marking sweep and take every existing cell.
         const bool dense = 2L * (n1 - n0) >= (long)ncell;
+        const bool by_rows = !dense && e0 <= 32;                       // one 32-bit x-mask per (y, z) tile row
         if (dense) {
             for (int t = tid; t < ncell; t += IB_THREADS) {
                 const int x = t % e0, r = t / e0;
                 const int y = r % e1, z = r / e1;
                 need[t] = (x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]) ? 1u : 0u;
+            }
+        } else if (by_rows) {
+            // lane = oz: the node's four x cells of row (oy, oz) are four adjacent bits of that row's
+            // mask -- 4 marks per lane instead of 16, and most of them only read (the stencils of
+            // a mesh overlap about 13-fold)
+            const int nrow = e1 * T.e[2];
+            for (int t = tid; t < nrow; t += IB_THREADS) need[t] = 0u;
+            __syncthreads();
+            const unsigned below_hi = T.hi[0] >= 32 ? 0xffffffffu : ((1u << T.hi[0]) - 1u);
+            const unsigned below_lo = T.lo[0] >= 32 ? 0xffffffffu : ((1u << T.lo[0]) - 1u);
+            const unsigned exist = below_hi & ~below_lo;                   // x cells of the tile that lie on the lattice
+            for (int mb = n0; mb < n1; mb += IB_GROUPS) {
+                const bool valid = mb + group < n1;
+                const double x = node_coord(X, Y, Z, min(mb + group, n1 - 1), sub);
+                const NodeStencil st = node_stencil<false>(x, sub, o0, o1, o2);
+                const int tz = st.bz + sub;
+                if (!valid || tz < T.lo[2] || tz >= T.hi[2]) continue;
+                const unsigned m4 = (0xFu << st.bx) & exist;
+#pragma unroll
+                for (int oy = 0; oy < 4; ++oy) {
+                    const int ty = st.by + oy;
+                    if (ty < T.lo[1] || ty >= T.hi[1]) continue;
+                    unsigned* row = need + tz * e1 + ty;
+                    if ((*(volatile unsigned*)row & m4) != m4) atomicOr(row, m4);
+                }
             }
         } else {
             for (int t = tid; t < ncell; t += IB_THREADS) need[t] = 0u;
@@ -573,7 +599,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
         // compact the needed cells so that every lane of the moment pass has a cell
         for (int t0 = 0; t0 < ncell; t0 += IB_THREADS) {
             const int t = t0 + tid;
-            const bool want = t < ncell && need[t] != 0u;
+            const bool want = t < ncell && (by_rows ? ((need[t / e0] >> (t % e0)) & 1u) != 0u : need[t] != 0u);
             const unsigned vote = __ballot_sync(0xffffffffu, want);
             int base = 0;
             if ((tid & 31) == 0 && vote) base = atomicAdd(&T.n_need, __popc(vote));
