@@ -1,4 +1,6 @@
-"""Seeded synthetic input generators for the five BASELINE.json configs.
+"""Seeded synthetic input generators for the five BASELINE.json configs and
+for the two workloads of the widened rows: `flipping_platelet` (NEXT-3, section 4.1) and
+`adhering_platelets` (NEXT-4, section 3.2).
 
 This module is INPUT ONLY.  It is the one module the oracle tests and the CUDA path share, and it
 holds none of the method's arithmetic: no lattice-Boltzmann update, no delta kernel, no spring
