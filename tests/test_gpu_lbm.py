@@ -256,6 +256,45 @@ def test_config2_full_size_against_slab_oracle():
     assert amp == pytest.approx(math.exp(-2 * nu * k * k * steps), rel=1e-3)
 
 
+def test_maximum_size_grid_against_slab_oracle():
+    """Largest grid that fits one B200 beside the test's own buffers: 1024 x 512 x 1280 = 671 M cells
+    (ten times config 4; 102 GB of populations, byte offsets far beyond 2^32, cell indices beyond
+    2^29).  Same device as the config-2 full-size test: a field uniform in z, so every z-plane must
+    equal the oracle run on a 4-plane periodic slab of the same field.  Walls in y with a moving top
+    wall, so the bounce-back rows are exercised at this size too."""
+    nx, ny, nz, steps = 1024, 512, 1280, 10
+    free, _ = torch.cuda.mem_get_info()
+    if free < 150e9:
+        pytest.skip("needs ~145 GB of free device memory")
+    kind = (0, 1, 0)
+    u_hi = np.zeros((3, 3)); u_hi[1, 0] = 0.05
+    plane_u = wl.taylor_green_field(nx, ny, 1, 0.02)                     # [3, ny*nx], 2-D vortex in x-y
+    sim = plb.Simulation(nx, ny, nz, 0.6, kind, None, u_hi)
+    u_dev = torch.as_tensor(plane_u, dtype=torch.float32, device=DEV).view(3, 1, ny * nx).expand(3, nz, ny * nx).contiguous()
+    sim.set_equilibrium(None, u_dev.view(-1))
+    del u_dev
+    for _ in range(steps):
+        sim.step(None)
+    sim.status()
+    ora = orc.Oracle(nx, ny, 4, 0.6, kind, None, u_hi)
+    ora.set_equilibrium(None, np.ascontiguousarray(np.broadcast_to(plane_u.reshape(3, 1, ny * nx), (3, 4, ny * nx))).reshape(3, -1))
+    for _ in range(steps):
+        ora.step(None)
+    rho_o, u_o = ora.read_macros()
+    rho_g, u_g = sim.read_macros()
+    rho_g = rho_g.view(nz, -1)
+    u_g = u_g.view(3, nz, -1)
+    plane = nx * ny
+    for kz in (0, 1, nz // 2 + 1, nz - 1):
+        assert np.abs(rho_g[kz].cpu().numpy() - rho_o[:plane]).max() <= 1e-6
+        assert np.abs(u_g[:, kz].cpu().numpy() - u_o[:, :plane]).max() <= 1e-4 * 0.05
+    assert float((rho_g - rho_g[0:1]).abs().max()) == 0.0                 # every plane equals plane 0
+    for d in range(3):
+        assert float((u_g[d] - u_g[d, 0:1]).abs().max()) == 0.0
+    assert abs(float(rho_g.double().sum()) / (nx * ny * nz) - 1.0) <= 1e-9   # mass
+    sim.close(); ora.close()
+
+
 # ------------------------------------------------------------------ edge cases
 def test_degenerate_grids():
     """1-cell-thick periodic axes (a link wraps onto its own cell) and a 1-layer channel."""
