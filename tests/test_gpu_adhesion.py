@@ -152,6 +152,21 @@ def test_call_order_and_arguments():
     sim.close(); ora.close()
 
 
+def test_no_receptors_leaves_only_the_repulsion():
+    """empty receptor list: the update is a no-op, the bond table is empty, every node still feels F_rep"""
+    xyz = np.array([[3.0, 0.1, 3.0], [5.5, 2.0, 4.0]])
+    sim, ora = pair(xyz)
+    none = np.zeros(0, dtype=np.int32)
+    sim.set_receptors(none, PRM); ora.set_receptors(none, PRM)
+    sim.adhesion_update(3, 0); ora.adhesion_update(3, 0)
+    assert sim.read_bonds().shape == (0, 3)
+    sim.compute_membrane_forces(); ora.compute_membrane_forces()
+    Fg, Fo = sim.read_forces().astype(np.float64), ora.read_forces()
+    assert (Fo[:, 1] > 0).all() and np.abs(Fo[:, [0, 2]]).max() == 0.0
+    assert np.abs(Fg - Fo).max() <= 2e-6 * np.abs(Fo).max()
+    sim.close(); ora.close()
+
+
 def test_adhering_platelets_coupled_parity():
     """the NEXT-4 workload (4 platelets flat on the wall, 5344 receptors each, constraints on), 120
     coupled steps with the Monte-Carlo update after every advance: north_star tolerances on the
