@@ -171,9 +171,13 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
 //                 the 19 pulled populations (no velocity field in HBM) -> nodes gather from the tile.
 // A range whose bounding box does not fit the tile (a non-compact "mesh") takes the direct path:
 // global REDs per (node, cell) and on-the-fly cell moments.  Both paths compute the same sums.
-// Within a block FOUR lanes serve one node: lane = ox (the x offset of the stencil column), each
-// lane walks the 4 x 4 (oy, oz) cells of its column; the lanes also share the per-node set-up
-// (lane a < 3 does floor / sincospi of axis a) and finish with a 4-lane shuffle reduction.
+// Lane layouts (each measured against the alternatives on the B200):
+//   interpolate:  FOUR lanes serve one node: lane = ox (the x offset of the stencil column), each
+//                 lane walks the 4 x 4 (oy, oz) cells of its column; the lanes share the per-node
+//                 set-up (lane a < 3 does floor / sincospi of axis a) and finish with a 4-lane
+//                 shuffle reduction;
+//   spread:       SIXTEEN lanes serve one node (lane = (ox, oy), loop over oz) from per-node records
+//                 staged in shared memory (see spread_mesh_kernel).
 // ---------------------------------------------------------------------------------------------
 #ifndef PLB_IB_THREADS
 #define PLB_IB_THREADS 512
@@ -193,7 +197,7 @@ struct MeshTile {
     int interior;        // every tile cell and its 18 neighbours lie inside the grid: no wrap, no wall
     int mn[3], mx[3];    // reduction scratch: min / max of floor(X)
     unsigned fmax_bits;  // reduction scratch: largest |F| component (non-negative float bits)
-    int n_need;          // interpolate: number of tile cells some node needs
+    int n_need;          // interpolate: number of tile cells some node needs; spread: segments newly marked
 };
 
 // set the activity bit of the 8-cell segment of a cell; the thread that sets it first also appends
