@@ -204,6 +204,9 @@ PLB_API int ib_read_node_velocities(plb_ctx* ctx, float* h_U);     /* n x 3 AoS,
 /* populations in the paper's order, true f_i (not the stored f_i - w_i), float[19*cells] SoA */
 PLB_API int lbm_read_populations(plb_ctx* ctx, float* d_f);
 PLB_API int lbm_write_populations(plb_ctx* ctx, const float* d_f);
+/* debug aid: number of cells whose stored populations are not finite or whose density is not
+ * positive (0 = healthy); synchronises the stream */
+PLB_API int lbm_check_finite(plb_ctx* ctx, long* out_bad_cells);
 /* synchronise the stream; returns PLB_ERR_NODE_LEFT / PLB_ERR_CUDA if raised since creation */
 PLB_API int plb_status(plb_ctx* ctx);
 /* number of kernels this context has launched so far (for gpu_launches accounting) */

@@ -48,6 +48,7 @@ SYMBOLS = {
     "ib_n_receptors": (_i, [_vp, C.POINTER(_l)]),
     "ib_read_bonds": (_i, [_vp, _vp]),
     "ib_write_bonds": (_i, [_vp, _vp]),
+    "lbm_check_finite": (_i, [_vp, C.POINTER(_l)]),
     "plb_status": (_i, [_vp]),
     "plb_launch_count": (_i, [_vp, C.POINTER(_l)]),
     "plb_philox4x32_10": (_i, [_vp, _l, _vp, _vp, _vp]),
@@ -279,6 +280,12 @@ def ib_write_bonds(h, bonds):
     _check(lib().ib_write_bonds(h, _np_ptr(b)), "ib_write_bonds")
 
 
+def lbm_check_finite(h) -> int:
+    out = _l(0)
+    _check(lib().lbm_check_finite(h, C.byref(out)), "lbm_check_finite")
+    return out.value
+
+
 def plb_status(h):
     _check(lib().plb_status(h), "plb_status")
 
@@ -352,6 +359,9 @@ class Simulation:
         u = self.torch.empty(3 * self.cells, dtype=self.torch.float32, device=self.device)
         lbm_read_macros(self.h, rho, u)
         return rho, u.view(3, self.cells)
+
+    def check_finite(self) -> int:
+        return lbm_check_finite(self.h)
 
     def read_populations(self):
         f = self.torch.empty(19 * self.cells, dtype=self.torch.float32, device=self.device)

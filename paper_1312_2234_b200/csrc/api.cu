@@ -785,6 +785,22 @@ int ib_write_forces(plb_ctx* ctx, const float* h_F) {
     return rc;
 }
 
+int lbm_check_finite(plb_ctx* ctx, long* out_bad_cells) {
+    REQUIRE_CTX(ctx);
+    if (!out_bad_cells || !ctx->populated) {
+        set_error("lbm_check_finite: null output or populations not set");
+        return out_bad_cells ? PLB_ERR_ORDER : PLB_ERR_ARG;
+    }
+    int* d_bad = ctx->counters + 8;                    // scratch counter
+    int rc = cuda_check(cudaMemsetAsync(d_bad, 0, sizeof(int), ctx->stream), "clear counter");
+    if (!rc) rc = launch_check_finite(ctx, d_bad);
+    int h = 0;
+    if (!rc) rc = cuda_check(cudaMemcpyAsync(&h, d_bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream), "read counter");
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    *out_bad_cells = h;
+    return rc;
+}
+
 int plb_status(plb_ctx* ctx) {
     REQUIRE_CTX(ctx);
     return sync_status(ctx);

@@ -364,6 +364,18 @@ __global__ void __launch_bounds__(256) read_populations_kernel(const float* __re
     for (int d = 0; d < Q; ++d) f[(size_t)d * p.cells + idx] = h[d][0] + WGT(d);
 }
 
+// debug aid: count the cells whose stored populations are not finite or whose
+// density 1 + sum_d h_d is not positive
+__global__ void __launch_bounds__(256) check_finite_kernel(const float* __restrict__ src, int* __restrict__ bad,
+                                                           const LbmParams p) {
+    const int idx = blockIdx.x * 256 + threadIdx.x;
+    if (idx >= p.cells) return;
+    float sum = 0.f;
+#pragma unroll
+    for (int d = 0; d < Q; ++d) sum += __ldg(src + (size_t)d * p.cells + idx);
+    if (!isfinite(sum) || !(1.0f + sum > 0.f)) atomicAdd(bad, 1);
+}
+
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
@@ -413,6 +425,12 @@ int launch_read_macros(Ctx* c, float* d_rho, float* d_u) {
         macros_kernel<FORCE_SPARSE><<<grid, 256, 0, c->stream>>>(src, c->g_last, c->seg_mask, d_rho, d_u, c->prm);
     c->launches++;
     return cuda_check(cudaGetLastError(), "macros_kernel");
+}
+
+int launch_check_finite(Ctx* c, int* d_bad) {
+    check_finite_kernel<<<grid_cells(c), 256, 0, c->stream>>>(c->f[c->cur], d_bad, c->prm);
+    c->launches++;
+    return cuda_check(cudaGetLastError(), "check_finite_kernel");
 }
 
 int launch_read_populations(Ctx* c, float* d_f) {

@@ -295,6 +295,25 @@ def test_maximum_size_grid_against_slab_oracle():
     sim.close(); ora.close()
 
 
+def test_check_finite_counts_broken_cells():
+    """debug aid: 0 on a healthy state, the number of poisoned cells otherwise"""
+    sim = plb.Simulation(16, 12, 10, 0.7, (0, 1, 0))
+    with pytest.raises(plb.PlbError) as e:
+        sim.check_finite()                                   # populations not set yet
+    assert e.value.code == plb.PLB_ERR_ORDER
+    sim.set_equilibrium()
+    for _ in range(3):
+        sim.step(None)
+    assert sim.check_finite() == 0
+    f = sim.read_populations().clone()
+    f[5, 100] = float("nan")
+    f[:, 777] = -1.0                                        # density far below zero
+    f[2, 1500] = float("inf")
+    sim.write_populations(f)
+    assert sim.check_finite() == 3
+    sim.close()
+
+
 # ------------------------------------------------------------------ edge cases
 def test_degenerate_grids():
     """1-cell-thick periodic axes (a link wraps onto its own cell) and a 1-layer channel."""
