@@ -305,12 +305,18 @@ def test_check_finite_counts_broken_cells():
     for _ in range(3):
         sim.step(None)
     assert sim.check_finite() == 0
-    f = sim.read_populations().clone()
-    f[5, 100] = float("nan")
-    f[:, 777] = -1.0                                        # density far below zero
-    f[2, 1500] = float("inf")
+    clean = sim.read_populations().clone()
+    for d, q, value in ((5, 100, float("nan")), (2, 1500, float("inf"))):
+        f = clean.clone()
+        f[d, q] = value                                     # one stored slot -> exactly one cell
+        sim.write_populations(f)
+        assert sim.check_finite() == 1
+    f = clean.clone()
+    f[:, 16 * 12 * 5 + 16 * 6 + 8] = -1.0                   # an interior cell: its 19 values stream to 19 cells
     sim.write_populations(f)
-    assert sim.check_finite() == 3
+    assert sim.check_finite() == 19
+    sim.write_populations(clean)
+    assert sim.check_finite() == 0
     sim.close()
 
 
