@@ -58,9 +58,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     int4* tris = w.take<int4>((size_t)2 * max_nodes);
     float* tri_S0 = w.take<float>((size_t)2 * max_nodes);
     MeshConstraint* cons = w.take<MeshConstraint>((size_t)max_nodes / 4 + 1);
-    int4* mesh_info = w.take<int4>((size_t)max_nodes / 4 + 1);
     if (c) {
-        c->mesh_info = mesh_info; c->cap_meshes = max_nodes / 4 + 1;
         c->tris = tris; c->tri_S0 = tri_S0; c->cons = cons;
         c->cap_tris = 2 * max_nodes; c->cap_cons = max_nodes / 4 + 1;
         c->f[0] = f0; c->f[1] = f1;
@@ -218,7 +216,6 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->n_ranges = 0;
     c->n_tris = 0; c->n_cons = 0;
     c->adh_on = false; c->n_rec = 0;
-    c->mesh_kernel_ok = true; c->mesh_nodes_max = 0;
     c->list_parity = 0;
     c->tile_cap = 512;
     c->spread_cap = 1024;
@@ -414,23 +411,8 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
     }
     ctx->tile_cap = cap;
     ctx->spread_cap = scap;
-    // one thread block of mesh_force_kernel per mesh, as long as the table and the shared memory hold them
-    const long have = (long)ctx->mesh_node_off.size() - 1;
-    std::vector<int4> info;
-    if (ctx->mesh_kernel_ok && have + n_meshes <= ctx->cap_meshes && n_nodes <= ib_mesh_force_max_nodes() &&
-        ctx->n_edges + add_edges < (1L << 31)) {
-        for (int s = 0; s < n_meshes; ++s)
-            info.push_back(make_int4((int)(ctx->n_nodes + (long)s * n_nodes), n_nodes,
-                                     (int)(ctx->n_edges + (long)s * n_edges), n_edges));
-        if (n_nodes > ctx->mesh_nodes_max) ctx->mesh_nodes_max = n_nodes;
-    } else {
-        ctx->mesh_kernel_ok = false;
-    }
     int rc = cuda_check(cudaMemcpyAsync(ctx->ranges + ctx->n_ranges, rg.data(), rg.size() * sizeof(int2),
                                         cudaMemcpyHostToDevice, ctx->stream), "upload node ranges");
-    if (!rc && !info.empty())
-        rc = cuda_check(cudaMemcpyAsync(ctx->mesh_info + have, info.data(), info.size() * sizeof(int4),
-                                        cudaMemcpyHostToDevice, ctx->stream), "upload mesh table");
     for (int d = 0; d < 3 && !rc; ++d)
         rc = cuda_check(cudaMemcpyAsync(ctx->X[d] + ctx->n_nodes, soa.data() + (size_t)d * add_nodes,
                                         (size_t)add_nodes * sizeof(double), cudaMemcpyHostToDevice, ctx->stream),

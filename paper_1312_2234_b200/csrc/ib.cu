@@ -55,64 +55,6 @@ __global__ void __launch_bounds__(256) edge_force_kernel(const double* __restric
     atomicAdd(F + ab.y, make_float4(-ex, -ey, -ez, 0.f));
 }
 
-// S1, one thread block per mesh (used when every mesh fits): the mesh's positions are loaded once
-// into shared memory (fp64), its edges are streamed once, the nodal forces accumulate in shared
-// memory and leave with one coalesced store per node -- instead of six gathered fp64 loads and two
-// global vector atomics per edge.  The force noise of force_init_kernel is the accumulator's start.
-constexpr int MESH_FORCE_THREADS = 256;
-constexpr int MESH_FORCE_MAX_NODES = 4096;        // 36 B of shared memory per node
-
-__global__ void __launch_bounds__(MESH_FORCE_THREADS) mesh_force_kernel(
-    const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
-    const int2* __restrict__ edges, const float2* __restrict__ prm, float4* __restrict__ F,
-    const int4* __restrict__ mesh_info, int* __restrict__ counters, const int cap, const float sigma,
-    const unsigned long long seed, const unsigned step) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* sx = reinterpret_cast<double*>(smem_raw);
-    double* sy = sx + cap;
-    double* sz = sy + cap;
-    float* fx = reinterpret_cast<float*>(sz + cap);
-    float* fy = fx + cap;
-    float* fz = fy + cap;
-    const int4 info = __ldg(mesh_info + blockIdx.x);
-    const int n0 = info.x, n = info.y, e0 = info.z, ne = info.w;
-    for (int i = threadIdx.x; i < n; i += MESH_FORCE_THREADS) {
-        sx[i] = X[n0 + i]; sy[i] = Y[n0 + i]; sz[i] = Z[n0 + i];
-        float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (sigma > 0.f) {                               // as force_init_kernel
-            const uint4 r = noise_words(seed, (unsigned long long)(n0 + i), step, 2u);
-            const float r0 = sqrtf(-2.0f * logf(uniform01(r.x)));
-            const float r2 = sqrtf(-2.0f * logf(uniform01(r.z)));
-            float s1, c1;
-            sincospif(2.0f * uniform01(r.y), &s1, &c1);
-            f.x = sigma * r0 * c1;
-            f.y = sigma * r0 * s1;
-            f.z = sigma * r2 * cospif(2.0f * uniform01(r.w));
-        }
-        fx[i] = f.x; fy[i] = f.y; fz[i] = f.z;
-    }
-    __syncthreads();
-    for (int e = threadIdx.x; e < ne; e += MESH_FORCE_THREADS) {
-        const int2 ab = __ldg(edges + e0 + e);
-        const float2 Lk = __ldg(prm + e0 + e);
-        const int a = ab.x - n0, b = ab.y - n0;
-        const double rx = sx[b] - sx[a], ry = sy[b] - sy[a], rz = sz[b] - sz[a];
-        const double l = sqrt(rx * rx + ry * ry + rz * rz);
-        if (!(l > 0.0)) {
-            atomicOr(counters + 1, STATUS_ZERO_EDGE);
-            continue;
-        }
-        const float s = Lk.y * (float)((l - (double)Lk.x) / l);
-        const float ex = s * (float)rx, ey = s * (float)ry, ez = s * (float)rz;
-        atomicAdd(fx + a, ex); atomicAdd(fy + a, ey); atomicAdd(fz + a, ez);
-        atomicAdd(fx + b, -ex); atomicAdd(fy + b, -ey); atomicAdd(fz + b, -ez);
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < n; i += MESH_FORCE_THREADS) F[n0 + i] = make_float4(fx[i], fy[i], fz[i], 0.f);
-}
-
-int ib_mesh_force_max_nodes() { return MESH_FORCE_MAX_NODES; }
-
 // ---------------------------------------------------------------------------------------------
 // S1b: area and volume constraint forces, Eq. 4-5 (L101-108):
 //   H = k_s (S_tot - S0_tot)^2/(2 S0_tot) + sum_tri k_t (S - S_0)^2/(2 S_0) + k_v (V - V_0)^2/(2 V_0)
@@ -766,25 +708,13 @@ __global__ void philox_kernel(const long n, const uint4* __restrict__ ctr, const
 // ---------------------------------------------------------------------------------------------
 int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigned long long step) {
     if (c->n_nodes == 0) return PLB_OK;
-    const long n_meshes = (long)c->mesh_node_off.size() - 1;
-    if (c->mesh_kernel_ok && c->n_edges > 0 && n_meshes > 0) {
-        const int cap = c->mesh_nodes_max;
-        const size_t smem = (size_t)cap * 36;
-        int rc = cuda_check(cudaFuncSetAttribute(mesh_force_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
-                            "cudaFuncSetAttribute(mesh_force_kernel)");
-        if (rc) return rc;
-        mesh_force_kernel<<<(unsigned)n_meshes, MESH_FORCE_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->edges, c->edge_prm, c->F, c->mesh_info, c->counters, cap, sigma, seed, (unsigned)step);
+    force_init_kernel<<<(unsigned)((c->n_nodes + 255) / 256), 256, 0, c->stream>>>(c->F, c->n_nodes, sigma, seed,
+                                                                                  (unsigned)step);
+    c->launches++;
+    if (c->n_edges) {
+        edge_force_kernel<<<(unsigned)((c->n_edges + 255) / 256), 256, 0, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->edges, c->edge_prm, c->F, c->n_edges, c->counters);
         c->launches++;
-    } else {
-        force_init_kernel<<<(unsigned)((c->n_nodes + 255) / 256), 256, 0, c->stream>>>(c->F, c->n_nodes, sigma, seed,
-                                                                                      (unsigned)step);
-        c->launches++;
-        if (c->n_edges) {
-            edge_force_kernel<<<(unsigned)((c->n_edges + 255) / 256), 256, 0, c->stream>>>(
-                c->X[0], c->X[1], c->X[2], c->edges, c->edge_prm, c->F, c->n_edges, c->counters);
-            c->launches++;
-        }
     }
     if (c->n_cons) {
         constraint_force_kernel<<<(unsigned)c->n_cons, CON_THREADS, 0, c->stream>>>(

@@ -135,10 +135,6 @@ struct Ctx {
     MeshConstraint* cons;      // one entry per constrained mesh = one thread block of the kernel
     long cap_cons, n_cons;
     std::vector<char> mesh_constrained;
-    int4* mesh_info;           // per mesh (first node, nodes, first edge, edges): one block of mesh_force_kernel
-    long cap_meshes;           // capacity of mesh_info
-    bool mesh_kernel_ok;       // every mesh is listed in mesh_info and fits the kernel's shared memory
-    int mesh_nodes_max;        // largest mesh (nodes)
     int2* ranges;              // node ranges [first, last) served by one thread block of the IB kernels
     long n_ranges;
     int tile_cap;              // cells of the shared-memory lattice tile of the interpolation kernel
@@ -180,7 +176,6 @@ int launch_clear_spread(Ctx* c, float4* g);
 int launch_spread(Ctx* c, float4* g);
 int launch_interpolate_advance(Ctx* c);
 int ib_max_tile_cap();
-int ib_mesh_force_max_nodes();
 int ib_max_spread_cap();
 int launch_nodes_transpose(Ctx* c, bool to_aos);
 int launch_adhesion_forces(Ctx* c);
