@@ -1,7 +1,11 @@
 /* oracle/orc.c -- CPU ORACLE, TEST INFRASTRUCTURE ONLY (see orc.h).
  *
  * Plain nested loops over cells, nodes and edges, in the paper's order and notation; fp64 by
- * default.  No blocking, fusion or layout tricks; OpenMP over z-planes / nodes only.
+ * default.  No blocking, fusion or layout tricks.  OpenMP over z-planes (cells), nodes and meshes
+ * only ("It may use OpenMP over z-planes and over meshes; nothing else"): every
+ * parallel loop runs the same per-cell / per-node / per-mesh body as the serial one; the spread adds
+ * into the shared force field with `omp atomic`, so its sums are reordered at the 1e-16 level (any
+ * summation order is correct there).
  * Every function cites the passage of /root/reference/PAPER.md it follows ("L" = line number)
  * or the SURVEY.md section 8(c) reading ("O-n", "G-n") taken where the paper is silent/garbled.
  *
@@ -65,6 +69,7 @@ struct orc_ctx {
     real *rest, *kspring;              /* per edge */
     /* NEXT-2 (Eq. 4-5): triangles of the lipid-bilayer surface, per mesh */
     int *mesh_off;                     /* first global node of mesh s (n_meshes + 1 entries) */
+    int *mesh_edge_off;                /* first global edge of mesh s (n_meshes + 1 entries) */
     int n_tris, cap_tris;
     int *tri;                          /* global node index triples, outward orientation */
     int *tri_mesh;                     /* mesh of each triangle */
@@ -180,7 +185,7 @@ int orc_destroy(orc_ctx* c) {
     if (!c) return -1;
     free(c->f); free(c->fstar); free(c->g_last);
     free(c->X); free(c->F); free(c->U); free(c->edge); free(c->rest); free(c->kspring);
-    free(c->mesh_off); free(c->tri); free(c->tri_mesh); free(c->tri_S0);
+    free(c->mesh_off); free(c->mesh_edge_off); free(c->tri); free(c->tri_mesh); free(c->tri_S0);
     free(c->S0_tot); free(c->V0); free(c->k_s); free(c->k_t); free(c->k_v);
     free(c->rec_node); free(c->bond); free(c->site_count);
     free(c);
@@ -194,6 +199,7 @@ static void hecht_harting_faces(orc_ctx* c);   /* NEXT-1, below */
 int orc_set_equilibrium(orc_ctx* c, const double* rho, const double* u, double amp, uint64_t seed) {
     if (!c) return -1;
     const long N = c->cells;
+#pragma omp parallel for schedule(static)
     for (long q = 0; q < N; ++q) {
         real r = rho ? (real)rho[q] : (real)1;
         real v[3] = {u ? (real)u[q] : 0, u ? (real)u[N + q] : 0, u ? (real)u[2 * N + q] : 0};
@@ -353,6 +359,7 @@ int orc_step(orc_ctx* c, const double* g) {
 int orc_read_macros(orc_ctx* c, double* rho, double* u) {
     if (!c) return -1;
     const long N = c->cells;
+#pragma omp parallel for schedule(static)
     for (long q = 0; q < N; ++q) {
         real r = 0, j[3] = {0, 0, 0};
         for (int i = 0; i < Q; ++i) {
@@ -369,14 +376,16 @@ int orc_read_macros(orc_ctx* c, double* rho, double* u) {
 
 int orc_read_populations(orc_ctx* c, double* f) {
     if (!c || !f) return -1;
-    for (int i = 0; i < Q; ++i)
-        for (long q = 0; q < c->cells; ++q) f[(size_t)i * c->cells + q] = (double)c->f[FI(i, q)];
+#pragma omp parallel for schedule(static)
+    for (long q = 0; q < c->cells; ++q)
+        for (int i = 0; i < Q; ++i) f[(size_t)i * c->cells + q] = (double)c->f[FI(i, q)];
     return 0;
 }
 int orc_write_populations(orc_ctx* c, const double* f) {
     if (!c || !f) return -1;
-    for (int i = 0; i < Q; ++i)
-        for (long q = 0; q < c->cells; ++q) c->f[FI(i, q)] = (real)f[(size_t)i * c->cells + q];
+#pragma omp parallel for schedule(static)
+    for (long q = 0; q < c->cells; ++q)
+        for (int i = 0; i < Q; ++i) c->f[FI(i, q)] = (real)f[(size_t)i * c->cells + q];
     hecht_harting_faces(c);
     return 0;
 }
@@ -426,6 +435,9 @@ int orc_add_mesh(orc_ctx* c, int n_nodes, const double* xyz, int n_edges, const 
     c->mesh_off = (int*)realloc(c->mesh_off, (size_t)(c->n_meshes + 1) * sizeof(int));
     c->mesh_off[c->n_meshes - 1] = off;
     c->mesh_off[c->n_meshes] = c->n_nodes;
+    c->mesh_edge_off = (int*)realloc(c->mesh_edge_off, (size_t)(c->n_meshes + 1) * sizeof(int));
+    c->mesh_edge_off[c->n_meshes - 1] = c->n_edges - n_edges;
+    c->mesh_edge_off[c->n_meshes] = c->n_edges;
     c->S0_tot = (real*)realloc(c->S0_tot, (size_t)c->n_meshes * sizeof(real));
     c->V0 = (real*)realloc(c->V0, (size_t)c->n_meshes * sizeof(real));
     c->k_s = (real*)realloc(c->k_s, (size_t)c->n_meshes * sizeof(real));
@@ -578,25 +590,35 @@ static int adhesion_forces(orc_ctx* c);   /* NEXT-4, below */
 int orc_compute_membrane_forces(orc_ctx* c, double sigma, uint64_t seed, uint64_t step) {
     if (!c) return -1;
     for (int m = 0; m < 3 * c->n_nodes; ++m) c->F[m] = 0;
-    for (int e = 0; e < c->n_edges; ++e) {
-        const int a = c->edge[2 * e], b = c->edge[2 * e + 1];
-        real R[3], l2 = 0;
-        for (int d = 0; d < 3; ++d) {
-            R[d] = c->X[3 * b + d] - c->X[3 * a + d];
-            l2 += R[d] * R[d];
+    /* the edges of a mesh touch only that mesh's nodes: meshes are independent, and inside a mesh
+     * the edges are visited in their given order */
+    int zero_edge = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(| : zero_edge)
+    for (int s = 0; s < c->n_meshes; ++s)
+        for (int e = c->mesh_edge_off[s]; e < c->mesh_edge_off[s + 1]; ++e) {
+            const int a = c->edge[2 * e], b = c->edge[2 * e + 1];
+            real R[3], l2 = 0;
+            for (int d = 0; d < 3; ++d) {
+                R[d] = c->X[3 * b + d] - c->X[3 * a + d];
+                l2 += R[d] * R[d];
+            }
+            const real l = (real)sqrt((double)l2);
+            if (!(l > 0)) {
+                zero_edge = 1;
+                continue;
+            }
+            for (int d = 0; d < 3; ++d) {
+                const real ed = c->kspring[e] * (l - c->rest[e]) * R[d] / l;
+                c->F[3 * a + d] += ed;
+                c->F[3 * b + d] -= ed;
+            }
         }
-        const real l = (real)sqrt((double)l2);
-        if (!(l > 0)) return -1;
-        for (int d = 0; d < 3; ++d) {
-            const real ed = c->kspring[e] * (l - c->rest[e]) * R[d] / l;
-            c->F[3 * a + d] += ed;
-            c->F[3 * b + d] -= ed;
-        }
-    }
+    if (zero_edge) return -1;
     area_volume_forces(c);
     int rc = adhesion_forces(c);
     if (rc) return rc;
     if (sigma > 0)
+#pragma omp parallel for schedule(static)
         for (int m = 0; m < c->n_nodes; ++m) {
             double z[3];
             orc_noise_normal3(seed, (uint64_t)m, (uint32_t)step, 2u, z);
@@ -650,18 +672,28 @@ int orc_spread(orc_ctx* c, double* g) {
     if (!c || !g) return -1;
     if (c->n_nodes && !c->forces_valid) return -4;
     const long N = c->cells;
-    real* acc = (real*)calloc((size_t)3 * N, sizeof(real));
-    for (int m = 0; m < c->n_nodes; ++m)
-        for (int oz = 0; oz < 4; ++oz)
-            for (int oy = 0; oy < 4; ++oy)
-                for (int ox = 0; ox < 4; ++ox) {
-                    const int o[3] = {ox, oy, oz};
-                    real W;
-                    const long q = stencil_cell(c, &c->X[3 * m], o, &W);
-                    if (q < 0) continue;
-                    for (int d = 0; d < 3; ++d) acc[(size_t)d * N + q] += W * c->F[3 * m + d];
-                }
-    for (size_t s = 0; s < (size_t)3 * N; ++s) g[s] = (double)acc[s];
+    real* acc = (real*)malloc((size_t)3 * N * sizeof(real));
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < 3 * N; ++s) acc[s] = 0;
+    /* mesh by mesh; the stencils of different meshes may share cells, hence the atomic add */
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int s = 0; s < c->n_meshes; ++s)
+        for (int m = c->mesh_off[s]; m < c->mesh_off[s + 1]; ++m)
+            for (int oz = 0; oz < 4; ++oz)
+                for (int oy = 0; oy < 4; ++oy)
+                    for (int ox = 0; ox < 4; ++ox) {
+                        const int o[3] = {ox, oy, oz};
+                        real W;
+                        const long q = stencil_cell(c, &c->X[3 * m], o, &W);
+                        if (q < 0) continue;
+                        for (int d = 0; d < 3; ++d) {
+                            const real add = W * c->F[3 * m + d];
+#pragma omp atomic
+                            acc[(size_t)d * N + q] += add;
+                        }
+                    }
+#pragma omp parallel for schedule(static)
+    for (long s = 0; s < 3 * N; ++s) g[s] = (double)acc[s];
     free(acc);
     return 0;
 }
@@ -705,6 +737,7 @@ int orc_interpolate_advance(orc_ctx* c) {
     if (!c) return -1;
     const long N = c->cells;
     real* v = (real*)malloc((size_t)3 * N * sizeof(real));
+#pragma omp parallel for schedule(static)
     for (long q = 0; q < N; ++q) {
         real r = 0, j[3] = {0, 0, 0};
         for (int i = 0; i < Q; ++i) {
@@ -717,6 +750,7 @@ int orc_interpolate_advance(orc_ctx* c) {
     interpolate(c, v, c->U);
     free(v);
     int left = 0;
+#pragma omp parallel for schedule(static) reduction(| : left)
     for (int m = 0; m < c->n_nodes; ++m)
         for (int d = 0; d < 3; ++d) {
             c->X[3 * m + d] += c->U[3 * m + d];
