@@ -254,9 +254,9 @@ def time_oracle(config, steps, warmup):
             "sample": "%s; %d coupled steps (%d cells, %d nodes) in %.2f s" % (what, steps, w.cells, w.n_nodes, dt)}, dt, w
 
 
-def oracle_single_thread(config, steps=5):
-    """the oracle timed once with ONE thread too (a child process: the OpenMP team
-    size is read when the library loads).  Returns MLUPS or None."""
+def oracle_single_thread(config, steps=10):
+    """the oracle timed once with ONE thread too, on >= 10 steps (a child process:
+    the OpenMP team size is read when the library loads).  Returns MLUPS or None."""
     env = dict(os.environ, OMP_NUM_THREADS="1")
     try:
         out = subprocess.run([sys.executable, os.path.abspath(__file__), "--impl", "reference", "--config", str(config),
@@ -353,10 +353,19 @@ def run_ours(args):
             plb.lbm_step(sim.h, None)
             if marks is not None: marks[3].record()
 
+    def reset():
+        """back to the initial state (SURVEY.md 8(d) protocol: warm-up, reset, then time)"""
+        u = None if w.u0 is None else torch.as_tensor(w.u0, dtype=torch.float32).to(device).contiguous()
+        sim.set_equilibrium(None, u, w.noise_amp, w.noise_seed)
+        if coupled:
+            sim.write_nodes(np.ascontiguousarray(w.mesh_xyz.reshape(-1, 3)))
+        torch.cuda.synchronize(device)
+
     # ---- device-resident leg: inputs already in HBM, CUDA events on the launching stream
     clocks = ClockSampler(device.index)
     for s in range(W):
         one_step(s)
+    reset()
     marks = [[ev() for _ in range(5)] for _ in range(K)]
     t_beg, t_end = ev(), ev()
     barrier(device)
@@ -369,7 +378,23 @@ def run_ours(args):
     barrier(device)
     clk = clocks.stop()
     launches = sim.launch_count() - launches0
-    sim.status()
+    # ---- the state the timed run produced: sticky error flags, non-finite / non-positive cells,
+    # mass (P1: halfway bounce-back and the Guo force conserve it exactly), nodes inside the channel
+    state = {"status": "ok", "steps_from_initial_state": K}
+    try:
+        sim.status()
+    except plb.PlbError as err:
+        state["status"] = "error %d: %s" % (err.code, err)
+    state["bad_cells"] = int(sim.check_finite())
+    rho_end, u_end = sim.read_macros()
+    state["mean_rho_minus_1"] = float(rho_end.double().mean().item() - 1.0)
+    state["max_speed"] = float(u_end.abs().max().item())
+    if coupled:
+        X_end = sim.read_nodes()
+        state["nodes_finite"] = bool(np.isfinite(X_end).all())
+        state["max_node_displacement"] = float(np.abs(X_end - w.mesh_xyz.reshape(-1, 3)).max())
+        state["spread_form"] = {0: "auto", 1: "scatter", 2: "aggregate", 3: "gather"}[sim.spread_mode()]
+    del rho_end, u_end
     seconds = max_over_ranks(t_beg.elapsed_time(t_end) * 1e-3, device)
     value = aggregate(w.cells, K, world, seconds)
     lbm_ms = sum(m[2].elapsed_time(m[3]) for m in marks) / K
@@ -390,7 +415,10 @@ def run_ours(args):
     peak, peak_src = hbm_peak()
     achieved = BYTES_PER_CELL * w.cells / (lbm_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "lbm_step_vec_kernel<MODE,4,128,4> (lbm_step)", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(args.config), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": ncu_traffic(args.config),
+                "traffic_source": "static: profiles/lbm_dram_traffic.txt (one ncu --set full capture of this kernel; "
+                                  "not measured in this run)",
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": BYTES_PER_CELL * w.cells, "avg_launch_ms": lbm_ms,
                 "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                 "lbm_only_mlups": w.cells / (lbm_ms * 1e-3) / 1e6}
@@ -403,7 +431,7 @@ def run_ours(args):
                    "l2": "inputs exceed L2 (%.2f GB of populations per step)" % (BYTES_PER_CELL * w.cells / 1e9),
                    "multi_gpu": "replicas only (no exchange step in this build)", "notes": w.notes},
         "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-        "coupled_steps_per_s": K * world / seconds, "split_ms": split, "ib_share": ib_share,
+        "coupled_steps_per_s": K * world / seconds, "split_ms": split, "ib_share": ib_share, "state_check": state,
         "step_ms_rank0": step_ms,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -74,7 +74,7 @@ enum {
 PLB_API const char* plb_last_error(void);
 
 /* Bytes of workspace lbm_create needs for this grid and mesh capacity (two fp32 lattices, the
- * sparse velocity field, segment bookkeeping, node and edge arrays). */
+ * activity-segment mask and list, node, edge and triangle arrays). */
 PLB_API int lbm_workspace_bytes(const plb_grid* grid, long max_nodes, long max_edges, size_t* out_bytes);
 
 /* Create a context.  tau > 1/2 is the BGK relaxation time (Eq. 16).  d_workspace must stay
@@ -94,8 +94,9 @@ PLB_API int lbm_set_equilibrium(plb_ctx* ctx, const float* d_rho, const float* d
 /* One fused collide + stream + boundary step (Eq. 16-21 with the Guo forcing of Eq. 19, periodic
  * wrap L217, bounce-back as above).  d_forcing: float4 per cell, or NULL = no force.  When
  * d_forcing is the buffer ib_spread last filled, only the cells that spread touched are read.
- * The buffer must stay unmodified until ib_interpolate_advance / lbm_read_macros have consumed
- * it (they add g/2 to the momentum, L201). */
+ * LIFETIME: the library keeps the pointer.  The buffer must stay allocated and unmodified until
+ * the next lbm_step, lbm_set_equilibrium, lbm_write_populations or lbm_destroy, because
+ * ib_interpolate_advance and lbm_read_macros read it (they add g/2 to the momentum, L201). */
 PLB_API int lbm_step(plb_ctx* ctx, const float* d_forcing);
 
 /* rho = sum f_i (Eq. 17), v = (sum c_i f_i + g_last/2)/rho (Eq. 18) of the current state.
@@ -105,7 +106,10 @@ PLB_API int lbm_read_macros(plb_ctx* ctx, float* d_rho, float* d_u);
 /* Add one mesh (nodes = actin vertices, edges = filaments).  h_xyz: n_nodes x 3
  * doubles (AoS, unwrapped lattice coordinates); h_edges: n_edges x 2 mesh-local node indices;
  * h_rest: n_edges rest lengths L_ij (NULL = the lengths of h_xyz); k: spring stiffness of Eq. 2.
- * Meshes are concatenated; global node index = running offset + local index. */
+ * Meshes are concatenated; global node index = running offset + local index.  (Inside the
+ * library the nodes of a mesh are stored in a different, spatially coherent order; every call
+ * that names a node -- ib_read/write_*, ib_set_triangles, ib_set_receptors, the noise key --
+ * speaks the caller's indices.) */
 PLB_API int ib_add_mesh(plb_ctx* ctx, int n_nodes, const double* h_xyz, int n_edges, const int* h_edges,
                 const float* h_rest, float k, int* out_mesh_id);
 /* n_meshes meshes of identical topology and rest lengths: h_xyz is n_meshes x n_nodes x 3. */
@@ -136,12 +140,34 @@ PLB_API int ib_compute_membrane_forces(plb_ctx* ctx, float noise_sigma, unsigned
  * 4-point cosine kernel phi(r) = (1 + cos(pi r/2))/4, |r| < 2, over the 4x4x4 cells
  * floor(X) - 1 .. floor(X) + 2; periodic axes wrap the index, cells beyond a wall axis are
  * dropped.  d_forcing (float4 per cell) must have been zero-filled once by the caller; each call
- * first clears what the previous call on the same buffer wrote. */
+ * first clears what the previous call wrote.  LIFETIME: the library keeps the pointer and the
+ * next ib_spread WRITES zeros into the previous call's buffer, whichever buffer it is given: a
+ * buffer handed to ib_spread must stay allocated until the second next ib_spread,
+ * ib_release_forcing or lbm_destroy. */
 PLB_API int ib_spread(plb_ctx* ctx, float* d_forcing);
+
+/* The three forms of the S2 kernel (all compute the sum of Eq. 34; they differ in how the
+ * contributions of the nodes of one thread block meet in its shared-memory lattice tile):
+ *   SCATTER   one shared-memory atomic per (node, cell, component);
+ *   AGGREGATE nodes counting-sorted by base cell, one warp per occupied base cell sums its nodes in
+ *             registers: one shared-memory atomic per (base cell, cell, component);
+ *   GATHER    same sort, one thread per tile cell sums over the 4 x 4 x 4 base cells around it: no
+ *             atomics (the form of the paper's own fluid3d_force_distribute_kernel, L356-362).
+ * AUTO (default) picks SCATTER or AGGREGATE from the sampling density of the tiles.
+ * ib_get_spread_mode returns the form ib_spread would launch now. */
+/* Forget the forcing buffers the context still points to (the one ib_spread last filled, the one
+ * lbm_step last read), clearing what ib_spread wrote first; the caller may free them afterwards.
+ * ib_interpolate_advance / lbm_read_macros then see g = 0 until the next lbm_step. */
+PLB_API int ib_release_forcing(plb_ctx* ctx);
+
+enum { PLB_SPREAD_AUTO = 0, PLB_SPREAD_SCATTER = 1, PLB_SPREAD_AGGREGATE = 2, PLB_SPREAD_GATHER = 3 };
+PLB_API int ib_set_spread_mode(plb_ctx* ctx, int mode);
+PLB_API int ib_get_spread_mode(plb_ctx* ctx, int* out_mode_in_use);
 
 /* S4 + S5.  U_m = sum_ijk v_ijk phi phi phi (Eq. 33) with v the velocity lbm_read_macros
  * would return now (state after lbm_step, force just applied) and the stencil around the not yet
  * moved X_m; then X_m <- X_m + U_m (forward Euler).  Positions are kept unwrapped in fp64.
+ * Needs no preceding ib_spread: lbm_step(NULL) -> ib_interpolate_advance is passive advection.
  * A node ending outside [-1/2, n_a - 1/2] on a wall axis raises a sticky flag that plb_status and
  * ib_read_nodes report as PLB_ERR_NODE_LEFT. */
 PLB_API int ib_interpolate_advance(plb_ctx* ctx);
@@ -186,8 +212,7 @@ PLB_API int ib_set_receptors(plb_ctx* ctx, long n_receptors, const int* h_node, 
  * is closer than l_max is tested for formation (order of L276).  Uniforms from Philox keyed on
  * (seed; receptor, step, tag 3): word 0 breaks (u < P_r), word 1 forms (u < P_f).  Probabilities
  * are evaluated in fp64.  When more receptors pass the formation test for one site than it has
- * free places, the lowest receptor indices take them.  More than 32 same-step candidates for one
- * site raise a sticky error that plb_status reports as PLB_ERR_WORKSPACE. */
+ * free places, the lowest receptor indices take them (any number of same-step candidates). */
 PLB_API int ib_adhesion_update(plb_ctx* ctx, unsigned long long seed, unsigned long long step);
 PLB_API int ib_n_receptors(plb_ctx* ctx, long* out);
 /* h_bonds: 3 ints per receptor = (bound 0/1, s0, s1) */
@@ -204,8 +229,9 @@ PLB_API int ib_read_node_velocities(plb_ctx* ctx, float* h_U);     /* n x 3 AoS,
 /* populations in the paper's order, true f_i (not the stored f_i - w_i), float[19*cells] SoA */
 PLB_API int lbm_read_populations(plb_ctx* ctx, float* d_f);
 PLB_API int lbm_write_populations(plb_ctx* ctx, const float* d_f);
-/* debug aid: number of cells whose stored populations are not finite or whose density is not
- * positive (0 = healthy); synchronises the stream */
+/* debug aid: number of cells of the current state (what lbm_read_macros sees) with a non-finite
+ * population or a density sum_i f_i (Eq. 17) that is not positive (0 = healthy); synchronises the
+ * stream */
 PLB_API int lbm_check_finite(plb_ctx* ctx, long* out_bad_cells);
 /* synchronise the stream; returns PLB_ERR_NODE_LEFT / PLB_ERR_CUDA if raised since creation */
 PLB_API int plb_status(plb_ctx* ctx);

@@ -150,6 +150,12 @@ void orc_noise_normal3(uint64_t seed, uint64_t index, uint32_t step, uint32_t ta
     z[2] = r2 * cos(2.0 * PI * xi[3]);
 }
 
+/* the same for n indices at once (z: n x 3) -- a loop over the call above, for the tests */
+void orc_noise_normal3_many(uint64_t seed, const uint64_t* index, long n, uint32_t step, uint32_t tag, double* z) {
+#pragma omp parallel for schedule(static)
+    for (long t = 0; t < n; ++t) orc_noise_normal3(seed, index[t], step, tag, z + 3 * t);
+}
+
 /* ------------------------------------------------------------------------------------------ */
 int orc_create(int nx, int ny, int nz, double tau, const int kind[3], const double u_lo[9],
                const double u_hi[9], orc_ctx** out) {

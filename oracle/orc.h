@@ -40,6 +40,7 @@ void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t 
 double orc_uniform01(uint32_t r);                                  /* ((r>>8)+0.5) 2^-24 */
 void   orc_noise_uniform(uint64_t seed, uint64_t index, uint32_t step, uint32_t tag, double xi[4]);
 void   orc_noise_normal3(uint64_t seed, uint64_t index, uint32_t step, uint32_t tag, double z[3]);
+void   orc_noise_normal3_many(uint64_t seed, const uint64_t* index, long n, uint32_t step, uint32_t tag, double* z);
 
 int orc_create(int nx, int ny, int nz, double tau, const int kind[3],
                const double u_lo[9] /*[axis][comp]*/, const double u_hi[9], orc_ctx** out);

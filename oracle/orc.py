@@ -51,6 +51,7 @@ def lib(fp32: bool = False):
             "orc_uniform01": (C.c_double, [u32]),
             "orc_noise_uniform": (None, [u64, u64, u32, u32, dp]),
             "orc_noise_normal3": (None, [u64, u64, u32, u32, dp]),
+            "orc_noise_normal3_many": (None, [u64, C.POINTER(u64), C.c_long, u32, u32, dp]),
             "orc_create": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_double, ip, dp, dp, C.POINTER(vp)]),
             "orc_destroy": (C.c_int, [vp]),
             "orc_set_equilibrium": (C.c_int, [vp, dp, dp, C.c_double, u64]),
@@ -133,6 +134,14 @@ def noise_uniform(seed, index, step, tag):
 def noise_normal3(seed, index, step, tag):
     out = np.zeros(3)
     lib().orc_noise_normal3(int(seed), int(index), int(step), int(tag), _dp(out))
+    return out
+
+
+def noise_normal3_many(seed, index, step, tag):
+    """[n, 3] normals of the n counters `index` (orc_noise_normal3 in a loop)"""
+    idx = np.ascontiguousarray(index, dtype=np.uint64)
+    out = np.zeros((idx.shape[0], 3))
+    lib().orc_noise_normal3_many(int(seed), idx.ctypes.data_as(C.POINTER(C.c_uint64)), idx.shape[0], int(step), int(tag), _dp(out))
     return out
 
 

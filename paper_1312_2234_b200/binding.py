@@ -33,6 +33,9 @@ SYMBOLS = {
     "ib_set_triangles": (_i, [_vp, _i, _i, _i, _vp, _vp, _f, _f, _f]),
     "ib_compute_membrane_forces": (_i, [_vp, _f, _u64, _u64]),
     "ib_spread": (_i, [_vp, _vp]),
+    "ib_release_forcing": (_i, [_vp]),
+    "ib_set_spread_mode": (_i, [_vp, _i]),
+    "ib_get_spread_mode": (_i, [_vp, C.POINTER(_i)]),
     "ib_interpolate_advance": (_i, [_vp]),
     "ib_n_nodes": (_i, [_vp, C.POINTER(_l)]),
     "ib_read_nodes": (_i, [_vp, _vp]),
@@ -200,6 +203,24 @@ def ib_compute_membrane_forces(h, noise_sigma=0.0, noise_seed=0, step=0):
 
 def ib_spread(h, d_forcing):
     _check(lib().ib_spread(h, _dev_ptr(d_forcing)), "ib_spread")
+
+
+PLB_SPREAD_AUTO, PLB_SPREAD_SCATTER, PLB_SPREAD_AGGREGATE, PLB_SPREAD_GATHER = 0, 1, 2, 3
+SPREAD_MODES = {"auto": 0, "scatter": 1, "aggregate": 2, "gather": 3}
+
+
+def ib_release_forcing(h):
+    _check(lib().ib_release_forcing(h), "ib_release_forcing")
+
+
+def ib_set_spread_mode(h, mode):
+    _check(lib().ib_set_spread_mode(h, int(SPREAD_MODES.get(mode, mode))), "ib_set_spread_mode")
+
+
+def ib_get_spread_mode(h) -> int:
+    out = _i(0)
+    _check(lib().ib_get_spread_mode(h, C.byref(out)), "ib_get_spread_mode")
+    return out.value
 
 
 def ib_interpolate_advance(h):
@@ -402,6 +423,12 @@ class Simulation:
 
     def spread(self, d_forcing=None):
         ib_spread(self.h, self.forcing if d_forcing is None else d_forcing)
+
+    def set_spread_mode(self, mode):
+        ib_set_spread_mode(self.h, mode)
+
+    def spread_mode(self) -> int:
+        return ib_get_spread_mode(self.h)
 
     def interpolate_advance(self):
         ib_interpolate_advance(self.h)

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libplb.so")
 SOURCES = ["api.cu", "lbm.cu", "ib.cu", "adhesion.cu"]
-HEADERS = ["plb_internal.cuh", os.path.join("..", "..", "include", "plb.h")]
+HEADERS = ["plb_internal.cuh", "lbm_device.cuh", os.path.join("..", "..", "include", "plb.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -30,7 +30,9 @@ def stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    listed = {os.path.normpath(os.path.join(CSRC, s)) for s in SOURCES + HEADERS}
+    found = {os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))}
+    deps = sorted(listed | found) + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

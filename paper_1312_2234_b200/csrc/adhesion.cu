@@ -3,7 +3,7 @@
 // L244-246), the step after S5 in the paper's loop (L276).  The paper's own kernel
 // (sem_platelet_wall_kernel, L364-373) is "one thread per receptor"; so is this one, with the
 // contention for the places of a vWF site resolved deterministically (lowest receptor index first)
-// instead of by arrival order.
+// instead of by arrival order, for any number of same-step candidates per site.
 //
 // Monte-Carlo decisions are integer outcomes: the probabilities and the capture test are evaluated
 // in fp64 (B200 has full-rate-enough fp64 for a few million receptors), the same precision the
@@ -43,13 +43,11 @@ __device__ __forceinline__ double adh_uniform(const uint32_t r) {      // ((r >>
 
 // pass 1, one thread per receptor: break test of an existing bond, then (if the receptor is or has
 // just become unbound) formation test against its nearest site; a receptor that passes the
-// formation test enters the candidate list of the site.  bond = (bound, s0, s1, candidate site)
+// formation test becomes a candidate of the site.  bond = (bound, s0, s1, candidate site or -1)
 __global__ void __launch_bounds__(256) adhesion_test_kernel(const NodeArrays nodes, const int* __restrict__ rec_node,
                                                             int4* __restrict__ bond, int* __restrict__ site_count,
-                                                            int* __restrict__ cand_n, int* __restrict__ cand,
-                                                            int* __restrict__ counters, const long n_rec,
-                                                            const AdhParams p, const unsigned long long seed,
-                                                            const unsigned step) {
+                                                            const long n_rec, const AdhParams p,
+                                                            const unsigned long long seed, const unsigned step) {
     const long r = blockIdx.x * 256L + threadIdx.x;
     if (r >= n_rec) return;
     int4 b = bond[r];
@@ -73,9 +71,6 @@ __global__ void __launch_bounds__(256) adhesion_test_kernel(const NodeArrays nod
             const double r0 = (double)s0 - q.t0, r1 = (double)s1 - q.t1;
             const double x_b = sqrt(hw * hw + r0 * r0 + r1 * r1);
             if (x_b < p.l_max && adh_uniform(w.y) < adh_P_form(p, x_b)) {
-                const int slot = atomicAdd(cand_n + si, 1);
-                if (slot < ADH_MAX_CAND) cand[si * ADH_MAX_CAND + slot] = (int)r;
-                else atomicOr(counters + 1, STATUS_ADH_OVERFLOW);
                 b.y = (int)s0; b.z = (int)s1; b.w = (int)si;
             }
         }
@@ -83,33 +78,48 @@ __global__ void __launch_bounds__(256) adhesion_test_kernel(const NodeArrays nod
     bond[r] = b;
 }
 
-// pass 2: a candidate binds if (bonds the site still holds) + (candidates with a lower receptor
-// index) < max_per_site.  site_count is only read here; pass 3 commits.
-__global__ void __launch_bounds__(256) adhesion_resolve_kernel(int4* __restrict__ bond, const int* __restrict__ site_count,
-                                                               const int* __restrict__ cand_n, const int* __restrict__ cand,
-                                                               const long n_rec, const int max_per_site) {
+// passes 2 .. : the places of a site go to its candidates in the order of their receptor index (rule
+// 2 of L148 read as a sweep in index order, A-7), however many candidates there are.
+// One ROUND gives every site with candidates one decision: every pending candidate offers its
+// index to its site by atomicMin, then the candidate that sees its own index has the lowest one
+// left; it binds if the site still has a free place, and leaves the contest either way.  A site
+// can take at most max_per_site bonds, so after max_per_site rounds every candidate still pending
+// belongs to a full site and loses (last = true).
+__global__ void __launch_bounds__(256) adhesion_offer_kernel(const int4* __restrict__ bond, int* __restrict__ site_min,
+                                                             const long n_rec) {
+    const long r = blockIdx.x * 256L + threadIdx.x;
+    if (r >= n_rec) return;
+    const int si = bond[r].w;
+    if (si >= 0) atomicMin(site_min + si, (int)r);
+}
+
+__global__ void __launch_bounds__(256) adhesion_award_kernel(int4* __restrict__ bond, int* __restrict__ site_count,
+                                                             int* __restrict__ site_min, const long n_rec,
+                                                             const int max_per_site, const bool last) {
     const long r = blockIdx.x * 256L + threadIdx.x;
     if (r >= n_rec) return;
     int4 b = bond[r];
     if (b.w < 0) return;
-    const int n = min(__ldg(cand_n + b.w), ADH_MAX_CAND);
-    int rank = 0;
-    for (int i = 0; i < n; ++i) rank += __ldg(cand + (long)b.w * ADH_MAX_CAND + i) < (int)r ? 1 : 0;
-    if (__ldg(site_count + b.w) + rank < max_per_site) b.x = 1;
-    else { b.y = 0; b.z = 0; }
+    if (site_min[b.w] == (int)r) {                       // the only thread that touches this site now
+        const int held = site_count[b.w];
+        if (held < max_per_site) { b.x = 1; site_count[b.w] = held + 1; }
+        else { b.y = 0; b.z = 0; }
+        b.w = -1;
+    } else if (last) {
+        b.y = 0; b.z = 0; b.w = -1;
+    }
     bond[r] = b;
 }
 
-__global__ void __launch_bounds__(256) adhesion_commit_kernel(int4* __restrict__ bond, int* __restrict__ site_count,
-                                                              int* __restrict__ cand_n, const long n_rec) {
+// between two rounds: the minimum of a site that just decided is forgotten (its winner no longer
+// offers); one thread per receptor that decided would race with the readers above, so this is a
+// pass of its own over the candidates still pending
+__global__ void __launch_bounds__(256) adhesion_reset_kernel(const int4* __restrict__ bond, int* __restrict__ site_min,
+                                                             const long n_rec) {
     const long r = blockIdx.x * 256L + threadIdx.x;
     if (r >= n_rec) return;
-    int4 b = bond[r];
-    if (b.w < 0) return;
-    if (b.x) atomicAdd(site_count + b.w, 1);
-    cand_n[b.w] = 0;                                  // every candidate of the site stores the same 0
-    b.w = -1;
-    bond[r] = b;
+    const int si = bond[r].w;
+    if (si >= 0) site_min[si] = ADH_NO_OFFER;
 }
 
 // per-site bond counts from the bond table (ib_write_bonds)
@@ -184,12 +194,26 @@ int launch_adhesion_forces(Ctx* c) {
 int launch_adhesion_update(Ctx* c, unsigned long long seed, unsigned long long step) {
     if (!c->n_rec) return PLB_OK;
     const unsigned grid = blocks_for(c->n_rec);
-    adhesion_test_kernel<<<grid, 256, 0, c->stream>>>(node_arrays(c), c->rec_node, c->bond, c->site_count, c->cand_n, c->cand,
-                                                      c->counters, c->n_rec, c->adh, seed, (unsigned)step);
-    adhesion_resolve_kernel<<<grid, 256, 0, c->stream>>>(c->bond, c->site_count, c->cand_n, c->cand, c->n_rec,
-                                                         c->adh.max_per_site);
-    adhesion_commit_kernel<<<grid, 256, 0, c->stream>>>(c->bond, c->site_count, c->cand_n, c->n_rec);
-    c->launches += 3;
+    adhesion_test_kernel<<<grid, 256, 0, c->stream>>>(node_arrays(c), c->rec_node, c->bond, c->site_count, c->n_rec, c->adh,
+                                                      seed, (unsigned)step);
+    c->launches++;
+    // site_min is INT_MAX everywhere between updates (set at ib_set_receptors; every site that was
+    // offered to is reset below or decided for good in the last round)
+    const int rounds = c->adh.max_per_site;
+    for (int round = 0; round < rounds; ++round) {
+        adhesion_offer_kernel<<<grid, 256, 0, c->stream>>>(c->bond, c->site_min, c->n_rec);
+        adhesion_award_kernel<<<grid, 256, 0, c->stream>>>(c->bond, c->site_count, c->site_min, c->n_rec,
+                                                           c->adh.max_per_site, round == rounds - 1);
+        c->launches += 2;
+        if (round < rounds - 1) {
+            adhesion_reset_kernel<<<grid, 256, 0, c->stream>>>(c->bond, c->site_min, c->n_rec);
+            c->launches++;
+        }
+    }
+    // the sites decided in the last round still hold their winner's index
+    int rc = cuda_check(cudaMemsetAsync(c->site_min, 0x7f, (size_t)c->adh.n0 * c->adh.n1 * sizeof(int), c->stream),
+                        "reset site minima");
+    if (rc) return rc;
     return cuda_check(cudaGetLastError(), "adhesion update kernels");
 }
 

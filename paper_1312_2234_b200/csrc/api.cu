@@ -1,5 +1,6 @@
 // api.cu -- the C-ABI of libplb (include/plb.h): argument checks, workspace carving, call-order
 // bookkeeping.  Every step of the path runs in the kernels of lbm.cu / ib.cu.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -45,6 +46,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     unsigned* seg_mask = w.take<unsigned>((size_t)(n_segs + 31) / 32);
     int* counters = w.take<int>(64);
     int* seg_list = w.take<int>((size_t)n_segs);
+    float4* vfield = w.take<float4>((size_t)n_segs * SEG);
     double* X0 = w.take<double>((size_t)max_nodes);
     double* X1 = w.take<double>((size_t)max_nodes);
     double* X2 = w.take<double>((size_t)max_nodes);
@@ -54,6 +56,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     int2* edges = w.take<int2>((size_t)max_edges);
     float2* eprm = w.take<float2>((size_t)max_edges);
     int2* ranges = w.take<int2>((size_t)max_nodes);
+    int* orig = w.take<int>((size_t)max_nodes);
     // a closed genus-0 triangulated surface of N nodes has 2N - 4 triangles and at least 4 nodes
     int4* tris = w.take<int4>((size_t)2 * max_nodes);
     float* tri_S0 = w.take<float>((size_t)2 * max_nodes);
@@ -62,11 +65,47 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
         c->tris = tris; c->tri_S0 = tri_S0; c->cons = cons;
         c->cap_tris = 2 * max_nodes; c->cap_cons = max_nodes / 4 + 1;
         c->f[0] = f0; c->f[1] = f1;
-        c->seg_mask = seg_mask; c->counters = counters; c->seg_list = seg_list;
+        c->seg_mask = seg_mask; c->counters = counters; c->seg_list = seg_list; c->vfield = vfield;
         c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
-        c->edges = edges; c->edge_prm = eprm; c->ranges = ranges;
+        c->edges = edges; c->edge_prm = eprm; c->ranges = ranges; c->orig = orig;
     }
     return w.off;
+}
+
+// Order of the nodes of one mesh along the Morton (Z-order) curve of its shape: 10 bits per axis
+// over the cube that bounds the mesh, ties broken by the caller's index.  ord[j] = caller's local
+// index of the j-th stored node.
+static unsigned spread_bits10(unsigned v) {
+    v &= 0x3ffu;
+    v = (v | (v << 16)) & 0x030000ffu;
+    v = (v | (v << 8)) & 0x0300f00fu;
+    v = (v | (v << 4)) & 0x030c30c3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+static std::vector<int> morton_order(const double* xyz, int n) {
+    double lo[3] = {xyz[0], xyz[1], xyz[2]}, hi[3] = {xyz[0], xyz[1], xyz[2]};
+    for (int m = 1; m < n; ++m)
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = xyz[3 * m + d] < lo[d] ? xyz[3 * m + d] : lo[d];
+            hi[d] = xyz[3 * m + d] > hi[d] ? xyz[3 * m + d] : hi[d];
+        }
+    double ext = 0.0;
+    for (int d = 0; d < 3; ++d) ext = hi[d] - lo[d] > ext ? hi[d] - lo[d] : ext;
+    const double scale = (ext > 0.0 && std::isfinite(ext)) ? 1023.0 / ext : 0.0;
+    std::vector<unsigned> code((size_t)n);
+    for (int m = 0; m < n; ++m) {
+        unsigned q[3];
+        for (int d = 0; d < 3; ++d) {
+            const double t = (xyz[3 * m + d] - lo[d]) * scale;
+            q[d] = t >= 0.0 && t <= 1023.0 ? (unsigned)t : 0u;
+        }
+        code[m] = spread_bits10(q[0]) | (spread_bits10(q[1]) << 1) | (spread_bits10(q[2]) << 2);
+    }
+    std::vector<int> ord((size_t)n);
+    for (int m = 0; m < n; ++m) ord[m] = m;
+    std::sort(ord.begin(), ord.end(), [&](int a, int b) { return code[a] != code[b] ? code[a] < code[b] : a < b; });
+    return ord;
 }
 
 static int check_grid(const plb_grid* g, long* cells) {
@@ -92,10 +131,6 @@ static int sync_status(Ctx* c) {
     if (h[1] & STATUS_ZERO_EDGE) {
         set_error("a mesh edge has zero length");
         return PLB_ERR_ARG;
-    }
-    if (h[1] & STATUS_ADH_OVERFLOW) {
-        set_error("more than %d same-step bond candidates for one vWF site", ADH_MAX_CAND);
-        return PLB_ERR_WORKSPACE;
     }
     if (h[1] & STATUS_ADH_BAD_SITE) {
         set_error("ib_write_bonds: a bond names a site outside a non-periodic tangential axis");
@@ -219,6 +254,8 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->list_parity = 0;
     c->tile_cap = 512;
     c->spread_cap = 1024;
+    c->spread_mode = PLB_SPREAD_AUTO;
+    c->tile_nodes = 0.0; c->tile_cells = 0.0; c->tile_density = 0.0;
     c->sm_count = sms;
     c->mesh_node_off.push_back(0);
     c->mesh_edge_off.push_back(0);
@@ -347,16 +384,39 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
         set_error("ib_add_meshes: more than 2^31 nodes");
         return PLB_ERR_ARG;
     }
+    // Internal node order (hidden behind every call that names a node: ib_read/write_*, triangles,
+    // receptors, the noise key): the nodes of a mesh are stored along the Morton curve of the first
+    // mesh's shape.  The topology is fixed, so nodes that are consecutive in storage stay
+    // neighbours on the surface however the mesh moves or deforms: a run of consecutive nodes is a
+    // compact patch (small lattice tile, several blocks per mesh), and the two ends of an edge lie
+    // close together in memory.
+    const std::vector<int> ord = morton_order(h_xyz, n_nodes);           // ord[stored local] = caller's local
+    std::vector<int> inv((size_t)n_nodes);
+    for (int j = 0; j < n_nodes; ++j) inv[ord[j]] = j;
     // host-side marshalling: AoS -> SoA positions, mesh-local -> global edge indices
     std::vector<double> soa((size_t)3 * add_nodes);
-    for (long m = 0; m < add_nodes; ++m)
-        for (int d = 0; d < 3; ++d) soa[(size_t)d * add_nodes + m] = h_xyz[3 * m + d];
+    std::vector<int> og((size_t)add_nodes);
+    for (int s = 0; s < n_meshes; ++s)
+        for (int j = 0; j < n_nodes; ++j) {
+            const long m = (long)s * n_nodes + j, src = (long)s * n_nodes + ord[j];
+            for (int d = 0; d < 3; ++d) soa[(size_t)d * add_nodes + m] = h_xyz[3 * src + d];
+            og[m] = (int)(ctx->n_nodes + src);
+        }
+    // edges in stored indices, ordered by their lower end (orientation kept: R = X_b - X_a)
+    std::vector<int> eorder((size_t)n_edges);
+    for (int e = 0; e < n_edges; ++e) eorder[e] = e;
+    std::sort(eorder.begin(), eorder.end(), [&](int p, int q) {
+        const int ap = inv[h_edges[2 * p]], bp = inv[h_edges[2 * p + 1]], aq = inv[h_edges[2 * q]], bq = inv[h_edges[2 * q + 1]];
+        const int lp = ap < bp ? ap : bp, lq = aq < bq ? aq : bq, hp = ap < bp ? bp : ap, hq = aq < bq ? bq : aq;
+        return lp != lq ? lp < lq : (hp != hq ? hp < hq : p < q);
+    });
     std::vector<int2> eg((size_t)add_edges);
     std::vector<float2> ep((size_t)add_edges);
     for (int s = 0; s < n_meshes; ++s) {
         const long noff = ctx->n_nodes + (long)s * n_nodes;
         const double* x = h_xyz + (size_t)3 * s * n_nodes;
-        for (int e = 0; e < n_edges; ++e) {
+        for (int i = 0; i < n_edges; ++i) {
+            const int e = eorder[i];
             const int a = h_edges[2 * e], b = h_edges[2 * e + 1];
             float L;
             if (h_rest) L = h_rest[e];
@@ -365,37 +425,49 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
                 for (int d = 0; d < 3; ++d) s2 += (x[3 * b + d] - x[3 * a + d]) * (x[3 * b + d] - x[3 * a + d]);
                 L = (float)sqrt(s2);
             }
-            eg[(size_t)s * n_edges + e] = make_int2((int)(noff + a), (int)(noff + b));
-            ep[(size_t)s * n_edges + e] = make_float2(L, k);
+            eg[(size_t)s * n_edges + i] = make_int2((int)(noff + inv[a]), (int)(noff + inv[b]));
+            ep[(size_t)s * n_edges + i] = make_float2(L, k);
         }
     }
-    // node ranges of the IB thread blocks (a mesh, cut every IB_RANGE_NODES nodes) and the tile
-    // capacity their initial bounding boxes ask for (two cells of slack per axis for deformation)
-    constexpr int IB_RANGE_NODES = 4096;
+    // Node ranges of the IB thread blocks: a mesh, cut into runs of consecutive stored nodes (=
+    // surface patches) so that the IB kernels get about two blocks per SM even when there are few
+    // meshes (Eq. 33-34 are sums over nodes with no per-mesh structure), and never longer than
+    // IB_RANGE_NODES.  Tile capacity: what the initial bounding boxes of the ranges ask for (two
+    // cells of slack per axis for deformation).
+    constexpr int IB_RANGE_NODES = 4096, IB_MIN_RANGE_NODES = 64;
+    const long meshes_after = (long)ctx->mesh_node_off.size() - 1 + n_meshes;
+    long parts = (2L * ctx->sm_count + meshes_after - 1) / meshes_after;
+    if (parts > n_nodes / IB_MIN_RANGE_NODES) parts = n_nodes / IB_MIN_RANGE_NODES;
+    if (parts < (n_nodes + IB_RANGE_NODES - 1) / IB_RANGE_NODES) parts = (n_nodes + IB_RANGE_NODES - 1) / IB_RANGE_NODES;
+    if (parts < 1) parts = 1;
     std::vector<int2> rg;
     int cap = ctx->tile_cap, scap = ctx->spread_cap;
     for (int s = 0; s < n_meshes; ++s) {
         const long noff = ctx->n_nodes + (long)s * n_nodes;
         const double* x = h_xyz + (size_t)3 * s * n_nodes;
-        for (int a = 0; a < n_nodes; a += IB_RANGE_NODES) {
-            const int b = a + IB_RANGE_NODES < n_nodes ? a + IB_RANGE_NODES : n_nodes;
+        for (long part = 0; part < parts; ++part) {
+            const int a = (int)((long)n_nodes * part / parts), b = (int)((long)n_nodes * (part + 1) / parts);
+            if (b <= a) continue;
             rg.push_back(make_int2((int)(noff + a), (int)(noff + b)));
-            double vol = 1.0;
+            double vol = 1.0, box = 1.0;
             int ext[3];
             for (int d = 0; d < 3; ++d) {
-                double lo = floor(x[3 * a + d]), hi = lo;
+                double lo = floor(x[3 * ord[a] + d]), hi = lo;
                 for (int m = a + 1; m < b; ++m) {
-                    const double f = floor(x[3 * m + d]);
+                    const double f = floor(x[3 * ord[m] + d]);
                     lo = f < lo ? f : lo;
                     hi = f > hi ? f : hi;
                 }
                 vol *= hi - lo + 4.0 + 2.0;
+                box *= hi - lo + 4.0;
                 ext[d] = hi - lo < 1e6 ? (int)(hi - lo) + 6 : 1 << 20;
             }
             // A mesh may turn (a flipping platelet).  The spread tile is sized for the cube of the
             // largest extent when that fits; the interpolation tile, whose kernel wants the L1 cache
             // that shared memory takes away (measured: 105 KB instead of 78 KB per block costs 45 %),
             // for the initial box, but for at least min(cube, 4352 cells).
+            ctx->tile_nodes += (double)(b - a);
+            ctx->tile_cells += box;
             const int emax = ext[0] > ext[1] ? (ext[0] > ext[2] ? ext[0] : ext[2]) : (ext[1] > ext[2] ? ext[1] : ext[2]);
             const double cube = (double)emax * emax * emax;
             if (vol <= (double)ib_max_tile_cap()) {
@@ -411,12 +483,15 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
     }
     ctx->tile_cap = cap;
     ctx->spread_cap = scap;
+    ctx->tile_density = ctx->tile_cells > 0.0 ? ctx->tile_nodes / ctx->tile_cells : 0.0;
     int rc = cuda_check(cudaMemcpyAsync(ctx->ranges + ctx->n_ranges, rg.data(), rg.size() * sizeof(int2),
                                         cudaMemcpyHostToDevice, ctx->stream), "upload node ranges");
     for (int d = 0; d < 3 && !rc; ++d)
         rc = cuda_check(cudaMemcpyAsync(ctx->X[d] + ctx->n_nodes, soa.data() + (size_t)d * add_nodes,
                                         (size_t)add_nodes * sizeof(double), cudaMemcpyHostToDevice, ctx->stream),
                         "upload node positions");
+    if (!rc) rc = cuda_check(cudaMemcpyAsync(ctx->orig + ctx->n_nodes, og.data(), (size_t)add_nodes * sizeof(int),
+                                             cudaMemcpyHostToDevice, ctx->stream), "upload node order");
     if (!rc) rc = cuda_check(cudaMemsetAsync(ctx->F + ctx->n_nodes, 0, (size_t)add_nodes * sizeof(float4), ctx->stream), "clear forces");
     if (!rc) rc = cuda_check(cudaMemsetAsync(ctx->U + ctx->n_nodes, 0, (size_t)add_nodes * sizeof(float4), ctx->stream), "clear node velocities");
     if (!rc && add_edges) {
@@ -428,6 +503,9 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
     if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
     if (rc) return rc;
     ctx->n_ranges += (long)rg.size();
+    ctx->h_orig.insert(ctx->h_orig.end(), og.begin(), og.end());
+    ctx->h_stored.resize(ctx->h_orig.size());
+    for (long m = ctx->n_nodes; m < ctx->n_nodes + add_nodes; ++m) ctx->h_stored[ctx->h_orig[m]] = (int)m;
     if (out_first_mesh_id) *out_first_mesh_id = (int)ctx->mesh_node_off.size() - 1;
     for (int s = 0; s < n_meshes; ++s) {
         ctx->n_nodes += n_nodes;
@@ -495,8 +573,8 @@ int ib_set_triangles(plb_ctx* ctx, int first_mesh_id, int n_meshes, int n_tris, 
                 set_error("ib_set_triangles: triangle %d of the unstressed shape has zero area", t);
                 return PLB_ERR_ARG;
             }
-            tg[(size_t)s * n_tris + t] = make_int4((int)(noff + h_tris[3 * t]), (int)(noff + h_tris[3 * t + 1]),
-                                                   (int)(noff + h_tris[3 * t + 2]), 0);
+            tg[(size_t)s * n_tris + t] = make_int4(ctx->h_stored[noff + h_tris[3 * t]], ctx->h_stored[noff + h_tris[3 * t + 1]],
+                                                   ctx->h_stored[noff + h_tris[3 * t + 2]], 0);
         }
         if (!(m.V0 > 0.0)) {
             set_error("ib_set_triangles: the surface is not closed or not oriented outwards (V_0 = %g)", m.V0);
@@ -550,11 +628,42 @@ int ib_spread(plb_ctx* ctx, float* d_forcing) {
     return launch_spread(ctx, (float4*)d_forcing);
 }
 
+int ib_release_forcing(plb_ctx* ctx) {
+    REQUIRE_CTX(ctx);
+    int rc = PLB_OK;
+    if (ctx->spread_target) rc = launch_clear_spread(ctx, ctx->spread_target);
+    if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
+    ctx->spread_target = nullptr;
+    ctx->spread_current = false;
+    ctx->g_last = nullptr;
+    ctx->g_last_mode = FORCE_NONE;
+    return rc;
+}
+
+int ib_set_spread_mode(plb_ctx* ctx, int mode) {
+    REQUIRE_CTX(ctx);
+    if (mode != PLB_SPREAD_AUTO && mode != PLB_SPREAD_SCATTER && mode != PLB_SPREAD_AGGREGATE && mode != PLB_SPREAD_GATHER) {
+        set_error("ib_set_spread_mode: unknown mode %d", mode);
+        return PLB_ERR_ARG;
+    }
+    ctx->spread_mode = mode;
+    return PLB_OK;
+}
+
+int ib_get_spread_mode(plb_ctx* ctx, int* out_mode_in_use) {
+    REQUIRE_CTX(ctx);
+    if (!out_mode_in_use) return PLB_ERR_ARG;
+    *out_mode_in_use = spread_mode_of(ctx);
+    return PLB_OK;
+}
+
 int ib_interpolate_advance(plb_ctx* ctx) {
     REQUIRE_CTX(ctx);
     if (ctx->n_nodes == 0) return PLB_OK;
-    if (!ctx->populated || !ctx->spread_current) {
-        set_error("ib_interpolate_advance must follow ib_spread (and lbm_step) for the current node positions");
+    // no ib_spread needs to have run: lbm_step(NULL) -> ib_interpolate_advance is passive advection
+    // (Eq. 33 alone); the force term of v is that of the last lbm_step, whatever its source
+    if (!ctx->populated) {
+        set_error("ib_interpolate_advance before the populations were set");
         return PLB_ERR_ORDER;
     }
     const int rc = launch_interpolate_advance(ctx);
@@ -570,10 +679,9 @@ static size_t carve_adhesion(Ctx* c, char* base, long n_sites, long n_rec) {
     int* rec_node = w.take<int>((size_t)n_rec);
     int4* bond = w.take<int4>((size_t)n_rec);
     int* site_count = w.take<int>((size_t)n_sites);
-    int* cand_n = w.take<int>((size_t)n_sites);
-    int* cand = w.take<int>((size_t)n_sites * ADH_MAX_CAND);
+    int* site_min = w.take<int>((size_t)n_sites);
     if (c) {
-        c->rec_node = rec_node; c->bond = bond; c->site_count = site_count; c->cand_n = cand_n; c->cand = cand;
+        c->rec_node = rec_node; c->bond = bond; c->site_count = site_count; c->site_min = site_min;
     }
     return w.off;
 }
@@ -610,13 +718,13 @@ int ib_set_receptors(plb_ctx* ctx, long n_receptors, const int* h_node, const pl
         set_error("ib_set_receptors: wall_axis %d is not a wall axis of this context", a);
         return PLB_ERR_ARG;
     }
-    if (prm->max_per_site < 1 || prm->max_per_site > ADH_MAX_CAND || !(prm->l_max > 0.f) || prm->k_on0 < 0.f ||
-        prm->k_off0 < 0.f || prm->F0 < 0.f || prm->tau_rep < 0.f) {
-        set_error("ib_set_receptors: invalid parameters (1 <= max_per_site <= %d, l_max > 0, rates, F0, tau_rep >= 0)", ADH_MAX_CAND);
+    if (prm->max_per_site < 1 || prm->max_per_site > ADH_MAX_PER_SITE || !(prm->l_max > 0.f) || prm->k_on0 < 0.f ||
+        prm->k_off0 < 0.f || prm->F0 < 0.f || prm->tau_rep < 0.f || (prm->F0 > 0.f && !(prm->tau_rep > 0.f))) {
+        set_error("ib_set_receptors: invalid parameters (1 <= max_per_site <= %d, l_max > 0, rates, F0, tau_rep >= 0, tau_rep > 0 when F0 > 0)", ADH_MAX_PER_SITE);
         return PLB_ERR_ARG;
     }
-    if (n_receptors >= (1L << 31)) {
-        set_error("ib_set_receptors: more than 2^31 receptors");
+    if (n_receptors >= (long)ADH_NO_OFFER) {
+        set_error("ib_set_receptors: more than 0x7f7f7f7f receptors");
         return PLB_ERR_ARG;
     }
     for (long r = 0; r < n_receptors; ++r)
@@ -644,8 +752,11 @@ int ib_set_receptors(plb_ctx* ctx, long n_receptors, const int* h_node, const pl
     ctx->n_rec = n_receptors;
     ctx->adh_on = true;
     int rc = cuda_check(cudaMemsetAsync(d_workspace, 0, need, ctx->stream), "clear adhesion workspace");
+    if (!rc) rc = cuda_check(cudaMemsetAsync(ctx->site_min, 0x7f, (size_t)n_sites * sizeof(int), ctx->stream), "reset site minima");
+    std::vector<int> stored((size_t)n_receptors);
+    for (long r = 0; r < n_receptors; ++r) stored[r] = ctx->h_stored[h_node[r]];
     if (!rc && n_receptors)
-        rc = cuda_check(cudaMemcpyAsync(ctx->rec_node, h_node, (size_t)n_receptors * sizeof(int), cudaMemcpyHostToDevice,
+        rc = cuda_check(cudaMemcpyAsync(ctx->rec_node, stored.data(), (size_t)n_receptors * sizeof(int), cudaMemcpyHostToDevice,
                                         ctx->stream), "upload receptor nodes");
     if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
     ctx->forces_valid = false;
@@ -698,6 +809,14 @@ int ib_write_bonds(plb_ctx* ctx, const int* h_bonds) {
     for (long r = 0; r < n; ++r) {
         const int on = h_bonds[3 * r] ? 1 : 0;
         tmp[r] = make_int4(on, on ? h_bonds[3 * r + 1] : 0, on ? h_bonds[3 * r + 2] : 0, -1);
+        // a bond to a site outside a non-periodic tangential axis is refused here, before anything is
+        // uploaded: left in the table, the next update would index the site counts out of bounds
+        if (on && ((!ctx->adh.per0 && (tmp[r].y < 0 || tmp[r].y >= ctx->adh.n0)) ||
+                   (!ctx->adh.per1 && (tmp[r].z < 0 || tmp[r].z >= ctx->adh.n1)))) {
+            set_error("ib_write_bonds: receptor %ld is bound to site (%d, %d), outside a non-periodic tangential axis", r,
+                      tmp[r].y, tmp[r].z);
+            return PLB_ERR_ARG;
+        }
     }
     int rc = PLB_OK;
     if (n) rc = cuda_check(cudaMemcpyAsync(ctx->bond, tmp.data(), (size_t)n * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream),
@@ -755,7 +874,8 @@ static int read_node_float4(plb_ctx* ctx, const float4* d_src, float* h_out) {
     if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
     if (rc) return rc;
     for (long m = 0; m < n; ++m) {
-        h_out[3 * m] = tmp[m].x; h_out[3 * m + 1] = tmp[m].y; h_out[3 * m + 2] = tmp[m].z;
+        const long o = ctx->h_orig[m];
+        h_out[3 * o] = tmp[m].x; h_out[3 * o + 1] = tmp[m].y; h_out[3 * o + 2] = tmp[m].z;
     }
     return PLB_OK;
 }
@@ -777,7 +897,10 @@ int ib_write_forces(plb_ctx* ctx, const float* h_F) {
     if (!h_F) return PLB_ERR_ARG;
     const long n = ctx->n_nodes;
     std::vector<float4> tmp((size_t)n);
-    for (long m = 0; m < n; ++m) tmp[m] = make_float4(h_F[3 * m], h_F[3 * m + 1], h_F[3 * m + 2], 0.f);
+    for (long m = 0; m < n; ++m) {
+        const long o = ctx->h_orig[m];
+        tmp[m] = make_float4(h_F[3 * o], h_F[3 * o + 1], h_F[3 * o + 2], 0.f);
+    }
     int rc = cuda_check(cudaMemcpyAsync(ctx->F, tmp.data(), (size_t)n * sizeof(float4), cudaMemcpyHostToDevice, ctx->stream),
                         "upload forces");
     if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");

@@ -14,14 +14,16 @@ namespace plb {
 // R and |R| - L are formed in fp64 (positions reach ~1e3, lengths ~1, stretches ~1e-3), the
 // rest in fp32; two vector atomics per edge.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) force_init_kernel(float4* __restrict__ F, const long n, const float sigma,
-                                                         const unsigned long long seed, const unsigned step) {
+__global__ void __launch_bounds__(256) force_init_kernel(float4* __restrict__ F, const int* __restrict__ orig, const long n,
+                                                         const float sigma, const unsigned long long seed,
+                                                         const unsigned step) {
     const long m = blockIdx.x * 256L + threadIdx.x;
     if (m >= n) return;
     float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
     if (sigma > 0.f) {
-        // Box-Muller on the four uniforms of counter (node, step, tag 2)
-        const uint4 r = noise_words(seed, (unsigned long long)m, step, 2u);
+        // Box-Muller on the four uniforms of counter (node, step, tag 2); the key is the caller's
+        // global node index, not the stored one
+        const uint4 r = noise_words(seed, (unsigned long long)__ldg(orig + m), step, 2u);
         const float r0 = sqrtf(-2.0f * logf(uniform01(r.x)));
         const float r2 = sqrtf(-2.0f * logf(uniform01(r.z)));
         float s1, c1;
@@ -373,6 +375,44 @@ __device__ __forceinline__ void spread_record(const SpreadChunk& ch, const int r
     ch.f[r] = F.x * scale; ch.f[SPREAD_CHUNK + r] = F.y * scale; ch.f[2 * SPREAD_CHUNK + r] = F.z * scale;
 }
 
+// Flush of a spread tile: one vector RED per non-zero tile cell.  The segments this block is the
+// first to mark are collected in shared memory and appended to the global list with ONE atomicAdd
+// per block (a returning atomic per segment on the single list counter was 58 % of the scatter
+// kernel's stall samples).  All threads of the block call it, after a __syncthreads().
+__device__ __forceinline__ void spread_flush(MeshTile& T, const int* __restrict__ tile, int* __restrict__ new_segs,
+                                             const int cap, const float inv_scale, float4* __restrict__ g,
+                                             unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
+                                             int* __restrict__ seg_count, const LbmParams& p) {
+    const int tid = threadIdx.x;
+    const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+    for (int t = tid; t < ncell; t += IB_THREADS) {
+        const int x = t % e0, r = t / e0;
+        const int y = r % e1, z = r / e1;
+        const int w = z * T.pp + y * T.p0 + x;
+        const int qx = tile[w], qy = tile[cap + w], qz = tile[2 * cap + w];
+        if ((qx | qy | qz) != 0) {
+            const Cell c = tile_cell(T, t, p);
+            const int cell = c.i + p.nx * (c.j + p.ny * c.k);
+            atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
+            const int seg = cell >> SEG_SHIFT;
+            const unsigned bit = 1u << (seg & 31);
+            unsigned* word = seg_mask + (seg >> 5);
+            if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u) {
+                const int slot = atomicAdd(&T.n_need, 1);               // n_need doubles as the block's list length
+                if (slot < SPREAD_SEG_LIST) new_segs[slot] = seg;
+                else seg_list[atomicAdd(seg_count, 1)] = seg;          // list full: append directly
+            }
+        }
+    }
+    __syncthreads();
+    const int n_new = min(T.n_need, SPREAD_SEG_LIST);
+    if (n_new == 0) return;
+    if (tid == 0) T.mn[0] = atomicAdd(seg_count, n_new);
+    __syncthreads();
+    const int first = T.mn[0];
+    for (int i = tid; i < n_new; i += IB_THREADS) seg_list[first + i] = new_segs[i];
+}
+
 __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_kernel(
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
@@ -451,36 +491,239 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     }
     if (!tiled) return;
     __syncthreads();
-    // flush: one vector RED per non-zero tile cell.  The segments this block is the first to mark are
-    // collected in shared memory and appended to the global list with ONE atomicAdd per block (a
-    // returning atomic per segment on the single list counter was 58 % of this kernel's stall samples).
-    const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
-    for (int t = tid; t < ncell; t += IB_THREADS) {
-        const int x = t % e0, r = t / e0;
-        const int y = r % e1, z = r / e1;
-        const int w = z * T.pp + y * T.p0 + x;
-        const int qx = tile[w], qy = tile[cap + w], qz = tile[2 * cap + w];
-        if ((qx | qy | qz) != 0) {
-            const Cell c = tile_cell(T, t, p);
-            const int cell = c.i + p.nx * (c.j + p.ny * c.k);
-            atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
-            const int seg = cell >> SEG_SHIFT;
-            const unsigned bit = 1u << (seg & 31);
-            unsigned* word = seg_mask + (seg >> 5);
-            if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u) {
-                const int slot = atomicAdd(&T.n_need, 1);               // n_need doubles as the block's list length
-                if (slot < SPREAD_SEG_LIST) new_segs[slot] = seg;
-                else seg_list[atomicAdd(seg_count, 1)] = seg;          // list full: append directly
-            }
+    spread_flush(T, tile, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
+}
+
+// ---------------------------------------------------------------------------------------------
+// S2, BINNED forms (north_star: "gather-by-cell over Morton-sorted nodes or warp-aggregated
+// atomics, whichever the counters favour"; the paper's own fluid3d_force_distribute_kernel is
+// gather-shaped, L356-362).  The nodes of a chunk are counting-sorted in shared memory by their
+// base cell b = floor(X) - 1 (a "bin"): all nodes of a bin spread into the SAME 4 x 4 x 4 cells.
+//   AGGREGATE (warp-aggregated atomics): one warp per occupied bin; lane = (ox, oy, oz mod 2) owns
+//     the two cells (ox, oy, oz) and (ox, oy, oz + 2) of the bin's stencil, reads the bin's node
+//     records as shared-memory broadcasts, sums W F over the nodes IN REGISTERS and issues one
+//     shared-memory atomic per (bin, cell, component) instead of one per (node, cell, component).
+//   GATHER (no atomics at all): one thread per tile cell sums W F over the nodes of the (up to)
+//     4 x 4 x 4 bins whose stencil contains the cell, and adds the total to its own tile cell.
+// Both accumulate in 32-bit fixed point, so the result does not depend on the order of the nodes
+// inside a bin (which the counting sort does not fix): each product W F 2^k is rounded to an
+// integer on its own -- by the magic-number addition fma(w, f, 1.5 * 2^23), a full-rate FMA
+// instead of a quarter-rate F2I -- and integer addition commutes.  |W F 2^k| < 2^22 by the choice of k.
+// ---------------------------------------------------------------------------------------------
+constexpr int BIN_CHUNK = IB_THREADS;              // nodes sorted per pass: one per thread
+constexpr float FIX_MAGIC = 12582912.0f;           // 1.5 * 2^23
+constexpr int FIX_MAGIC_BITS = 0x4B400000;
+
+// direct path of a range whose bounding box does not fit the tile: one RED per (node, cell)
+__device__ __forceinline__ void spread_direct(const double* __restrict__ X, const double* __restrict__ Y,
+                                              const double* __restrict__ Z, const float4* __restrict__ F, const int n0,
+                                              const int n1, float4* __restrict__ g, unsigned* __restrict__ seg_mask,
+                                              int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams& p) {
+    const int sub = threadIdx.x & (SPREAD_LANES - 1), ox = sub & 3, oy = sub >> 2;
+    for (int m = n0 + (int)threadIdx.x / SPREAD_LANES; m < n1; m += SPREAD_GROUPS) {
+        const double x = X[m], y = Y[m], z = Z[m];
+        const float4 Fm = __ldg(F + m);
+        const double fx = floor(x), fy = floor(y), fz = floor(z);
+        float sx, cx, sy, cy, sz, cz;
+        sincospif(0.5f * (float)(x - fx), &sx, &cx);
+        sincospif(0.5f * (float)(y - fy), &sy, &cy);
+        sincospif(0.5f * (float)(z - fz), &sz, &cz);
+        const int qx = wrap_index((int)fx - 1 + ox, p.nx, p.wall[0]), qy = wrap_index((int)fy - 1 + oy, p.ny, p.wall[1]);
+        if (qx < 0 || qy < 0) continue;
+        const float wxy = weight_o(sx, cx, ox) * weight_o(sy, cy, oy);
+        const float gx = wxy * Fm.x, gy = wxy * Fm.y, gz = wxy * Fm.z;
+#pragma unroll
+        for (int oz = 0; oz < 4; ++oz) {
+            const int qz = wrap_index((int)fz - 1 + oz, p.nz, p.wall[2]);
+            if (qz < 0) continue;
+            const float wz = weight_o(sz, cz, oz);
+            const int cell = qx + p.nx * (qy + p.ny * qz);
+            atomicAdd(g + cell, make_float4(wz * gx, wz * gy, wz * gz, 0.f));
+            mark_segment(cell, seg_mask, seg_list, seg_count);
         }
     }
+}
+
+// in-place exclusive prefix sum of a[0 .. n) in shared memory, a[n] = total; all threads call it
+__device__ __forceinline__ void block_exclusive_scan(int* __restrict__ a, const int n, int* __restrict__ warp_tot) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int items = (n + IB_THREADS - 1) / IB_THREADS, first = tid * items;
+    int sum = 0;
+    for (int i = 0; i < items; ++i) sum += first + i < n ? a[first + i] : 0;
+    int incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) warp_tot[warp] = incl;
     __syncthreads();
-    const int n_new = min(T.n_need, SPREAD_SEG_LIST);
-    if (n_new == 0) return;
-    if (tid == 0) T.mn[0] = atomicAdd(seg_count, n_new);
+    if (warp == 0) {
+        const int w = lane < IB_THREADS / 32 ? warp_tot[lane] : 0;
+        int wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += v;
+        }
+        if (lane < IB_THREADS / 32) warp_tot[lane] = wi - w;
+        if (lane == IB_THREADS / 32 - 1) a[n] = wi;
+    }
     __syncthreads();
-    const int first = T.mn[0];
-    for (int i = tid; i < n_new; i += IB_THREADS) seg_list[first + i] = new_segs[i];
+    int run = warp_tot[warp] + incl - sum;
+    for (int i = 0; i < items; ++i)
+        if (first + i < n) {
+            const int v = a[first + i];
+            a[first + i] = run;
+            run += v;
+        }
+    __syncthreads();
+}
+
+template <bool GATHER>
+__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_binned_kernel(
+    const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
+    const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
+    unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
+    const int cap) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ MeshTile T;
+    __shared__ int warp_tot[IB_THREADS / 32];
+    int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point, padded pitches
+    int* new_segs = tile + 3 * cap;                                    // [SPREAD_SEG_LIST]
+    int* bin_start = new_segs + SPREAD_SEG_LIST;                       // [cap + 4] counts, then first slot of each bin
+    float4* rec = reinterpret_cast<float4*>(bin_start + ((cap + 4) & ~3));   // [3][BIN_CHUNK] sorted node records
+    const int2 range = __ldg(ranges + blockIdx.x);
+    const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true);
+    const float fmax = __uint_as_float(T.fmax_bits);
+    if (!(fmax > 0.f)) return;                                         // nothing to spread
+    if (T.enabled == 0 || !(fmax < 3.0e38f)) {
+        spread_direct(X, Y, Z, F, n0, n1, g, seg_mask, seg_list, seg_count, p);
+        return;
+    }
+    // |tile value| <= n_nodes max W max|F| 2^k < 2^30 and every product |W F 2^k| <= max|F| 2^k / 8 < 2^22
+    const int k = max(-100, min(100, min(29 - ilogbf(0.125f * (float)(n1 - n0) * fmax), 21 - ilogbf(0.125f * fmax))));
+    const float scale = ldexpf(1.0f, k), inv_scale = ldexpf(1.0f, -k);
+    const int p0 = T.p0, pp = T.pp, nword = pp * T.e[2];
+    for (int t = tid; t < nword; t += IB_THREADS) {
+        tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
+    }
+    const int nb0 = T.e[0] - 3, nb1 = T.e[1] - 3, nb2 = T.e[2] - 3, nbins = nb0 * nb1 * nb2;
+    const bool clipped = T.clipped != 0;
+    const int n_chunks = (n1 - n0 + BIN_CHUNK - 1) / BIN_CHUNK;
+    const int lane = tid & 31, warp = tid >> 5;
+    for (int c = 0; c < n_chunks; ++c) {
+        const int c0 = n0 + (int)((long)(n1 - n0) * c / n_chunks), c1 = n0 + (int)((long)(n1 - n0) * (c + 1) / n_chunks);
+        for (int b = tid; b <= nbins; b += IB_THREADS) bin_start[b] = 0;
+        __syncthreads();                                               // also: tile zeroed / previous chunk consumed
+        // ---- one node per thread: its bin, its rank inside the bin, its record
+        const bool have = c0 + tid < c1;
+        int bin = 0, rank = 0;
+        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0, r2 = r0;
+        if (have) {
+            const int m = c0 + tid;
+            const double x = X[m], y = Y[m], z = Z[m];
+            const float4 Fm = __ldg(F + m);
+            const double fx = floor(x), fy = floor(y), fz = floor(z);
+            const int bx = (int)fx - 1 - T.o[0], by = (int)fy - 1 - T.o[1], bz = (int)fz - 1 - T.o[2];
+            bin = (bz * nb1 + by) * nb0 + bx;
+            rank = atomicAdd(bin_start + bin, 1);
+            sincospif(0.5f * (float)(x - fx), &r0.x, &r0.y);
+            sincospif(0.5f * (float)(y - fy), &r0.z, &r0.w);
+            sincospif(0.5f * (float)(z - fz), &r1.x, &r1.y);
+            r1.z = Fm.x * scale; r1.w = Fm.y * scale; r2.x = Fm.z * scale;
+            r2.y = __int_as_float(bx);
+        }
+        __syncthreads();
+        block_exclusive_scan(bin_start, nbins, warp_tot);
+        if (have) {
+            const int slot = bin_start[bin] + rank;
+            rec[slot] = r0; rec[BIN_CHUNK + slot] = r1; rec[2 * BIN_CHUNK + slot] = r2;
+        }
+        __syncthreads();
+        if (!GATHER) {
+            // ---- one warp per occupied bin (32 bins examined at a time)
+            const int ox = lane & 3, oy = (lane >> 2) & 3, h = lane >> 4;
+            const float ax = (ox == 0 || ox == 3) ? -0.25f : 0.25f, ay = (oy == 0 || oy == 3) ? -0.25f : 0.25f;
+            const float az = h ? 0.25f : -0.25f;                       // oz = h: (0: 1/4 - s/4, 1: 1/4 + c/4); oz = h + 2: opposite sign
+            for (int b0 = warp * 32; b0 < nbins; b0 += IB_THREADS) {
+                const int bl = b0 + lane;
+                const int my_s = bl < nbins ? bin_start[bl] : 0, my_e = bl < nbins ? bin_start[bl + 1] : 0;
+                unsigned occupied = __ballot_sync(0xffffffffu, my_e > my_s);
+                while (occupied) {
+                    const int src = __ffs(occupied) - 1;
+                    occupied &= occupied - 1;
+                    const int js = __shfl_sync(0xffffffffu, my_s, src), je = __shfl_sync(0xffffffffu, my_e, src);
+                    const int b = b0 + src;
+                    const int bx = b % nb0, br = b / nb0;
+                    const int by = br % nb1, bz = br / nb1;
+                    int a0x = 0, a0y = 0, a0z = 0, a1x = 0, a1y = 0, a1z = 0;
+                    for (int j = js; j < je; ++j) {
+                        const float4 q0 = rec[j], q1 = rec[BIN_CHUNK + j];
+                        const float fzc = rec[2 * BIN_CHUNK + j].x;
+                        const float wx = fmaf(ax, (ox & 1) ? q0.y : q0.x, 0.25f);
+                        const float wy = fmaf(ay, (oy & 1) ? q0.w : q0.z, 0.25f);
+                        const float tz = h ? q1.y : q1.x;
+                        const float wlo = fmaf(az, tz, 0.25f), whi = fmaf(-az, tz, 0.25f);
+                        const float wxy = wx * wy;
+                        const float gx = wxy * q1.z, gy = wxy * q1.w, gz = wxy * fzc;
+                        a0x += __float_as_int(fmaf(wlo, gx, FIX_MAGIC));
+                        a0y += __float_as_int(fmaf(wlo, gy, FIX_MAGIC));
+                        a0z += __float_as_int(fmaf(wlo, gz, FIX_MAGIC));
+                        a1x += __float_as_int(fmaf(whi, gx, FIX_MAGIC));
+                        a1y += __float_as_int(fmaf(whi, gy, FIX_MAGIC));
+                        a1z += __float_as_int(fmaf(whi, gz, FIX_MAGIC));
+                    }
+                    const int bias = (je - js) * FIX_MAGIC_BITS;           // wraps; so did the sums
+                    const int tx = bx + ox, ty = by + oy, tz0 = bz + h, tz1 = bz + h + 2;
+                    if (clipped && (tx < T.lo[0] || tx >= T.hi[0] || ty < T.lo[1] || ty >= T.hi[1])) continue;
+                    const int t0 = tz0 * pp + ty * p0 + tx, t1 = t0 + 2 * pp;
+                    if (!clipped || (tz0 >= T.lo[2] && tz0 < T.hi[2])) {
+                        atomicAdd(tile + t0, a0x - bias);
+                        atomicAdd(tile + cap + t0, a0y - bias);
+                        atomicAdd(tile + 2 * cap + t0, a0z - bias);
+                    }
+                    if (!clipped || (tz1 >= T.lo[2] && tz1 < T.hi[2])) {
+                        atomicAdd(tile + t1, a1x - bias);
+                        atomicAdd(tile + cap + t1, a1y - bias);
+                        atomicAdd(tile + 2 * cap + t1, a1z - bias);
+                    }
+                }
+            }
+        } else {
+            // ---- one thread per tile cell: the bins (bx, by, bz) with cell - bin in {0..3}^3; the x-run
+            // of bins of one (by, bz) row is one run of sorted nodes
+            const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+            for (int t = tid; t < ncell; t += IB_THREADS) {
+                const int x = t % e0, r = t / e0;
+                const int y = r % e1, z = r / e1;
+                if (clipped && (x < T.lo[0] || x >= T.hi[0] || y < T.lo[1] || y >= T.hi[1] || z < T.lo[2] || z >= T.hi[2])) continue;
+                const int bx_lo = max(0, x - 3), bx_hi = min(nb0 - 1, x);
+                int ax_ = 0, ay_ = 0, az_ = 0, n_add = 0;
+                for (int bz = max(0, z - 3); bz <= min(nb2 - 1, z); ++bz)
+                    for (int by = max(0, y - 3); by <= min(nb1 - 1, y); ++by) {
+                        const int row = (bz * nb1 + by) * nb0;
+                        const int js = bin_start[row + bx_lo], je = bin_start[row + bx_hi + 1];
+                        const int oy = y - by, oz = z - bz;
+                        for (int j = js; j < je; ++j) {
+                            const float4 q0 = rec[j], q1 = rec[BIN_CHUNK + j], q2 = rec[2 * BIN_CHUNK + j];
+                            const int ox = x - __float_as_int(q2.y);
+                            const float wxy = weight_o(q0.x, q0.y, ox) * weight_o(q0.z, q0.w, oy);
+                            const float wz = weight_o(q1.x, q1.y, oz);
+                            ax_ += __float_as_int(fmaf(wz, wxy * q1.z, FIX_MAGIC));
+                            ay_ += __float_as_int(fmaf(wz, wxy * q1.w, FIX_MAGIC));
+                            az_ += __float_as_int(fmaf(wz, wxy * q2.x, FIX_MAGIC));
+                        }
+                        n_add += je - js;
+                    }
+                const int bias = n_add * FIX_MAGIC_BITS, w = z * pp + y * p0 + x;
+                tile[w] += ax_ - bias; tile[cap + w] += ay_ - bias; tile[2 * cap + w] += az_ - bias;
+            }
+        }
+        __syncthreads();                                               // bins and records consumed
+    }
+    spread_flush(T, tile, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
 // zero the cells of the segments the previous spread touched (its list), and drop their activity
@@ -499,6 +742,28 @@ __global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ 
         if (lane8 == 0) seg_mask[seg >> 5] = 0u;          // every set bit of the word is in the list
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) *count_next = 0;
+}
+
+// S4 pre-pass: (vx, vy, vz, rho) of the state after lbm_step for every cell of the 8-cell segments
+// the last ib_spread listed -- exactly the cells inside some node's stencil (plus the rounding to
+// aligned segments).  Eight adjacent lanes pull the 19 populations of eight adjacent cells: every
+// load instruction of the group reads one whole 32-byte sector of a population row, and the result
+// is one 128-byte line of the velocity field.  The interpolation kernel then fills its tile from
+// that field instead of gathering 19 scattered values per tile cell (whose 12-cell tile rows used
+// 2.4 x the sectors they needed).
+__global__ void __launch_bounds__(256, 4) segment_macros_kernel(const float* __restrict__ src, const float4* __restrict__ g,
+                                                             const int* __restrict__ seg_list, const int* __restrict__ seg_count,
+                                                             float4* __restrict__ vfield, const LbmParams p) {
+    const int n = *seg_count;
+    const int lane8 = threadIdx.x & (SEG - 1);
+    const int stride = gridDim.x * (256 / SEG);
+    for (int e = blockIdx.x * (256 / SEG) + (threadIdx.x >> SEG_SHIFT); e < n; e += stride) {
+        const int cell = __ldg(seg_list + e) * SEG + lane8;
+        if (cell >= p.cells) continue;
+        const Cell c = cell_of(cell, p);
+        const bool interior = c.i >= 1 && c.i <= p.nx - 2 && c.j >= 1 && c.j <= p.ny - 2 && c.k >= 1 && c.k <= p.nz - 2;
+        vfield[cell] = interior ? cell_macros_interior(src, g, p, cell) : cell_macros(src, g, p, c);
+    }
 }
 
 // one lane's column of the gather from the shared velocity tile
@@ -529,7 +794,8 @@ __device__ __forceinline__ void gather_column(const float4* __restrict__ tile, c
 __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mesh_kernel(
     double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z, float4* __restrict__ U,
     const int2* __restrict__ ranges, const float* __restrict__ src, const float4* __restrict__ g,
-    int* __restrict__ counters, const LbmParams p, const int cap) {
+    const float4* __restrict__ vfield, const unsigned* __restrict__ seg_mask, int* __restrict__ counters,
+    const LbmParams p, const int cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
     float4* tile = reinterpret_cast<float4*>(smem_raw);                // [cap] (vx, vy, vz, rho)
@@ -612,6 +878,9 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
         }
         __syncthreads();
         const int n_need = T.n_need;
+        // a cell of a segment the last spread listed has its velocity in the field already
+        // (segment_macros_kernel); any other cell -- a mesh without force, passive advection -- is
+        // computed here from its 19 pulled populations
         if (T.interior) {
             const int sy = p.nx, sz = p.nx * p.ny;
             const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
@@ -619,23 +888,30 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
                 const int t = list[e];
                 const int x = t % e0, r = t / e0;
                 const int y = r % e1, z = r / e1;
-                tile[t] = cell_macros_interior(src, g, p, origin + x + sy * y + sz * z);
+                const int cell = origin + x + sy * y + sz * z;
+                tile[t] = seg_active(seg_mask, cell) ? __ldg(vfield + cell) : cell_macros_interior(src, g, p, cell);
             }
         } else {
             for (int e = tid; e < n_need; e += IB_THREADS) {
                 const int t = list[e];
-                tile[t] = cell_macros(src, g, p, tile_cell(T, t, p));
+                const Cell c = tile_cell(T, t, p);
+                const int cell = c.i + p.nx * (c.j + p.ny * c.k);
+                tile[t] = seg_active(seg_mask, cell) ? __ldg(vfield + cell) : cell_macros(src, g, p, c);
             }
         }
         __syncthreads();
     }
     for (int mb = n0; mb < n1; mb += IB_GROUPS) {
+        // Lanes without a node take no part in the gather and read no position: another warp may
+        // already be writing the advanced position of node n1 - 1, and a stencil built from a moved
+        // node could leave the tile.  They still run the shuffles of node_stencil and the reduction.
         const bool valid = mb + group < n1;
         const int m = valid ? mb + group : n1 - 1;
-        const double x = node_coord(X, Y, Z, m, sub);
+        const double x = valid ? node_coord(X, Y, Z, m, sub) : 0.0;
         const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
         float ux = 0.f, uy = 0.f, uz = 0.f;
-        if (tiled) {
+        if (!valid) {
+        } else if (tiled) {
             if (T.clipped) gather_column<true>(tile, T, st, st.bx + sub, ux, uy, uz);
             else           gather_column<false>(tile, T, st, st.bx + sub, ux, uy, uz);
         } else {
@@ -685,16 +961,18 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
 }
 
 // positions: device SoA <-> AoS staging buffer (so host transfers are one contiguous copy)
+// (also stored order <-> caller's order)
 __global__ void __launch_bounds__(256) nodes_transpose_kernel(double* __restrict__ X, double* __restrict__ Y,
                                                               double* __restrict__ Z, double* __restrict__ aos,
-                                                              const long n, const bool to_aos) {
+                                                              const int* __restrict__ orig, const long n, const bool to_aos) {
     const long t = blockIdx.x * 256L + threadIdx.x;
     if (t >= 3 * n) return;
     const long m = t / 3;
     const int d = (int)(t - 3 * m);
     double* comp = d == 0 ? X : (d == 1 ? Y : Z);
-    if (to_aos) aos[t] = comp[m];
-    else        comp[m] = aos[t];
+    const long a = 3L * __ldg(orig + m) + d;
+    if (to_aos) aos[a] = comp[m];
+    else        comp[m] = aos[a];
 }
 
 __global__ void philox_kernel(const long n, const uint4* __restrict__ ctr, const uint2* __restrict__ key,
@@ -708,7 +986,7 @@ __global__ void philox_kernel(const long n, const uint4* __restrict__ ctr, const
 // ---------------------------------------------------------------------------------------------
 int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigned long long step) {
     if (c->n_nodes == 0) return PLB_OK;
-    force_init_kernel<<<(unsigned)((c->n_nodes + 255) / 256), 256, 0, c->stream>>>(c->F, c->n_nodes, sigma, seed,
+    force_init_kernel<<<(unsigned)((c->n_nodes + 255) / 256), 256, 0, c->stream>>>(c->F, c->orig, c->n_nodes, sigma, seed,
                                                                                   (unsigned)step);
     c->launches++;
     if (c->n_edges) {
@@ -739,7 +1017,19 @@ int launch_clear_spread(Ctx* c, float4* g) {
 }
 
 static size_t spread_smem(int cap) { return (size_t)cap * 12 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)SPREAD_CHUNK * 48; }
+static size_t binned_smem(int cap) {
+    return (size_t)cap * 12 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)((cap + 4) & ~3) * 4 + (size_t)BIN_CHUNK * 48;
+}
 static size_t interp_smem(int cap) { return (size_t)cap * 16 + (((size_t)cap * 2 + 15) & ~(size_t)15); }
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per kernel and size, not once per step
+template <typename K>
+static int ensure_smem(K kernel, size_t smem, size_t& granted, const char* what) {
+    if (smem <= granted) return PLB_OK;
+    const int rc = cuda_check(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), what);
+    if (!rc) granted = smem;
+    return rc;
+}
 
 // Largest tile (in cells) both kernels can hold with at least one block per SM; a tile cell index
 // must also fit the 16-bit entries of the interpolation's compact list.
@@ -752,28 +1042,63 @@ int ib_max_tile_cap() {
 // words per component of the padded spread tile: two blocks of 110 KB per SM
 int ib_max_spread_cap() { return (int)((90 * 1024) / 12); }
 
+// Which form of the spread runs: the caller's choice (ib_set_spread_mode), else by how densely the
+// tiles are sampled -- measured on the B200 (profiles/): the scatter form wins on sparsely sampled
+// tiles (config 4: 0.4 nodes per tile cell, 1.5 per occupied bin), the warp-aggregated form on
+// densely sampled ones (config 5: 0.9 per tile cell, 6 per occupied bin).
+int spread_mode_of(const Ctx* c) {
+    if (c->spread_mode != PLB_SPREAD_AUTO) return c->spread_mode;
+    return c->tile_density >= 0.6 ? PLB_SPREAD_AGGREGATE : PLB_SPREAD_SCATTER;
+}
+
 int launch_spread(Ctx* c, float4* g) {
     if (c->n_nodes == 0) return PLB_OK;
-    const size_t smem = spread_smem(c->spread_cap);
-    int rc = cuda_check(cudaFuncSetAttribute(spread_mesh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
-                        "cudaFuncSetAttribute(spread_mesh_kernel)");
-    if (rc) return rc;
-    spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, c->counters + 2 + c->list_parity, c->prm,
-        c->spread_cap);
+    static size_t granted_scatter = 0, granted_aggregate = 0, granted_gather = 0;
+    const int cap = (c->spread_cap + 3) & ~3;
+    int* seg_count = c->counters + 2 + c->list_parity;
+    const int mode = spread_mode_of(c);
+    int rc;
+    if (mode == PLB_SPREAD_SCATTER) {
+        const size_t smem = spread_smem(cap);
+        rc = ensure_smem(spread_mesh_kernel, smem, granted_scatter, "cudaFuncSetAttribute(spread_mesh_kernel)");
+        if (rc) return rc;
+        spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap);
+    } else if (mode == PLB_SPREAD_AGGREGATE) {
+        const size_t smem = binned_smem(cap);
+        rc = ensure_smem(spread_binned_kernel<false>, smem, granted_aggregate, "cudaFuncSetAttribute(spread_binned_kernel<false>)");
+        if (rc) return rc;
+        spread_binned_kernel<false><<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap);
+    } else {
+        const size_t smem = binned_smem(cap);
+        rc = ensure_smem(spread_binned_kernel<true>, smem, granted_gather, "cudaFuncSetAttribute(spread_binned_kernel<true>)");
+        if (rc) return rc;
+        spread_binned_kernel<true><<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap);
+    }
     c->launches++;
-    return cuda_check(cudaGetLastError(), "spread_mesh_kernel");
+    return cuda_check(cudaGetLastError(), "spread kernel");
 }
 
 int launch_interpolate_advance(Ctx* c) {
     if (c->n_nodes == 0) return PLB_OK;
+    static size_t granted = 0;
     const size_t smem = interp_smem(c->tile_cap);
-    int rc = cuda_check(cudaFuncSetAttribute(interpolate_mesh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
-                        "cudaFuncSetAttribute(interpolate_mesh_kernel)");
+    const int rc = ensure_smem(interpolate_mesh_kernel, smem, granted, "cudaFuncSetAttribute(interpolate_mesh_kernel)");
     if (rc) return rc;
     const float4* g = (c->g_last_mode == FORCE_NONE) ? nullptr : c->g_last;
+    // velocities of the listed segments first (the list of the last spread; empty before any)
+    {
+        const long want = (c->n_segs + 31) / 32;
+        const unsigned grid = (unsigned)(want < (long)c->sm_count * 16 ? (want > 0 ? want : 1) : (long)c->sm_count * 16);
+        segment_macros_kernel<<<grid, 256, 0, c->stream>>>(c->f[c->cur], g, c->seg_list, c->counters + 2 + c->list_parity,
+                                                           c->vfield, c->prm);
+        c->launches++;
+    }
     interpolate_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->f[c->cur], g, c->counters, c->prm, c->tile_cap);
+        c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->f[c->cur], g, c->vfield, c->seg_mask, c->counters, c->prm,
+        c->tile_cap);
     c->launches++;
     return cuda_check(cudaGetLastError(), "interpolate_mesh_kernel");
 }
@@ -781,7 +1106,7 @@ int launch_interpolate_advance(Ctx* c) {
 int launch_nodes_transpose(Ctx* c, bool to_aos) {
     if (c->n_nodes == 0) return PLB_OK;
     nodes_transpose_kernel<<<(unsigned)((3 * c->n_nodes + 255) / 256), 256, 0, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->stage, c->n_nodes, to_aos);
+        c->X[0], c->X[1], c->X[2], c->stage, c->orig, c->n_nodes, to_aos);
     c->launches++;
     return cuda_check(cudaGetLastError(), "nodes_transpose_kernel");
 }

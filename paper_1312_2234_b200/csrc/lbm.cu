@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(256) lbm_step_kernel(const float* __restrict__
 //  * c_x = 0 populations: one aligned 128-bit (V = 4) load;
 //  * c_x = +-1 populations: the aligned vector of the same V cells, shifted by one through the
 //    neighbouring lane (shfl), the lane at a warp / row edge fetching the one missing element;
-//  * stores are aligned vectors.  Rows on a bounce-back face take the generic per-cell path.
+//  * stores are aligned vectors.
 // ---------------------------------------------------------------------------------------------
 template <int V> struct Vec;
 template <> struct Vec<4> {
@@ -151,6 +151,14 @@ template <> struct Vec<2> {
     }
 };
 
+// Hecht-Harting closure of every column of a row that lies on an on-site velocity face
+template <int V, int COL>
+__device__ __forceinline__ void close_on_site_walls(float (&h)[Q][V], const int hy, const int hz, const LbmParams& p) {
+    if (hy) hecht_harting_close<1, V, COL>(h, hy, p.uw[1][hy < 0]);
+    if (hz) hecht_harting_close<2, V, COL>(h, hz, p.uw[2][hz < 0]);
+    if constexpr (COL + 1 < V) close_on_site_walls<V, COL + 1>(h, hy, hz, p);
+}
+
 template <int MODE, int V, int COL>
 __device__ __forceinline__ void collide_cols(float (&h)[Q][V], const float4 (&g4)[V], const bool forced,
                                              const float omega, const float pref) {
@@ -159,7 +167,13 @@ __device__ __forceinline__ void collide_cols(float (&h)[Q][V], const float4 (&g4
     if constexpr (COL + 1 < V) collide_cols<MODE, V, COL + 1>(h, g4, forced, omega, pref);
 }
 
-template <int MODE, int V, int THREADS, int MINB>
+// WALLS = false: y and z are periodic too (config 2); WALLS = true: rows on a y / z wall face are
+// handled in the same vector form.  A population whose source cell lies beyond a bounce-back face
+// is T_dbar of the SAME cell plus the moving-wall term: an aligned vector of row dbar with no x
+// shift; beyond an on-site velocity face it is "undetermined" (not loaded) and closed from the
+// others (Eq. 23-30) column by column.  The x shuffles run unconditionally; a bounced lane
+// ignores what they deliver (lanes of one row bounce together).
+template <int MODE, int V, int THREADS, int MINB, bool WALLS>
 __global__ void __launch_bounds__(THREADS, MINB) lbm_step_vec_kernel(const float* __restrict__ src, float* __restrict__ dst,
                                                                     const float4* __restrict__ g,
                                                                     const unsigned* __restrict__ seg_mask,
@@ -175,17 +189,22 @@ __global__ void __launch_bounds__(THREADS, MINB) lbm_step_vec_kernel(const float
     const int i0 = idx0 - (int)(row * (unsigned)nx);
     const int k = (int)(row / (unsigned)ny);
     const int j = (int)row - k * ny;
-    const bool wall_row = (p.wall[1] && (j == 0 || j == ny - 1)) || (p.wall[2] && (k == 0 || k == nz - 1));
     const size_t N = (size_t)p.cells;
+    const bool ylo = j == 0, yhi = j == ny - 1, zlo = k == 0, zhi = k == nz - 1;
+    const bool bylo = WALLS && p.wall[1] == PLB_WALL_BB && ylo, byhi = WALLS && p.wall[1] == PLB_WALL_BB && yhi;
+    const bool bzlo = WALLS && p.wall[2] == PLB_WALL_BB && zlo, bzhi = WALLS && p.wall[2] == PLB_WALL_BB && zhi;
+    // on-site velocity wall: face of this row, 0 = none, +1 = low, -1 = high
+    const int hy = (WALLS && p.wall[1] == PLB_WALL_HH) ? (ylo ? 1 : (yhi ? -1 : 0)) : 0;
+    const int hz = (WALLS && p.wall[2] == PLB_WALL_HH) ? (zlo ? 1 : (zhi ? -1 : 0)) : 0;
     float h[Q][V];
-    if (!__all_sync(FULL, wall_row)) {
+    {
         const int lane = threadIdx.x & 31;
         const bool first = lane == 0 || i0 == 0;          // cell i0 - 1 is not in the lane below
         const bool last = lane == 31 || i0 + V == nx;     // cell i0 + V is not in the lane above
         const int xm = i0 == 0 ? nx - 1 : -1;             // offset of cell i0 - 1 (periodic)
         const int xp = i0 + V == nx ? V - nx : V;         // offset of cell i0 + V (periodic)
-        const int dym = (j == 0 ? ny - 1 : -1) * nx, dyp = (j == ny - 1 ? 1 - ny : 1) * nx;
-        const int dzm = (k == 0 ? nz - 1 : -1) * nx * ny, dzp = (k == nz - 1 ? 1 - nz : 1) * nx * ny;
+        const int dym = (ylo ? ny - 1 : -1) * nx, dyp = (yhi ? 1 - ny : 1) * nx;
+        const int dzm = (zlo ? nz - 1 : -1) * nx * ny, dzp = (zhi ? 1 - nz : 1) * nx * ny;
 #pragma unroll
         for (int d = 0; d < Q; ++d) {
             const int cx = CX(d), cy = CY(d), cz = CZ(d);
@@ -194,37 +213,42 @@ __global__ void __launch_bounds__(THREADS, MINB) lbm_step_vec_kernel(const float
             if (cy == -1) off += dyp;
             if (cz == 1) off += dzm;
             if (cz == -1) off += dzp;
+            // bounce-back: z first, then y, so that y wins (corner rule: first wall axis in x, y, z order)
+            bool b = false;
+            float corr = 0.f;
+            if (WALLS) {
+                if (cz == 1 && bzlo) { b = true; corr = p.corr[2][0][d]; }
+                if (cz == -1 && bzhi) { b = true; corr = p.corr[2][1][d]; }
+                if (cy == 1 && bylo) { b = true; corr = p.corr[1][0][d]; }
+                if (cy == -1 && byhi) { b = true; corr = p.corr[1][1][d]; }
+            }
+            const bool undetermined = WALLS && ((cy != 0 && cy == hy) || (cz != 0 && cz == hz));
             const float* base = src + (size_t)d * N + (idx0 + off);
+            const float* from = (WALLS && b) ? src + (size_t)OPP(d) * N + idx0 : base;
             float a[V];
-            Vec<V>::load(base, a);
+#pragma unroll
+            for (int c = 0; c < V; ++c) a[c] = 0.f;
+            if (!undetermined) Vec<V>::load(from, a);
             if (cx == 0) {
 #pragma unroll
-                for (int c = 0; c < V; ++c) h[d][c] = a[c];
+                for (int c = 0; c < V; ++c) h[d][c] = a[c] + corr;
             } else if (cx == 1) {                         // f_d(i) = T_d(i - 1)
                 float prev = __shfl_up_sync(FULL, a[V - 1], 1);
-                if (first) prev = __ldg(base + xm);
-                h[d][0] = prev;
+                if (first && !b && !undetermined) prev = __ldg(base + xm);
+                h[d][0] = b ? a[0] + corr : prev;
 #pragma unroll
-                for (int c = 1; c < V; ++c) h[d][c] = a[c - 1];
+                for (int c = 1; c < V; ++c) h[d][c] = b ? a[c] + corr : a[c - 1];
             } else {                                      // f_d(i) = T_d(i + 1)
                 float next = __shfl_down_sync(FULL, a[0], 1);
-                if (last) next = __ldg(base + xp);
+                if (last && !b && !undetermined) next = __ldg(base + xp);
 #pragma unroll
-                for (int c = 0; c + 1 < V; ++c) h[d][c] = a[c + 1];
-                h[d][V - 1] = next;
+                for (int c = 0; c + 1 < V; ++c) h[d][c] = b ? a[c] + corr : a[c + 1];
+                h[d][V - 1] = b ? a[V - 1] + corr : next;
             }
         }
     }
     if (!live) return;
-    if (wall_row) {
-#pragma unroll 1
-        for (int c = 0; c < V; ++c) {
-            Cell cell;
-            cell.i = i0 + c; cell.j = j; cell.k = k;
-            step_one_cell<MODE>(src, dst, g, seg_mask, p, cell, idx0 + c);
-        }
-        return;
-    }
+    if (WALLS && (hy | hz)) close_on_site_walls<V, 0>(h, hy, hz, p);
     bool forced = false;
     float4 g4[V];
     if (MODE == FORCE_DENSE) forced = true;
@@ -364,16 +388,21 @@ __global__ void __launch_bounds__(256) read_populations_kernel(const float* __re
     for (int d = 0; d < Q; ++d) f[(size_t)d * p.cells + idx] = h[d][0] + WGT(d);
 }
 
-// debug aid: count the cells whose stored populations are not finite or whose
-// density 1 + sum_d h_d is not positive
+// debug aid: count the cells whose current state -- the 19 populations that
+// stream INTO the cell, what lbm_read_macros sees -- has a non-finite population or a density
+// rho = 1 + sum_d h_d (Eq. 17) that is not positive
 __global__ void __launch_bounds__(256) check_finite_kernel(const float* __restrict__ src, int* __restrict__ bad,
                                                            const LbmParams p) {
     const int idx = blockIdx.x * 256 + threadIdx.x;
     if (idx >= p.cells) return;
-    float sum = 0.f;
+    float h[Q][1];
+    pull19<1, 0>(src, p, cell_of(idx, p), idx, h);
+    bool finite = true;
 #pragma unroll
-    for (int d = 0; d < Q; ++d) sum += __ldg(src + (size_t)d * p.cells + idx);
-    if (!isfinite(sum) || !(1.0f + sum > 0.f)) atomicAdd(bad, 1);
+    for (int d = 0; d < Q; ++d) finite = finite && isfinite(h[d][0]);
+    float drho, jx, jy, jz;
+    moments<1, 0>(h, drho, jx, jy, jz);
+    if (!finite || !(1.0f + drho > 0.f)) atomicAdd(bad, 1);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -396,8 +425,11 @@ static void launch_step_mode(Ctx* c, const float* src, float* dst, const float4*
     const LbmParams& p = c->prm;
     if (p.nx % LBM_V == 0 && !p.wall[0]) {
         const unsigned nvec = (unsigned)p.cells / LBM_V;
-        lbm_step_vec_kernel<MODE, LBM_V, LBM_THREADS, LBM_MINB>
-            <<<(nvec + LBM_THREADS - 1) / LBM_THREADS, LBM_THREADS, 0, c->stream>>>(src, dst, g, c->seg_mask, p);
+        const unsigned grid = (nvec + LBM_THREADS - 1) / LBM_THREADS;
+        if (p.wall[1] || p.wall[2])
+            lbm_step_vec_kernel<MODE, LBM_V, LBM_THREADS, LBM_MINB, true><<<grid, LBM_THREADS, 0, c->stream>>>(src, dst, g, c->seg_mask, p);
+        else
+            lbm_step_vec_kernel<MODE, LBM_V, LBM_THREADS, LBM_MINB, false><<<grid, LBM_THREADS, 0, c->stream>>>(src, dst, g, c->seg_mask, p);
     } else {
         lbm_step_kernel<MODE><<<grid_cells(c), 256, 0, c->stream>>>(src, dst, g, c->seg_mask, p);
     }

@@ -57,17 +57,23 @@ struct MeshConstraint {
 // Pitches of the spread kernel's shared-memory tile (ib.cu): a row pitch = 4 (mod 8) words puts the
 // 4 x 4 cells one node touches per instruction (4 consecutive x in 4 rows) into 16 different banks.
 __host__ __device__ inline int tile_row_pitch(const int e0) { return e0 + ((4 - (e0 & 7)) & 7); }
-__host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e1) { return row_pitch * e1; }
+// A plane pitch = 8 (mod 16) words puts the second half-warp of the binned spread (same 4 x 4 cells,
+// two planes further) into the other 16 banks.
+__host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e1) {
+    const int r = row_pitch * e1;
+    return r + ((8 - (r & 15)) & 15);
+}
 
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 
 // status bits raised by kernels (sticky)
-enum { STATUS_NODE_LEFT = 1, STATUS_ZERO_EDGE = 2, STATUS_ADH_OVERFLOW = 4, STATUS_ADH_BAD_SITE = 8 };
+enum { STATUS_NODE_LEFT = 1, STATUS_ZERO_EDGE = 2, STATUS_ADH_BAD_SITE = 8 };
 
 // NEXT-4 (section 3.2 / 3.4.1): adhesion parameters as the kernels take them.  a = wall
 // axis, (t0, t1) the tangential axes in x, y, z order, (n0, n1) their sizes = the vWF site grid,
 // plane = position of the wall plane on axis a.  Decision arithmetic is fp64 (adhesion.cu).
-constexpr int ADH_MAX_CAND = 32;   // same-step formation candidates one site can list
+constexpr int ADH_MAX_PER_SITE = 32;        // bound on plb_adhesion.max_per_site = rounds of the arbitration
+constexpr int ADH_NO_OFFER = 0x7f7f7f7f;    // site_min of a site nobody offers to (memset 0x7f)
 struct AdhParams {
     int a, t0, t1, n0, n1, per0, per1, max_per_site;
     double plane, k_on0, k_off0, s, gamma, sigma, l_b, l_max, F0, tau_rep;
@@ -118,6 +124,7 @@ struct Ctx {
     unsigned* seg_mask;        // one bit per segment, (n_segs + 31) / 32 words
     int* counters;             // [1] status bits, [2], [3] lengths of the segment list (alternating)
     int* seg_list;             // segments the last spread marked (n_segs entries)
+    float4* vfield;            // (vx, vy, vz, rho) per cell, valid in the listed segments after segment_macros_kernel
     int list_parity;           // which counter the next spread appends to
     // meshes
     long cap_nodes, cap_edges, n_nodes, n_edges;
@@ -125,6 +132,9 @@ struct Ctx {
     float4* F;                 // nodal forces (Fx, Fy, Fz, 0)
     float4* U;                 // nodal velocities of the last interpolate
     double* stage;             // 3 * cap_nodes: AoS staging for ib_read_nodes / ib_write_nodes
+    int* orig;                 // caller's global index of each stored node (the stored order is internal)
+    std::vector<int> h_orig;   // the same on the host, and its inverse: h_stored[caller's index] = stored index
+    std::vector<int> h_stored;
     int2* edges;               // global node index pairs
     float2* edge_prm;          // (rest length, k)
     std::vector<long> mesh_node_off, mesh_edge_off;
@@ -139,6 +149,9 @@ struct Ctx {
     long n_ranges;
     int tile_cap;              // cells of the shared-memory lattice tile of the interpolation kernel
     int spread_cap;            // words per component of the (padded, bank-conflict-free) spread tile
+    int spread_mode;           // PLB_SPREAD_*: which form of the spread kernel runs (AUTO: by tile_density)
+    double tile_nodes, tile_cells;   // sums over the ranges at ib_add_meshes time: nodes, cells of their tiles
+    double tile_density;       // tile_nodes / tile_cells
     // NEXT-4: receptors and bonds (carved from the caller's adhesion workspace)
     bool adh_on;
     AdhParams adh;
@@ -146,8 +159,7 @@ struct Ctx {
     int* rec_node;             // global node of each receptor
     int4* bond;                // (bound, s0, s1, candidate site of the running update or -1)
     int* site_count;           // bonds per vWF site, n0 * n1
-    int* cand_n;               // same-step formation candidates per site
-    int* cand;                 // their receptor indices, ADH_MAX_CAND per site
+    int* site_min;             // lowest receptor index among the pending candidates of a site (ADH_NO_OFFER: none)
     // bookkeeping
     const float4* g_last;
     int g_last_mode;           // ForceMode used by the last lbm_step
@@ -174,6 +186,7 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
 void reference_area_volume(const double* xyz, int n_tris, const int* tris, float* S0, double* S0_tot, double* V0);
 int launch_clear_spread(Ctx* c, float4* g);
 int launch_spread(Ctx* c, float4* g);
+int spread_mode_of(const Ctx* c);
 int launch_interpolate_advance(Ctx* c);
 int ib_max_tile_cap();
 int ib_max_spread_cap();

@@ -41,7 +41,7 @@ def test_north_star_calls_present(plb):
 def test_workspace_bytes_host_only(plb):
     n1 = plb.lbm_workspace_bytes(32, 32, 64, 0, 0)
     cells = 32 * 32 * 64
-    assert n1 >= 2 * 19 * cells * 4          # two fp32 lattices; no velocity field is kept in HBM
+    assert n1 >= 2 * 19 * cells * 4 + 16 * cells   # two fp32 lattices + the (sparsely filled) node-velocity field
     n2 = plb.lbm_workspace_bytes(32, 32, 64, 1000, 3000)
     assert n2 >= n1 + 1000 * (24 + 32) + 3000 * 16
     assert n2 % 256 == 0
@@ -93,8 +93,9 @@ def test_product_does_not_import_oracle():
 def test_adhesion_workspace_bytes_host_only(plb):
     n = plb.ib_adhesion_workspace_bytes(64, 32, 48, 1, 10000)       # wall axis y: 64 x 48 vWF sites
     sites = 64 * 48
-    assert n >= 10000 * (4 + 16) + sites * (4 + 4 + 32 * 4) and n % 256 == 0
-    assert plb.ib_adhesion_workspace_bytes(64, 32, 48, 2, 0) >= 64 * 32 * (4 + 4 + 32 * 4)
+    # per receptor: node index + (bound, s0, s1, pending site); per site: bond count + lowest pending index
+    assert 10000 * (4 + 16) + sites * (4 + 4) <= n <= 10000 * (4 + 16) + sites * (4 + 4) + 4 * 256 and n % 256 == 0
+    assert plb.ib_adhesion_workspace_bytes(64, 32, 48, 2, 0) >= 64 * 32 * (4 + 4)
     with pytest.raises(plb.PlbError) as e:
         plb.ib_adhesion_workspace_bytes(64, 32, 48, 3, 10)
     assert e.value.code == plb.PLB_ERR_ARG

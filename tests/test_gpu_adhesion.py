@@ -36,15 +36,17 @@ def near_wall_cloud(rng, n, nx, nz, plane=-0.5):
     return np.stack([-3 + (nx + 6) * rng.random(n), plane + 0.02 + 0.9 * rng.random(n), -3 + (nz + 6) * rng.random(n)], axis=1)
 
 
+@pytest.mark.parametrize("n_rec,min_total,min_on", [(8000, 8000, 300), (20000, 20000, 500)])
 @pytest.mark.parametrize("kind,plane", [((0, 1, 0), -0.5), ((0, 2, 0), 0.0)])
-def test_bond_tables_are_bit_exact_over_many_updates(kind, plane):
-    """3000 nodes jittering near the wall (some across the periodic seams), 8000 receptors, 30
-    updates with the same positions on both sides: break, form, contention for the 4 places"""
+def test_bond_tables_are_bit_exact_over_many_updates(kind, plane, n_rec, min_total, min_on):
+    """3000 nodes jittering near the wall (some across the periodic seams), 8000 or 20,000
+    receptors (the larger case puts dozens of same-step candidates on one site), 30 updates with
+    the same positions on both sides: break, form, contention for the 4 places"""
     rng = np.random.default_rng(41)
     nx, nz = 24, 20
     xyz = near_wall_cloud(rng, 3000, nx, nz, plane)
     sim, ora = pair(xyz, nx=nx, nz=nz, kind=kind)
-    rec = rng.integers(0, 3000, size=8000)
+    rec = rng.integers(0, 3000, size=n_rec)
     sim.set_receptors(rec, PRM); ora.set_receptors(rec, PRM)
     total = 0
     for step in range(30):
@@ -56,7 +58,7 @@ def test_bond_tables_are_bit_exact_over_many_updates(kind, plane):
         xyz[:, 1] = np.clip(xyz[:, 1], plane + 0.01, None)
         sim.write_nodes(xyz); ora.write_nodes(xyz)
     on = bo[bo[:, 0] == 1]
-    assert total > 8000 and len(on) > 300                              # plenty of bonds formed and broke
+    assert total > min_total and len(on) > min_on                      # plenty of bonds formed and broke
     _, counts = np.unique((on[:, 1] % nx) + nx * (on[:, 2] % nz), return_counts=True)
     assert counts.max() == 4                                            # rule 2 was binding somewhere
     sim.close(); ora.close()
@@ -77,13 +79,13 @@ def test_contention_lowest_indices_win_and_overflow_is_reported():
     sim.adhesion_update(1, 9); ora.adhesion_update(1, 9)
     assert (sim.read_bonds() == ora.read_bonds()).all() and sim.read_bonds()[:4, 0].tolist() == [1, 1, 1, 1]
     sim.close(); ora.close()
-    # 40 same-step candidates for one site exceed the 32 the site's list holds: reported, not silent
+    # any number of same-step candidates for one site: 500 receptors on one node, 4 places
     sim, ora = pair(xyz)
-    sim.set_receptors(np.zeros(40, dtype=np.int32), prm)
-    sim.adhesion_update(1, 0)
-    with pytest.raises(plb.PlbError) as e:
-        sim.status()
-    assert e.value.code == plb.PLB_ERR_WORKSPACE
+    node = np.zeros(500, dtype=np.int32)
+    sim.set_receptors(node, prm); ora.set_receptors(node, prm)
+    sim.adhesion_update(1, 0); ora.adhesion_update(1, 0)
+    sim.status()
+    assert (sim.read_bonds() == ora.read_bonds()).all() and sim.read_bonds()[:, 0].tolist() == [1] * 4 + [0] * 496
     sim.close(); ora.close()
 
 
@@ -150,6 +152,28 @@ def test_call_order_and_arguments():
         sim.set_receptors([5], PRM)                             # node out of range
     assert e.value.code == plb.PLB_ERR_ARG
     sim.close(); ora.close()
+
+
+def test_bad_parameters_and_bad_bonds_are_refused():
+    """F0 > 0 needs tau_rep > 0 (F_rep would be 0/0); a bond to a site outside a non-periodic
+    tangential axis is refused before it reaches the device table"""
+    sim = plb.Simulation(12, 8, 10, 0.8, (1, 1, 0), max_nodes=2, max_edges=0)
+    sim.set_equilibrium()
+    sim.add_mesh(np.array([[3.0, 0.1, 3.0], [5.5, 2.0, 4.0]]), np.zeros((0, 2), dtype=np.int32))
+    with pytest.raises(plb.PlbError) as e:
+        sim.set_receptors([0, 1], dict(PRM, F0=1e-4, tau_rep=0.0))
+    assert e.value.code == plb.PLB_ERR_ARG
+    sim.set_receptors([0, 1], PRM)
+    ok = np.array([[1, 3, 3], [0, 0, 0]], dtype=np.int32)
+    sim.write_bonds(ok)
+    for bad in ([[1, -1, 3], [0, 0, 0]], [[1, 12, 3], [0, 0, 0]]):      # x is a wall axis here: sites 0..11 only
+        with pytest.raises(plb.PlbError) as e:
+            sim.write_bonds(np.array(bad, dtype=np.int32))
+        assert e.value.code == plb.PLB_ERR_ARG
+    assert (sim.read_bonds() == ok).all()                               # the table still holds the last good one
+    sim.adhesion_update(1, 0)
+    sim.status()
+    sim.close()
 
 
 def test_no_receptors_leaves_only_the_repulsion():

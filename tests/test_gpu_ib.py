@@ -121,12 +121,18 @@ def test_membrane_force_default_rest_lengths_and_zero_edge():
 
 
 # ------------------------------------------------------------------ O-6 spread
+SPREAD_FORMS = ["scatter", "aggregate", "gather"]
+
+
+@pytest.mark.parametrize("mode", SPREAD_FORMS)
 @pytest.mark.parametrize("kind", [(0, 0, 0), (0, 1, 0), (1, 1, 1)])
-def test_spread_matches_oracle(kind):
+def test_spread_matches_oracle(kind, mode):
     n = (37, 19, 23)
     X = scattered_nodes(n, kind, 400, 47)
     F = np.random.default_rng(53).standard_normal((400, 3))
     sim, ora = mesh_pair(n, kind, X, np.zeros((0, 2), dtype=np.int32), None, 0.0)
+    sim.set_spread_mode(mode)
+    assert sim.spread_mode() == plb.SPREAD_MODES[mode]
     sim.write_forces(F)
     ora.write_forces(F)
     sim.spread()
@@ -148,6 +154,91 @@ def test_spread_matches_oracle(kind):
     ora.write_forces(F)
     sim.spread()
     assert np.abs(pu.forcing_to_soa(sim) - ora.spread()).max() <= 2e-6
+
+
+@pytest.mark.parametrize("mode", SPREAD_FORMS)
+def test_spread_dense_meshes_all_forms(mode):
+    """Densely sampled tiles (config 5's shape: 2562 nodes on ~2700 tile cells, ~6 nodes per occupied
+    base cell): one platelet in the interior, one across the periodic x seam (unwrapped), one
+    poking through the y wall (clipped tile, dropped cells G15), one 12-node mesh (fixed-point
+    scale bounded by the single product, not by the node count) and one with zero force."""
+    n = (40, 24, 36)
+    kind = (0, 1, 0)
+    v4, e4, _ = wl.icosphere(4)
+    v0, e0, _ = wl.icosphere(0)
+    rng = np.random.default_rng(83)
+    sim = plb.Simulation(*n, 0.8, kind, max_nodes=4 * len(v4) + len(v0), max_edges=1)
+    ora = orc.Oracle(*n, 0.8, kind)
+    meshes = [v4 * (5.0, 5.0, 1.25) + (20.3, 12.1, 18.7),
+              v4 * (5.0, 1.25, 5.0) + (39.6 + 40.0, 11.0, 9.2),
+              v4 * (1.25, 5.0, 5.0) + (11.1, 2.2, 27.9),
+              v0 * (1.5, 1.5, 1.5) + (30.2, 18.4, 30.1),
+              v4 * (5.0, 5.0, 1.25) + (8.0, 17.0, 8.0)]
+    edges = np.zeros((0, 2), dtype=np.int32)
+    for x in meshes:
+        sim.add_mesh(x, edges, None, 0.0)
+        ora.add_mesh(x, edges, None, 0.0)
+    sim.set_spread_mode(mode)
+    F = rng.standard_normal((sim.n_nodes, 3)) * np.array([1.0, 0.3, 2.0])
+    F[-len(v4):] = 0.0
+    F[3 * len(v4)] *= 50.0                                     # one dominant nodal force in the tiny mesh
+    sim.write_forces(F)
+    ora.write_forces(F)
+    sim.spread()
+    g_g, g_o = pu.forcing_to_soa(sim), ora.spread()
+    scale = np.abs(g_o).max()
+    assert scale > 10.0
+    # a cell collects up to ~300 contributions, each rounded to the tile's fixed-point quantum
+    # q = (n/8) 2^-30 max|F| (DESIGN.md section 6): error ~ q sqrt(300/12) ~ 5 q, 40 q allowed;
+    # the fp32 products add ~300 x 6e-8 x |F W| on top
+    quantum = (len(v4) / 8.0) * 2.0 ** -29 * np.abs(F).max()
+    assert np.abs(g_g - g_o).max() <= 40 * quantum + 2e-6 * scale
+    # the forms agree with each other to a few quanta: same products, order-independent integer
+    # sums (the scatter form rounds a product twice, the binned forms once)
+    sim.set_spread_mode("scatter" if mode != "scatter" else "aggregate")
+    sim.write_forces(F)
+    sim.spread()
+    assert np.abs(pu.forcing_to_soa(sim) - g_g).max() <= 20 * quantum
+    sim.close(); ora.close()
+
+
+def test_spread_forms_are_reproducible():
+    """integer tile accumulation: two runs of the binned forms give identical bits although the
+    order of the nodes inside a base cell differs from launch to launch"""
+    w = wl.config5(n=32, grid_xz=4, layers=2, steps=1, subdiv=4)
+    sim = plb.Simulation.from_workload(w)
+    for mode in ("aggregate", "gather"):
+        sim.set_spread_mode(mode)
+        outs = []
+        for _ in range(3):
+            sim.compute_membrane_forces(1e-4, 5, 0)
+            sim.spread()
+            outs.append(sim.forcing.clone())
+        assert bool((outs[0] == outs[1]).all()) and bool((outs[0] == outs[2]).all())
+    sim.close()
+
+
+def test_node_order_is_hidden():
+    """the library stores the nodes of a mesh in its own (Morton) order; every call that names a
+    node speaks the caller's indices: positions, forces, velocities round-trip unchanged, and the
+    Philox force noise is keyed on the caller's global node index"""
+    w = wl.config3(nx=64, ny=32, nz=64, n_meshes=3, steps=1)
+    sim = plb.Simulation.from_workload(w)
+    X = w.mesh_xyz.reshape(-1, 3)
+    assert np.array_equal(sim.read_nodes(), X)
+    Y = X + np.random.default_rng(89).random(X.shape)
+    sim.write_nodes(Y)
+    assert np.array_equal(sim.read_nodes(), Y)
+    F = np.random.default_rng(97).standard_normal(X.shape).astype(np.float32)
+    sim.write_forces(F)
+    assert np.array_equal(sim.read_forces(), F)
+    sim.write_nodes(X)
+    sim.compute_membrane_forces(0.5, 1234, 7)                  # rest lengths = initial lengths: noise only
+    Fn = sim.read_forces().astype(np.float64)
+    for m in (0, 1, 641, 642, 1925):
+        z = 0.5 * np.asarray(orc.noise_normal3(1234, m, 7, 2))
+        assert np.abs(Fn[m] - z).max() <= 1e-5
+    sim.close()
 
 
 def test_spread_requires_forces_and_buffer():
@@ -190,6 +281,58 @@ def test_interpolate_advance_matches_oracle(kind):
     rho_o, u_o = ora.read_macros()
     assert np.abs(u_g.cpu().numpy() - u_o).max() <= 6e-7
     assert np.abs(rho_g.cpu().numpy() - rho_o).max() <= 6e-7
+
+
+def test_P13_passive_advection_across_the_seam():
+    """GPU twin of the oracle pin P13: lbm_step(NULL) -> ib_interpolate_advance with NO spread in
+    between (Eq. 33 alone).  A pre-stressed mesh in a uniform periodic flow translates rigidly by u0
+    per step, crosses the x seam with unwrapped coordinates, and keeps its spring forces."""
+    nx, ny, nz = 12, 10, 9
+    v, _, e = wl.icosphere(1)
+    x0 = 2.5 * v + np.array([nx - 3.0, 5.0, 4.5])
+    u0 = np.array([0.09, -0.02, 0.035])
+    rest = 0.9 * wl.edge_lengths(x0, e)
+    sim, ora = mesh_pair((nx, ny, nz), (0, 0, 0), x0, e, rest, 0.3)
+    uf = np.tile(u0[:, None], (1, nx * ny * nz))
+    sim.set_equilibrium(None, dev(uf)); ora.set_equilibrium(None, uf)
+    sim.compute_membrane_forces(); ora.compute_membrane_forces()
+    F0 = sim.read_forces().astype(np.float64)
+    assert np.abs(F0 - ora.read_forces()).max() <= 2e-6 * np.abs(F0).max()
+    for n in range(1, 61):
+        sim.step(None); sim.interpolate_advance()
+        ora.step(None); ora.interpolate_advance()
+    sim.status()
+    X = sim.read_nodes()
+    assert np.abs(X - (x0 + 60 * u0)).max() <= 60 * 2e-7          # fp32 velocities, fp64 positions
+    assert np.abs(X - ora.read_nodes()).max() <= 60 * 2e-7
+    assert np.abs(sim.read_node_velocities() - u0).max() <= 2e-7
+    assert X[:, 0].max() > nx + 2                                 # unwrapped storage (G17)
+    sim.compute_membrane_forces()
+    assert np.abs(sim.read_forces() - F0).max() <= 1e-5 * np.abs(F0).max()
+    sim.close(); ora.close()
+
+
+def test_release_forcing_forgets_the_buffers():
+    """ib_release_forcing clears what the last spread wrote and drops the pointers: the caller may
+    free the buffer, the next spread may go to another one, the macros see g = 0"""
+    w = wl.config1(steps=3)
+    sim, ora = pu.build_pair(w)
+    pu.run_pair(w, sim, ora, 3)
+    first = sim.forcing
+    assert float(first.abs().max()) > 0.0
+    plb.ib_release_forcing(sim.h)
+    assert float(first.abs().max()) == 0.0
+    sim.forcing = torch.zeros_like(first)
+    del first
+    _, u_g = sim.read_macros()                                   # g = 0 now: plain u = sum c f / rho
+    f = sim.read_populations().double()
+    c = torch.as_tensor(orc.lattice()[0], dtype=torch.float64, device=f.device)     # [19, 3]
+    u_plain = (c.t() @ f) / f.sum(0)
+    assert float((u_g.double() - u_plain).abs().max()) <= 2e-7
+    sim.coupled_step(); ora.coupled_step()
+    out = pu.compare(w, sim, ora)
+    assert out["dX"] <= 1e-6
+    sim.close(); ora.close()
 
 
 def test_node_leaving_channel_is_reported():

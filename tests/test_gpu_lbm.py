@@ -308,13 +308,18 @@ def test_check_finite_counts_broken_cells():
     clean = sim.read_populations().clone()
     for d, q, value in ((5, 100, float("nan")), (2, 1500, float("inf"))):
         f = clean.clone()
-        f[d, q] = value                                     # one stored slot -> exactly one cell
+        f[d, q] = value                                     # one population of one cell
         sim.write_populations(f)
         assert sim.check_finite() == 1
     f = clean.clone()
-    f[:, 16 * 12 * 5 + 16 * 6 + 8] = -1.0                   # an interior cell: its 19 values stream to 19 cells
+    f[:, 16 * 12 * 5 + 16 * 6 + 8] = -1.0                   # one cell with density -19: that cell, no other
     sim.write_populations(f)
-    assert sim.check_finite() == 19
+    assert sim.check_finite() == 1
+    f = clean.clone()
+    f[18, 7] = -2.0                                         # finite populations, density <= 0
+    f[18, 16 * 12 * 10 - 1] = -2.0                          # ... also in a wall-row cell
+    sim.write_populations(f)
+    assert sim.check_finite() == 2
     sim.write_populations(clean)
     assert sim.check_finite() == 0
     sim.close()
