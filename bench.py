@@ -43,6 +43,8 @@ def parse_args(argv=None):
     p.add_argument("--warmup", type=int, default=5)
     p.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--spread-mode", default="auto", choices=["auto", "scatter", "aggregate", "gather"],
+                   help="form of the S2 kernel (ib_set_spread_mode); auto = the library's own choice")
     p.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     p.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     p.add_argument("--dist-dry-run", action="store_true",
@@ -334,6 +336,8 @@ def run_ours(args):
     w = wl.config(args.config)
     sim = plb.Simulation.from_workload(w, device=str(device))
     coupled = w.n_meshes > 0
+    if coupled:
+        sim.set_spread_mode(args.spread_mode)
     K, W = args.steps, args.warmup
     ev = lambda: torch.cuda.Event(enable_timing=True)
 

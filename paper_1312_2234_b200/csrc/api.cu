@@ -53,8 +53,8 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     float4* F = w.take<float4>((size_t)max_nodes);
     float4* U = w.take<float4>((size_t)max_nodes);
     double* stage = w.take<double>((size_t)3 * max_nodes);
-    int2* edges = w.take<int2>((size_t)max_edges);
-    float2* eprm = w.take<float2>((size_t)max_edges);
+    int* csr_off = w.take<int>((size_t)2 * max_nodes + 2);
+    int2* csr_ent = w.take<int2>((size_t)2 * max_edges);
     int2* ranges = w.take<int2>((size_t)max_nodes);
     int* orig = w.take<int>((size_t)max_nodes);
     // a closed genus-0 triangulated surface of N nodes has 2N - 4 triangles and at least 4 nodes
@@ -67,7 +67,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
         c->f[0] = f0; c->f[1] = f1;
         c->seg_mask = seg_mask; c->counters = counters; c->seg_list = seg_list; c->vfield = vfield;
         c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
-        c->edges = edges; c->edge_prm = eprm; c->ranges = ranges; c->orig = orig;
+        c->csr_off = csr_off; c->csr_ent = csr_ent; c->ranges = ranges; c->orig = orig;
     }
     return w.off;
 }
@@ -106,6 +106,12 @@ static std::vector<int> morton_order(const double* xyz, int n) {
     for (int m = 0; m < n; ++m) ord[m] = m;
     std::sort(ord.begin(), ord.end(), [&](int a, int b) { return code[a] != code[b] ? code[a] < code[b] : a < b; });
     return ord;
+}
+
+static int __float_as_int_host(float f) {
+    int i;
+    memcpy(&i, &f, sizeof(i));
+    return i;
 }
 
 static int check_grid(const plb_grid* g, long* cells) {
@@ -249,6 +255,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->spread_current = false; c->forces_valid = false; c->populated = false;
     c->launches = 0;
     c->n_ranges = 0;
+    c->n_csr_off = 0; c->n_csr_ent = 0;
     c->n_tris = 0; c->n_cons = 0;
     c->adh_on = false; c->n_rec = 0;
     c->list_parity = 0;
@@ -374,6 +381,16 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
             return PLB_ERR_ARG;
         }
     }
+    if (!h_rest && n_meshes > 1 && n_edges > 0) {
+        // rest lengths = each mesh's own initial lengths: the meshes do not share one spring table
+        for (int s = 0; s < n_meshes; ++s) {
+            int id = 0;
+            const int rc = ib_add_meshes(ctx, 1, n_nodes, h_xyz + (size_t)3 * s * n_nodes, n_edges, h_edges, nullptr, k, &id);
+            if (rc) return rc;
+            if (s == 0 && out_first_mesh_id) *out_first_mesh_id = id;
+        }
+        return PLB_OK;
+    }
     const long add_nodes = (long)n_meshes * n_nodes, add_edges = (long)n_meshes * n_edges;
     if (ctx->n_nodes + add_nodes > ctx->cap_nodes || ctx->n_edges + add_edges > ctx->cap_edges) {
         set_error("ib_add_meshes: capacity exceeded (%ld/%ld nodes, %ld/%ld edges)", ctx->n_nodes + add_nodes,
@@ -402,32 +419,46 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
             for (int d = 0; d < 3; ++d) soa[(size_t)d * add_nodes + m] = h_xyz[3 * src + d];
             og[m] = (int)(ctx->n_nodes + src);
         }
-    // edges in stored indices, ordered by their lower end (orientation kept: R = X_b - X_a)
-    std::vector<int> eorder((size_t)n_edges);
-    for (int e = 0; e < n_edges; ++e) eorder[e] = e;
-    std::sort(eorder.begin(), eorder.end(), [&](int p, int q) {
-        const int ap = inv[h_edges[2 * p]], bp = inv[h_edges[2 * p + 1]], aq = inv[h_edges[2 * q]], bq = inv[h_edges[2 * q + 1]];
-        const int lp = ap < bp ? ap : bp, lq = aq < bq ? aq : bq, hp = ap < bp ? bp : ap, hq = aq < bq ? bq : aq;
-        return lp != lq ? lp < lq : (hp != hq ? hp < hq : p < q);
-    });
-    std::vector<int2> eg((size_t)add_edges);
-    std::vector<float2> ep((size_t)add_edges);
-    for (int s = 0; s < n_meshes; ++s) {
-        const long noff = ctx->n_nodes + (long)s * n_nodes;
-        const double* x = h_xyz + (size_t)3 * s * n_nodes;
-        for (int i = 0; i < n_edges; ++i) {
-            const int e = eorder[i];
+    // Spring table of the topology (S1 is a gather: every node sums over its incident edges), in
+    // stored local indices, ONE table for all meshes of the call: row i = the (neighbour, rest
+    // length) pairs of node i, neighbours ascending.  A call that repeats the previous call's
+    // topology, rest lengths and stiffness extends that group instead of adding a table.
+    std::vector<float> rest((size_t)n_edges);
+    for (int e = 0; e < n_edges; ++e) {
+        if (h_rest) rest[e] = h_rest[e];
+        else {
             const int a = h_edges[2 * e], b = h_edges[2 * e + 1];
-            float L;
-            if (h_rest) L = h_rest[e];
-            else {
-                double s2 = 0;
-                for (int d = 0; d < 3; ++d) s2 += (x[3 * b + d] - x[3 * a + d]) * (x[3 * b + d] - x[3 * a + d]);
-                L = (float)sqrt(s2);
-            }
-            eg[(size_t)s * n_edges + i] = make_int2((int)(noff + inv[a]), (int)(noff + inv[b]));
-            ep[(size_t)s * n_edges + i] = make_float2(L, k);
+            double s2 = 0;
+            for (int d = 0; d < 3; ++d) s2 += (h_xyz[3 * b + d] - h_xyz[3 * a + d]) * (h_xyz[3 * b + d] - h_xyz[3 * a + d]);
+            rest[e] = (float)sqrt(s2);
         }
+    }
+    bool extend = false;
+    if (!ctx->groups.empty()) {
+        const SpringGroupHost& last = ctx->group_src.back();
+        extend = last.nn == n_nodes && last.k == k && (int)last.rest.size() == n_edges &&
+                 std::equal(last.rest.begin(), last.rest.end(), rest.begin()) &&
+                 std::equal(last.edges.begin(), last.edges.end(), h_edges);
+    }
+    std::vector<int> off;
+    std::vector<int2> ent;
+    if (!extend) {
+        struct Half { int i, j; float L; };
+        std::vector<Half> half((size_t)2 * n_edges);
+        for (int e = 0; e < n_edges; ++e) {
+            const int a = inv[h_edges[2 * e]], b = inv[h_edges[2 * e + 1]];
+            half[2 * e] = Half{a, b, rest[e]};
+            half[2 * e + 1] = Half{b, a, rest[e]};
+        }
+        std::stable_sort(half.begin(), half.end(), [](const Half& p, const Half& q) { return p.i != q.i ? p.i < q.i : p.j < q.j; });
+        off.assign((size_t)n_nodes + 1, 0);
+        ent.resize(half.size());
+        for (size_t t = 0; t < half.size(); ++t) {
+            off[half[t].i + 1]++;
+            ent[t] = make_int2(half[t].j, __float_as_int_host(half[t].L));
+        }
+        for (int i = 0; i < n_nodes; ++i) off[i + 1] += off[i];
+        for (int i = 0; i <= n_nodes; ++i) off[i] += (int)ctx->n_csr_ent;      // rows index the global entry array
     }
     // Node ranges of the IB thread blocks: a mesh, cut into runs of consecutive stored nodes (=
     // surface patches) so that the IB kernels get about two blocks per SM even when there are few
@@ -494,15 +525,29 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
                                              cudaMemcpyHostToDevice, ctx->stream), "upload node order");
     if (!rc) rc = cuda_check(cudaMemsetAsync(ctx->F + ctx->n_nodes, 0, (size_t)add_nodes * sizeof(float4), ctx->stream), "clear forces");
     if (!rc) rc = cuda_check(cudaMemsetAsync(ctx->U + ctx->n_nodes, 0, (size_t)add_nodes * sizeof(float4), ctx->stream), "clear node velocities");
-    if (!rc && add_edges) {
-        rc = cuda_check(cudaMemcpyAsync(ctx->edges + ctx->n_edges, eg.data(), (size_t)add_edges * sizeof(int2),
-                                        cudaMemcpyHostToDevice, ctx->stream), "upload edges");
-        if (!rc) rc = cuda_check(cudaMemcpyAsync(ctx->edge_prm + ctx->n_edges, ep.data(), (size_t)add_edges * sizeof(float2),
-                                                 cudaMemcpyHostToDevice, ctx->stream), "upload edge parameters");
+    if (!rc && !extend) {
+        rc = cuda_check(cudaMemcpyAsync(ctx->csr_off + ctx->n_csr_off, off.data(), off.size() * sizeof(int),
+                                        cudaMemcpyHostToDevice, ctx->stream), "upload spring table rows");
+        if (!rc && !ent.empty())
+            rc = cuda_check(cudaMemcpyAsync(ctx->csr_ent + ctx->n_csr_ent, ent.data(), ent.size() * sizeof(int2),
+                                            cudaMemcpyHostToDevice, ctx->stream), "upload spring table");
     }
     if (!rc) rc = cuda_check(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
     if (rc) return rc;
     ctx->n_ranges += (long)rg.size();
+    if (extend) {
+        ctx->groups.back().n_meshes += n_meshes;
+    } else {
+        SpringGroup grp;
+        grp.node_first = (int)ctx->n_nodes; grp.n_meshes = n_meshes; grp.nn = n_nodes;
+        grp.off_first = (int)ctx->n_csr_off; grp.k = k;
+        ctx->groups.push_back(grp);
+        SpringGroupHost src;
+        src.nn = n_nodes; src.k = k; src.rest = rest; src.edges.assign(h_edges, h_edges + (size_t)2 * n_edges);
+        ctx->group_src.push_back(src);
+        ctx->n_csr_off += (long)off.size();
+        ctx->n_csr_ent += (long)ent.size();
+    }
     ctx->h_orig.insert(ctx->h_orig.end(), og.begin(), og.end());
     ctx->h_stored.resize(ctx->h_orig.size());
     for (long m = ctx->n_nodes; m < ctx->n_nodes + add_nodes; ++m) ctx->h_stored[ctx->h_orig[m]] = (int)m;

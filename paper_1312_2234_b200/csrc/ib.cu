@@ -10,16 +10,55 @@
 namespace plb {
 
 // ---------------------------------------------------------------------------------------------
-// S1: per-edge Hookean spring force (Eq. 2-3): e = k (|R| - L) R/|R| on node a, -e on node b.
-// R and |R| - L are formed in fp64 (positions reach ~1e3, lengths ~1, stretches ~1e-3), the
-// rest in fp32; two vector atomics per edge.
+// S1: Hookean spring forces (Eq. 2-3) as a GATHER: one thread per node sums
+//     F_i = sum_j k (|R| - L_ij) R/|R|,  R = X_j - X_i,  over its neighbours j
+// (the force on i of Eq. 3 with the sign of DESIGN.md G1; an edge is evaluated from both ends).
+// The topology is fixed and shared by all meshes of a group, so the (neighbour, rest length) table
+// is stored ONCE per topology (123 KB for a 2562-node platelet: it lives in L1/L2) and the kernel
+// streams only the positions and the forces: 24 B read + 16 B written per node instead of the
+// 12 B per edge + 2 x 16 B atomics of an edge-parallel scatter; no zero-fill pass, no atomics, a
+// fixed summation order (deterministic).  The hidden Morton order of the nodes keeps a node's
+// neighbours within a few sectors of it.
+// R and |R| - L are formed in fp64 (positions reach ~1e3, lengths ~1, stretches ~1e-3): 1/|R| is
+// an fp32 rsqrt refined by one Newton step in fp64 (error ~1e-13), not a division and a square
+// root.  Optional per-node noise (config 5): Box-Muller on Philox keyed on the caller's node index.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) force_init_kernel(float4* __restrict__ F, const int* __restrict__ orig, const long n,
-                                                         const float sigma, const unsigned long long seed,
-                                                         const unsigned step) {
-    const long m = blockIdx.x * 256L + threadIdx.x;
-    if (m >= n) return;
+__global__ void __launch_bounds__(256) node_force_kernel(const double* __restrict__ X, const double* __restrict__ Y,
+                                                         const double* __restrict__ Z, const int* __restrict__ orig,
+                                                         const int* __restrict__ csr_off, const int2* __restrict__ csr_ent,
+                                                         float4* __restrict__ F, const SpringGroup grp, const float sigma,
+                                                         const unsigned long long seed, const unsigned step,
+                                                         int* __restrict__ counters) {
+    const long t = blockIdx.x * 256L + threadIdx.x;
+    if (t >= (long)grp.n_meshes * grp.nn) return;
+    const int local = (int)(t % grp.nn);
+    const int base = grp.node_first + (int)(t - local);               // first node of this node's mesh
+    const int m = base + local;
+    const double xi = X[m], yi = Y[m], zi = Z[m];
     float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
+    const int e0 = __ldg(csr_off + grp.off_first + local), e1 = __ldg(csr_off + grp.off_first + local + 1);
+    for (int e = e0; e < e1; ++e) {
+        const int2 ent = __ldg(csr_ent + e);
+        const int j = base + ent.x;
+        const double rx = X[j] - xi, ry = Y[j] - yi, rz = Z[j] - zi;
+        const double l2 = rx * rx + ry * ry + rz * rz;
+        if (!(l2 > 0.0)) {
+            atomicOr(counters + 1, STATUS_ZERO_EDGE);
+            continue;
+        }
+        const float l2f = (float)l2;
+        double r;                                                     // 1/|R|
+        if (l2f > 1e-30f && l2f < 1e30f) {
+            r = (double)rsqrtf(l2f);
+            r = r * (1.5 - 0.5 * l2 * r * r);
+        } else {
+            r = 1.0 / sqrt(l2);
+        }
+        const float s = grp.k * (float)((l2 * r - (double)__int_as_float(ent.y)) * r);
+        f.x = fmaf(s, (float)rx, f.x);
+        f.y = fmaf(s, (float)ry, f.y);
+        f.z = fmaf(s, (float)rz, f.z);
+    }
     if (sigma > 0.f) {
         // Box-Muller on the four uniforms of counter (node, step, tag 2); the key is the caller's
         // global node index, not the stored one
@@ -28,33 +67,11 @@ __global__ void __launch_bounds__(256) force_init_kernel(float4* __restrict__ F,
         const float r2 = sqrtf(-2.0f * logf(uniform01(r.z)));
         float s1, c1;
         sincospif(2.0f * uniform01(r.y), &s1, &c1);
-        f.x = sigma * r0 * c1;
-        f.y = sigma * r0 * s1;
-        f.z = sigma * r2 * cospif(2.0f * uniform01(r.w));
+        f.x += sigma * r0 * c1;
+        f.y += sigma * r0 * s1;
+        f.z += sigma * r2 * cospif(2.0f * uniform01(r.w));
     }
     F[m] = f;
-}
-
-__global__ void __launch_bounds__(256) edge_force_kernel(const double* __restrict__ X, const double* __restrict__ Y,
-                                                         const double* __restrict__ Z, const int2* __restrict__ edges,
-                                                         const float2* __restrict__ prm, float4* __restrict__ F,
-                                                         const long n_edges, int* __restrict__ counters) {
-    const long e = blockIdx.x * 256L + threadIdx.x;
-    if (e >= n_edges) return;
-    const int2 ab = __ldg(edges + e);
-    const float2 Lk = __ldg(prm + e);
-    const double rx = __ldg(X + ab.y) - __ldg(X + ab.x);
-    const double ry = __ldg(Y + ab.y) - __ldg(Y + ab.x);
-    const double rz = __ldg(Z + ab.y) - __ldg(Z + ab.x);
-    const double l = sqrt(rx * rx + ry * ry + rz * rz);
-    if (!(l > 0.0)) {
-        atomicOr(counters + 1, STATUS_ZERO_EDGE);
-        return;
-    }
-    const float s = Lk.y * (float)((l - (double)Lk.x) / l);
-    const float ex = s * (float)rx, ey = s * (float)ry, ez = s * (float)rz;
-    atomicAdd(F + ab.x, make_float4(ex, ey, ez, 0.f));
-    atomicAdd(F + ab.y, make_float4(-ex, -ey, -ez, 0.f));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -986,12 +1003,10 @@ __global__ void philox_kernel(const long n, const uint4* __restrict__ ctr, const
 // ---------------------------------------------------------------------------------------------
 int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigned long long step) {
     if (c->n_nodes == 0) return PLB_OK;
-    force_init_kernel<<<(unsigned)((c->n_nodes + 255) / 256), 256, 0, c->stream>>>(c->F, c->orig, c->n_nodes, sigma, seed,
-                                                                                  (unsigned)step);
-    c->launches++;
-    if (c->n_edges) {
-        edge_force_kernel<<<(unsigned)((c->n_edges + 255) / 256), 256, 0, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->edges, c->edge_prm, c->F, c->n_edges, c->counters);
+    for (const SpringGroup& grp : c->groups) {                        // one launch per topology group
+        const long n = (long)grp.n_meshes * grp.nn;
+        node_force_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->orig, c->csr_off, c->csr_ent, c->F, grp, sigma, seed, (unsigned)step, c->counters);
         c->launches++;
     }
     if (c->n_cons) {

@@ -66,6 +66,18 @@ __host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e
 
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 
+// consecutive meshes that share one spring table: nodes [node_first, node_first + n_meshes * nn)
+struct SpringGroup {
+    int node_first, n_meshes, nn, off_first;
+    float k;
+};
+struct SpringGroupHost {
+    int nn;
+    float k;
+    std::vector<float> rest;
+    std::vector<int> edges;
+};
+
 // status bits raised by kernels (sticky)
 enum { STATUS_NODE_LEFT = 1, STATUS_ZERO_EDGE = 2, STATUS_ADH_BAD_SITE = 8 };
 
@@ -135,8 +147,12 @@ struct Ctx {
     int* orig;                 // caller's global index of each stored node (the stored order is internal)
     std::vector<int> h_orig;   // the same on the host, and its inverse: h_stored[caller's index] = stored index
     std::vector<int> h_stored;
-    int2* edges;               // global node index pairs
-    float2* edge_prm;          // (rest length, k)
+    // springs (Eq. 2-3): one table per topology, shared by all meshes of a group
+    int* csr_off;              // rows: first entry of each local node (+ one end entry per table), global entry indices
+    int2* csr_ent;             // entries: (neighbour's stored local index, rest length as float bits)
+    long n_csr_off, n_csr_ent;
+    std::vector<SpringGroup> groups;
+    std::vector<SpringGroupHost> group_src;   // what each group was built from (to recognise a repeat)
     std::vector<long> mesh_node_off, mesh_edge_off;
     // area / volume constraints (Eq. 4-5): triangles of the constrained meshes, mesh by mesh
     long cap_tris, n_tris;
