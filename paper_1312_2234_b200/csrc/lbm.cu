@@ -167,65 +167,71 @@ __device__ __forceinline__ void collide_cols(float (&h)[Q][V], const float4 (&g4
     if constexpr (COL + 1 < V) collide_cols<MODE, V, COL + 1>(h, g4, forced, omega, pref);
 }
 
-// WALLS = false: y and z are periodic too (config 2); WALLS = true: rows on a y / z wall face are
-// handled in the same vector form.  A population whose source cell lies beyond a bounce-back face
-// is T_dbar of the SAME cell plus the moving-wall term: an aligned vector of row dbar with no x
-// shift; beyond an on-site velocity face it is "undetermined" (not loaded) and closed from the
-// others (Eq. 23-30) column by column.  The x shuffles run unconditionally; a bounced lane
-// ignores what they deliver (lanes of one row bounce together).
-template <int MODE, int V, int THREADS, int MINB, bool WALLS>
-__global__ void __launch_bounds__(THREADS, MINB) lbm_step_vec_kernel(const float* __restrict__ src, float* __restrict__ dst,
-                                                                    const float4* __restrict__ g,
-                                                                    const unsigned* __restrict__ seg_mask,
-                                                                    const LbmParams p) {
+// Pull of the 19 populations of V consecutive cells of a row.  WALLS = false: the source rows
+// wrap periodically (interior rows, and every row of a fully periodic box).  WALLS = true: the
+// row may lie on a y / z wall face, handled in the same vector form: a population whose source
+// cell lies beyond a bounce-back face is T_dbar of the SAME cell plus the moving-wall term (an
+// aligned vector of row dbar with no x shift); beyond an on-site velocity face it is
+// "undetermined" (not loaded) and closed from the others (Eq. 23-30) column by column.  The x
+// shuffles run unconditionally; a bounced lane ignores what they deliver (lanes of one row
+// bounce together).  The kernel takes the WALLS = true form only in warps that hold a wall row,
+// so the interior keeps the branch-free schedule (19 independent vector loads in flight) that
+// reaches the copy bandwidth -- the all-rows general form cost 25 % at config 4 (measured).
+template <int V, bool WALLS>
+__device__ __forceinline__ void pull_rows(float (&h)[Q][V], const float* __restrict__ src, const LbmParams& p,
+                                          const int idx0, const int i0, const int j, const int k, const int hy,
+                                          const int hz) {
     constexpr unsigned FULL = 0xffffffffu;
     const int nx = p.nx, ny = p.ny, nz = p.nz;
-    const unsigned nvec = (unsigned)p.cells / V;
-    unsigned t = blockIdx.x * THREADS + threadIdx.x;
-    const bool live = t < nvec;
-    if (!live) t = nvec - 1;                            // keeps the lane for the shuffles below
-    const int idx0 = (int)(t * V);
-    const unsigned row = (unsigned)idx0 / (unsigned)nx;
-    const int i0 = idx0 - (int)(row * (unsigned)nx);
-    const int k = (int)(row / (unsigned)ny);
-    const int j = (int)row - k * ny;
     const size_t N = (size_t)p.cells;
     const bool ylo = j == 0, yhi = j == ny - 1, zlo = k == 0, zhi = k == nz - 1;
     const bool bylo = WALLS && p.wall[1] == PLB_WALL_BB && ylo, byhi = WALLS && p.wall[1] == PLB_WALL_BB && yhi;
     const bool bzlo = WALLS && p.wall[2] == PLB_WALL_BB && zlo, bzhi = WALLS && p.wall[2] == PLB_WALL_BB && zhi;
-    // on-site velocity wall: face of this row, 0 = none, +1 = low, -1 = high
-    const int hy = (WALLS && p.wall[1] == PLB_WALL_HH) ? (ylo ? 1 : (yhi ? -1 : 0)) : 0;
-    const int hz = (WALLS && p.wall[2] == PLB_WALL_HH) ? (zlo ? 1 : (zhi ? -1 : 0)) : 0;
-    float h[Q][V];
-    {
-        const int lane = threadIdx.x & 31;
-        const bool first = lane == 0 || i0 == 0;          // cell i0 - 1 is not in the lane below
-        const bool last = lane == 31 || i0 + V == nx;     // cell i0 + V is not in the lane above
-        const int xm = i0 == 0 ? nx - 1 : -1;             // offset of cell i0 - 1 (periodic)
-        const int xp = i0 + V == nx ? V - nx : V;         // offset of cell i0 + V (periodic)
-        const int dym = (ylo ? ny - 1 : -1) * nx, dyp = (yhi ? 1 - ny : 1) * nx;
-        const int dzm = (zlo ? nz - 1 : -1) * nx * ny, dzp = (zhi ? 1 - nz : 1) * nx * ny;
+    const int lane = threadIdx.x & 31;
+    const bool first = lane == 0 || i0 == 0;          // cell i0 - 1 is not in the lane below
+    const bool last = lane == 31 || i0 + V == nx;     // cell i0 + V is not in the lane above
+    const int xm = i0 == 0 ? nx - 1 : -1;             // offset of cell i0 - 1 (periodic)
+    const int xp = i0 + V == nx ? V - nx : V;         // offset of cell i0 + V (periodic)
+    const int dym = (ylo ? ny - 1 : -1) * nx, dyp = (yhi ? 1 - ny : 1) * nx;
+    const int dzm = (zlo ? nz - 1 : -1) * nx * ny, dzp = (zhi ? 1 - nz : 1) * nx * ny;
 #pragma unroll
-        for (int d = 0; d < Q; ++d) {
-            const int cx = CX(d), cy = CY(d), cz = CZ(d);
-            int off = 0;
-            if (cy == 1) off += dym;
-            if (cy == -1) off += dyp;
-            if (cz == 1) off += dzm;
-            if (cz == -1) off += dzp;
+    for (int d = 0; d < Q; ++d) {
+        const int cx = CX(d), cy = CY(d), cz = CZ(d);
+        int off = 0;
+        if (cy == 1) off += dym;
+        if (cy == -1) off += dyp;
+        if (cz == 1) off += dzm;
+        if (cz == -1) off += dzp;
+        const float* base = src + (size_t)d * N + (idx0 + off);
+        float a[V];
+        if constexpr (!WALLS) {
+            Vec<V>::load(base, a);
+            if (cx == 0) {
+#pragma unroll
+                for (int c = 0; c < V; ++c) h[d][c] = a[c];
+            } else if (cx == 1) {                         // f_d(i) = T_d(i - 1)
+                float prev = __shfl_up_sync(FULL, a[V - 1], 1);
+                if (first) prev = __ldg(base + xm);
+                h[d][0] = prev;
+#pragma unroll
+                for (int c = 1; c < V; ++c) h[d][c] = a[c - 1];
+            } else {                                      // f_d(i) = T_d(i + 1)
+                float next = __shfl_down_sync(FULL, a[0], 1);
+                if (last) next = __ldg(base + xp);
+#pragma unroll
+                for (int c = 0; c + 1 < V; ++c) h[d][c] = a[c + 1];
+                h[d][V - 1] = next;
+            }
+        } else {
             // bounce-back: z first, then y, so that y wins (corner rule: first wall axis in x, y, z order)
             bool b = false;
             float corr = 0.f;
-            if (WALLS) {
-                if (cz == 1 && bzlo) { b = true; corr = p.corr[2][0][d]; }
-                if (cz == -1 && bzhi) { b = true; corr = p.corr[2][1][d]; }
-                if (cy == 1 && bylo) { b = true; corr = p.corr[1][0][d]; }
-                if (cy == -1 && byhi) { b = true; corr = p.corr[1][1][d]; }
-            }
-            const bool undetermined = WALLS && ((cy != 0 && cy == hy) || (cz != 0 && cz == hz));
-            const float* base = src + (size_t)d * N + (idx0 + off);
-            const float* from = (WALLS && b) ? src + (size_t)OPP(d) * N + idx0 : base;
-            float a[V];
+            if (cz == 1 && bzlo) { b = true; corr = p.corr[2][0][d]; }
+            if (cz == -1 && bzhi) { b = true; corr = p.corr[2][1][d]; }
+            if (cy == 1 && bylo) { b = true; corr = p.corr[1][0][d]; }
+            if (cy == -1 && byhi) { b = true; corr = p.corr[1][1][d]; }
+            const bool undetermined = (cy != 0 && cy == hy) || (cz != 0 && cz == hz);
+            const float* from = b ? src + (size_t)OPP(d) * N + idx0 : base;
 #pragma unroll
             for (int c = 0; c < V; ++c) a[c] = 0.f;
             if (!undetermined) Vec<V>::load(from, a);
@@ -247,6 +253,33 @@ __global__ void __launch_bounds__(THREADS, MINB) lbm_step_vec_kernel(const float
             }
         }
     }
+}
+
+template <int MODE, int V, int THREADS, int MINB, bool WALLS>
+__global__ void __launch_bounds__(THREADS, MINB) lbm_step_vec_kernel(const float* __restrict__ src, float* __restrict__ dst,
+                                                                    const float4* __restrict__ g,
+                                                                    const unsigned* __restrict__ seg_mask,
+                                                                    const LbmParams p) {
+    constexpr unsigned FULL = 0xffffffffu;
+    const int nx = p.nx, ny = p.ny, nz = p.nz;
+    const unsigned nvec = (unsigned)p.cells / V;
+    unsigned t = blockIdx.x * THREADS + threadIdx.x;
+    const bool live = t < nvec;
+    if (!live) t = nvec - 1;                            // keeps the lane for the shuffles below
+    const int idx0 = (int)(t * V);
+    const unsigned row = (unsigned)idx0 / (unsigned)nx;
+    const int i0 = idx0 - (int)(row * (unsigned)nx);
+    const int k = (int)(row / (unsigned)ny);
+    const int j = (int)row - k * ny;
+    const size_t N = (size_t)p.cells;
+    const bool ylo = j == 0, yhi = j == ny - 1, zlo = k == 0, zhi = k == nz - 1;
+    // on-site velocity wall: face of this row, 0 = none, +1 = low, -1 = high
+    const int hy = (WALLS && p.wall[1] == PLB_WALL_HH) ? (ylo ? 1 : (yhi ? -1 : 0)) : 0;
+    const int hz = (WALLS && p.wall[2] == PLB_WALL_HH) ? (zlo ? 1 : (zhi ? -1 : 0)) : 0;
+    const bool wall_row = WALLS && ((p.wall[1] && (ylo || yhi)) || (p.wall[2] && (zlo || zhi)));
+    float h[Q][V];
+    if (WALLS && __any_sync(FULL, wall_row)) pull_rows<V, true>(h, src, p, idx0, i0, j, k, hy, hz);
+    else                                     pull_rows<V, false>(h, src, p, idx0, i0, j, k, 0, 0);
     if (!live) return;
     if (WALLS && (hy | hz)) close_on_site_walls<V, 0>(h, hy, hz, p);
     bool forced = false;

@@ -187,7 +187,7 @@ def test_spread_dense_meshes_all_forms(mode):
     sim.spread()
     g_g, g_o = pu.forcing_to_soa(sim), ora.spread()
     scale = np.abs(g_o).max()
-    assert scale > 10.0
+    assert scale > 1.0                                         # the field is not trivially small
     # a cell collects up to ~300 contributions, each rounded to the tile's fixed-point quantum
     # q = (n/8) 2^-30 max|F|: error ~ q sqrt(300/12) ~ 5 q, 40 q allowed;
     # the fp32 products add ~300 x 6e-8 x |F W| on top
@@ -203,18 +203,23 @@ def test_spread_dense_meshes_all_forms(mode):
 
 
 def test_spread_forms_are_reproducible():
-    """integer tile accumulation: two runs of the binned forms give identical bits although the
-    order of the nodes inside a base cell differs from launch to launch"""
+    """integer tile accumulation: the sum a block forms in its tile does not depend on the order
+    in which its nodes arrive, so repeated launches agree up to the order of the float adds with
+    which OVERLAPPING tiles (patches of one mesh, interpenetrating meshes) meet in the forcing
+    field: a few fp32 roundings of the cell value, and nothing at all where one tile owns a cell"""
     w = wl.config5(n=32, grid_xz=4, layers=2, steps=1, subdiv=4)
     sim = plb.Simulation.from_workload(w)
-    for mode in ("aggregate", "gather"):
+    for mode in SPREAD_FORMS:
         sim.set_spread_mode(mode)
         outs = []
         for _ in range(3):
             sim.compute_membrane_forces(1e-4, 5, 0)
             sim.spread()
             outs.append(sim.forcing.clone())
-        assert bool((outs[0] == outs[1]).all()) and bool((outs[0] == outs[2]).all())
+        scale = float(outs[0].abs().max())
+        assert scale > 0.0
+        for o in outs[1:]:
+            assert float((o - outs[0]).abs().max()) <= 8 * 6e-8 * scale
     sim.close()
 
 
