@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include "plb_internal.cuh"
@@ -57,6 +58,8 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
     int2* csr_ent = w.take<int2>((size_t)2 * max_edges);
     int2* ranges = w.take<int2>((size_t)max_nodes);
     int* orig = w.take<int>((size_t)max_nodes);
+    const long box_cap = max_nodes / 16 + 4096;
+    int* range_box = w.take<int>((size_t)8 * box_cap);
     // a closed genus-0 triangulated surface of N nodes has 2N - 4 triangles and at least 4 nodes
     int4* tris = w.take<int4>((size_t)2 * max_nodes);
     float* tri_S0 = w.take<float>((size_t)2 * max_nodes);
@@ -68,6 +71,7 @@ static size_t carve(Ctx* c, char* base, long cells, long n_segs, long max_nodes,
         c->seg_mask = seg_mask; c->counters = counters; c->seg_list = seg_list; c->vfield = vfield;
         c->X[0] = X0; c->X[1] = X1; c->X[2] = X2; c->F = F; c->U = U; c->stage = stage;
         c->csr_off = csr_off; c->csr_ent = csr_ent; c->ranges = ranges; c->orig = orig;
+        c->range_box = range_box; c->box_cap = (int)box_cap;
     }
     return w.off;
 }
@@ -262,6 +266,14 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->tile_cap = 512;
     c->spread_cap = 1024;
     c->spread_mode = PLB_SPREAD_AUTO;
+    c->interp_form = PLB_INTERP_AUTO;
+    if (const char* e = getenv("PLB_INTERP")) {                         // measurement knob
+        if (!strcmp(e, "direct")) c->interp_form = PLB_INTERP_DIRECT;
+        if (!strcmp(e, "tile")) c->interp_form = PLB_INTERP_TILE;
+        if (!strcmp(e, "general")) c->interp_form = PLB_INTERP_GENERAL;
+    }
+    c->range_nodes = 0;
+    if (const char* e = getenv("PLB_RANGE_NODES")) c->range_nodes = atoi(e);   // measurement knob: nodes per IB block
     c->tile_nodes = 0.0; c->tile_cells = 0.0; c->tile_density = 0.0;
     c->sm_count = sms;
     c->mesh_node_off.push_back(0);
@@ -288,6 +300,8 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     }
     rc = cuda_check(cudaMemsetAsync(c->seg_mask, 0, (size_t)((n_segs + 31) / 32) * sizeof(unsigned), c->stream), "clear segment mask");
     if (!rc) rc = cuda_check(cudaMemsetAsync(c->counters, 0, 64 * sizeof(int), c->stream), "clear counters");
+    // the velocity field only ever holds what segment_macros_kernel wrote; start it from finite values
+    if (!rc) rc = cuda_check(cudaMemsetAsync(c->vfield, 0, (size_t)n_segs * SEG * sizeof(float4), c->stream), "clear velocity field");
     if (rc) {
         delete c;
         return rc;
@@ -469,6 +483,7 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
     const long meshes_after = (long)ctx->mesh_node_off.size() - 1 + n_meshes;
     long parts = (2L * ctx->sm_count + meshes_after - 1) / meshes_after;
     if (parts > n_nodes / IB_MIN_RANGE_NODES) parts = n_nodes / IB_MIN_RANGE_NODES;
+    if (ctx->range_nodes > 0) parts = (n_nodes + ctx->range_nodes - 1) / ctx->range_nodes;
     if (parts < (n_nodes + IB_RANGE_NODES - 1) / IB_RANGE_NODES) parts = (n_nodes + IB_RANGE_NODES - 1) / IB_RANGE_NODES;
     if (parts < 1) parts = 1;
     std::vector<int2> rg;

@@ -23,7 +23,10 @@ namespace plb {
 // an fp32 rsqrt refined by one Newton step in fp64 (error ~1e-13), not a division and a square
 // root.  Optional per-node noise (config 5): Box-Muller on Philox keyed on the caller's node index.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) node_force_kernel(const double* __restrict__ X, const double* __restrict__ Y,
+#ifndef PLB_FORCE_MINB
+#define PLB_FORCE_MINB 5
+#endif
+__global__ void __launch_bounds__(256, PLB_FORCE_MINB) node_force_kernel(const double* __restrict__ X, const double* __restrict__ Y,
                                                          const double* __restrict__ Z, const int* __restrict__ orig,
                                                          const int* __restrict__ csr_off, const int2* __restrict__ csr_ent,
                                                          float4* __restrict__ F, const SpringGroup grp, const float sigma,
@@ -37,6 +40,8 @@ __global__ void __launch_bounds__(256) node_force_kernel(const double* __restric
     const double xi = X[m], yi = Y[m], zi = Z[m];
     float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
     const int e0 = __ldg(csr_off + grp.off_first + local), e1 = __ldg(csr_off + grp.off_first + local + 1);
+    // (one neighbour at a time: batching the loads of a node's 6 neighbours -- 64 to 96 registers --
+    // cost more in occupancy than it gained in latency: 0.64 to 1.08 ms against 0.61 ms at config 5)
     for (int e = e0; e < e1; ++e) {
         const int2 ent = __ldg(csr_ent + e);
         const int j = base + ent.x;
@@ -231,11 +236,44 @@ __device__ __forceinline__ void mark_segment(const int cell, unsigned* __restric
     }
 }
 
+// tile geometry from the box T.mn, T.mx of floor(X) over the range (one thread)
+__device__ __forceinline__ void tile_geometry(MeshTile& T, const bool nonempty, const LbmParams& p, const int cap,
+                                              const bool padded) {
+    const int n[3] = {p.nx, p.ny, p.nz};
+    long long vol = 1;
+    bool ok = nonempty, clipped = false, interior = true;
+    for (int a = 0; a < 3; ++a) {
+        const long long ext = (long long)T.mx[a] - (long long)T.mn[a] + 4;
+        ok = ok && ext <= (long long)cap;
+        T.o[a] = T.mn[a] - 1;
+        T.e[a] = ok ? (int)ext : 1;
+        vol *= T.e[a];
+        ok = ok && vol <= (long long)cap;
+        if (p.wall[a] && ok) {
+            const long long lo = -(long long)T.o[a], hi = (long long)n[a] - (long long)T.o[a];
+            T.lo[a] = (int)max(0LL, min(lo, ext));
+            T.hi[a] = (int)max(0LL, min(hi, ext));
+        } else {
+            T.lo[a] = 0; T.hi[a] = T.e[a];
+        }
+        clipped = clipped || T.lo[a] != 0 || T.hi[a] != T.e[a];
+        interior = interior && (long long)T.o[a] >= 1 && (long long)T.o[a] + ext <= (long long)n[a] - 1;
+    }
+    T.p0 = padded ? tile_row_pitch(T.e[0]) : T.e[0];
+    T.pp = padded ? tile_plane_pitch(T.p0, T.e[1]) : T.e[0] * T.e[1];
+    ok = ok && (long long)T.pp * T.e[2] <= (long long)cap;
+    T.enabled = ok ? 1 : 0;
+    T.clipped = clipped ? 1 : 0;
+    T.interior = (ok && interior) ? 1 : 0;
+}
+
 // bounding box of the supports of nodes [n0, n1) -> tile geometry (all threads of the block);
-// with F != nullptr also the largest force component of the range
+// with F != nullptr also the largest force component of the range; with box_out != nullptr the box
+// is also stored (8 ints) for the interpolation of the same positions
 __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict__ X, const double* __restrict__ Y,
                                            const double* __restrict__ Z, const float4* __restrict__ F, const int n0,
-                                           const int n1, const LbmParams& p, const int cap, const bool padded) {
+                                           const int n1, const LbmParams& p, const int cap, const bool padded,
+                                           int* __restrict__ box_out = nullptr) {
     if (threadIdx.x == 0) {
         for (int a = 0; a < 3; ++a) { T.mn[a] = INT_MAX; T.mx[a] = INT_MIN; }
         T.fmax_bits = 0u;
@@ -266,32 +304,11 @@ __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        const int n[3] = {p.nx, p.ny, p.nz};
-        long long vol = 1;
-        bool ok = n1 > n0, clipped = false, interior = true;
-        for (int a = 0; a < 3; ++a) {
-            const long long ext = (long long)T.mx[a] - (long long)T.mn[a] + 4;
-            ok = ok && ext <= (long long)cap;
-            T.o[a] = T.mn[a] - 1;
-            T.e[a] = ok ? (int)ext : 1;
-            vol *= T.e[a];
-            ok = ok && vol <= (long long)cap;
-            if (p.wall[a] && ok) {
-                const long long lo = -(long long)T.o[a], hi = (long long)n[a] - (long long)T.o[a];
-                T.lo[a] = (int)max(0LL, min(lo, ext));
-                T.hi[a] = (int)max(0LL, min(hi, ext));
-            } else {
-                T.lo[a] = 0; T.hi[a] = T.e[a];
-            }
-            clipped = clipped || T.lo[a] != 0 || T.hi[a] != T.e[a];
-            interior = interior && (long long)T.o[a] >= 1 && (long long)T.o[a] + ext <= (long long)n[a] - 1;
+        if (box_out) {
+            box_out[0] = T.mn[0]; box_out[1] = T.mn[1]; box_out[2] = T.mn[2]; box_out[3] = n1 > n0 ? 1 : 0;
+            box_out[4] = T.mx[0]; box_out[5] = T.mx[1]; box_out[6] = T.mx[2]; box_out[7] = 0;
         }
-        T.p0 = padded ? tile_row_pitch(T.e[0]) : T.e[0];
-        T.pp = padded ? tile_plane_pitch(T.p0, T.e[1]) : T.e[0] * T.e[1];
-        ok = ok && (long long)T.pp * T.e[2] <= (long long)cap;
-        T.enabled = ok ? 1 : 0;
-        T.clipped = clipped ? 1 : 0;
-        T.interior = (ok && interior) ? 1 : 0;
+        tile_geometry(T, n1 > n0, p, cap, padded);
     }
     __syncthreads();
 }
@@ -392,33 +409,71 @@ __device__ __forceinline__ void spread_record(const SpreadChunk& ch, const int r
     ch.f[r] = F.x * scale; ch.f[SPREAD_CHUNK + r] = F.y * scale; ch.f[2 * SPREAD_CHUNK + r] = F.z * scale;
 }
 
+// Touched cells: a tile cell inside some node's stencil is LISTED (its segment marked) whatever its
+// value, so that after ib_spread the segment list covers every cell the interpolation of the same
+// positions will read -- also where the force is zero or rounds to zero.  Every node sets ONE bit,
+// that of its base cell, in a bitmap with one 32-bit x-mask per (y, z) tile row; before the flush
+// the bitmap is dilated by the 4 x 4 x 4 stencil (x by shifts, y and z by OR-ing 16 rows), one
+// thread per row.  Tiles wider than 32 cells count every cell as touched.
+__device__ __forceinline__ void touch_base(unsigned* __restrict__ binrow, const MeshTile& T, const int bx, const int by,
+                                           const int bz) {
+    unsigned* row = binrow + bz * T.e[1] + by;
+    const unsigned bit = 1u << bx;
+    if ((*(volatile unsigned*)row & bit) == 0u) atomicOr(row, bit);
+}
+// x cells of a tile row that lie on the lattice
+__device__ __forceinline__ unsigned tile_exist_mask(const MeshTile& T) {
+    const unsigned below_hi = T.hi[0] >= 32 ? 0xffffffffu : ((1u << T.hi[0]) - 1u);
+    const unsigned below_lo = T.lo[0] >= 32 ? 0xffffffffu : ((1u << T.lo[0]) - 1u);
+    return below_hi & ~below_lo;
+}
+// all threads of the block, after a __syncthreads(); followed by one
+__device__ __forceinline__ void dilate_rows(const unsigned* __restrict__ binrow, unsigned* __restrict__ rowmask,
+                                            const MeshTile& T) {
+    const int e1 = T.e[1], e2 = T.e[2];
+    const unsigned exist = tile_exist_mask(T);
+    for (int r = threadIdx.x; r < e1 * e2; r += IB_THREADS) {
+        const int y = r % e1, z = r / e1;
+        unsigned m = 0u;
+        if (y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]) {
+            for (int bz = max(0, z - 3); bz <= z; ++bz)
+                for (int by = max(0, y - 3); by <= y; ++by) m |= binrow[bz * e1 + by];
+            m = (m | (m << 1) | (m << 2) | (m << 3)) & exist;
+        }
+        rowmask[r] = m;
+    }
+}
+
 // Flush of a spread tile: one vector RED per non-zero tile cell.  The segments this block is the
 // first to mark are collected in shared memory and appended to the global list with ONE atomicAdd
 // per block (a returning atomic per segment on the single list counter was 58 % of the scatter
 // kernel's stall samples).  All threads of the block call it, after a __syncthreads().
-__device__ __forceinline__ void spread_flush(MeshTile& T, const int* __restrict__ tile, int* __restrict__ new_segs,
-                                             const int cap, const float inv_scale, float4* __restrict__ g,
-                                             unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
-                                             int* __restrict__ seg_count, const LbmParams& p) {
+__device__ __forceinline__ void spread_flush(MeshTile& T, const int* __restrict__ tile, const unsigned* __restrict__ rowmask,
+                                             int* __restrict__ new_segs, const int cap, const float inv_scale,
+                                             float4* __restrict__ g, unsigned* __restrict__ seg_mask,
+                                             int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams& p) {
     const int tid = threadIdx.x;
     const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+    const bool by_rows = e0 <= 32;
     for (int t = tid; t < ncell; t += IB_THREADS) {
         const int x = t % e0, r = t / e0;
         const int y = r % e1, z = r / e1;
+        const bool touched = by_rows ? ((rowmask[r] >> x) & 1u) != 0u
+                                     : (x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]);
+        if (!touched) continue;
         const int w = z * T.pp + y * T.p0 + x;
         const int qx = tile[w], qy = tile[cap + w], qz = tile[2 * cap + w];
-        if ((qx | qy | qz) != 0) {
-            const Cell c = tile_cell(T, t, p);
-            const int cell = c.i + p.nx * (c.j + p.ny * c.k);
+        const Cell c = tile_cell(T, t, p);
+        const int cell = c.i + p.nx * (c.j + p.ny * c.k);
+        if ((qx | qy | qz) != 0)
             atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
-            const int seg = cell >> SEG_SHIFT;
-            const unsigned bit = 1u << (seg & 31);
-            unsigned* word = seg_mask + (seg >> 5);
-            if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u) {
-                const int slot = atomicAdd(&T.n_need, 1);               // n_need doubles as the block's list length
-                if (slot < SPREAD_SEG_LIST) new_segs[slot] = seg;
-                else seg_list[atomicAdd(seg_count, 1)] = seg;          // list full: append directly
-            }
+        const int seg = cell >> SEG_SHIFT;
+        const unsigned bit = 1u << (seg & 31);
+        unsigned* word = seg_mask + (seg >> 5);
+        if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u) {
+            const int slot = atomicAdd(&T.n_need, 1);                   // n_need doubles as the block's list length
+            if (slot < SPREAD_SEG_LIST) new_segs[slot] = seg;
+            else seg_list[atomicAdd(seg_count, 1)] = seg;              // list full: append directly
         }
     }
     __syncthreads();
@@ -434,7 +489,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
-    const int cap) {
+    const int cap, int* __restrict__ range_box, const int box_cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
     int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point, padded pitches
@@ -443,19 +498,24 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     ch.b = new_segs + SPREAD_SEG_LIST;
     ch.sc = reinterpret_cast<float*>(ch.b + 3 * SPREAD_CHUNK);
     ch.f = ch.sc + 6 * SPREAD_CHUNK;
+    unsigned* binrow = reinterpret_cast<unsigned*>(ch.f + 3 * SPREAD_CHUNK);    // [cap / 4] occupied base cells, x-mask per tile row
+    unsigned* rowmask = binrow + cap / 4;                              // [cap / 4] touched cells, x-mask per tile row
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true);
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
-    if (!(fmax > 0.f)) return;                                         // nothing to spread
     const bool tiled = T.enabled != 0 && fmax < 3.0e38f;
     const int nword = tiled ? T.pp * T.e[2] : 0;
     // |tile value| <= n_nodes * max W * max|F| = bound; scale = 2^k with bound * scale < 2^30
-    const int k = max(-100, min(100, 29 - ilogbf(0.125f * (float)(n1 - n0) * fmax)));
+    // (a range without force still runs: its cells are listed for the interpolation)
+    const int k = fmax > 0.f ? max(-100, min(100, 29 - ilogbf(0.125f * (float)(n1 - n0) * fmax))) : 0;
     const float scale = tiled ? ldexpf(1.0f, k) : 1.0f, inv_scale = ldexpf(1.0f, -k);
     for (int t = tid; t < nword; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
+    const bool by_rows = tiled && T.e[0] <= 32;
+    if (by_rows)
+        for (int t = tid; t < T.e[1] * T.e[2]; t += IB_THREADS) binrow[t] = 0u;
     const int sub = tid & (SPREAD_LANES - 1), ox = sub & 3, oy = sub >> 2, group = tid / SPREAD_LANES;
     const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
     const int p0 = T.p0, pp = T.pp;
@@ -467,7 +527,10 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     if (have) { px = X[n0 + tid]; py = Y[n0 + tid]; pz = Z[n0 + tid]; pF = __ldg(F + n0 + tid); }
     for (int c0 = n0; c0 < n1; c0 += SPREAD_CHUNK) {
         __syncthreads();                                               // tile zeroed / previous chunk consumed
-        if (have) spread_record(ch, tid, px, py, pz, pF, scale, o0, o1, o2);
+        if (have) {
+            spread_record(ch, tid, px, py, pz, pF, scale, o0, o1, o2);
+            if (by_rows) touch_base(binrow, T, ch.b[tid], ch.b[SPREAD_CHUNK + tid], ch.b[2 * SPREAD_CHUNK + tid]);
+        }
         __syncthreads();
         const int m_next = c0 + SPREAD_CHUNK + tid;
         have = tid < SPREAD_CHUNK && m_next < n1;
@@ -508,24 +571,33 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     }
     if (!tiled) return;
     __syncthreads();
-    spread_flush(T, tile, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
+    if (by_rows) {
+        dilate_rows(binrow, rowmask, T);
+        __syncthreads();
+    }
+    spread_flush(T, tile, rowmask, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
 // ---------------------------------------------------------------------------------------------
-// S2, BINNED forms (north_star: "gather-by-cell over Morton-sorted nodes or warp-aggregated
-// atomics, whichever the counters favour"; the paper's own fluid3d_force_distribute_kernel is
-// gather-shaped, L356-362).  The nodes of a chunk are counting-sorted in shared memory by their
-// base cell b = floor(X) - 1 (a "bin"): all nodes of a bin spread into the SAME 4 x 4 x 4 cells.
-//   AGGREGATE (warp-aggregated atomics): one warp per occupied bin; lane = (ox, oy, oz mod 2) owns
-//     the two cells (ox, oy, oz) and (ox, oy, oz + 2) of the bin's stencil, reads the bin's node
-//     records as shared-memory broadcasts, sums W F over the nodes IN REGISTERS and issues one
-//     shared-memory atomic per (bin, cell, component) instead of one per (node, cell, component).
-//   GATHER (no atomics at all): one thread per tile cell sums W F over the nodes of the (up to)
-//     4 x 4 x 4 bins whose stencil contains the cell, and adds the total to its own tile cell.
-// Both accumulate in 32-bit fixed point, so the result does not depend on the order of the nodes
-// inside a bin (which the counting sort does not fix): each product W F 2^k is rounded to an
-// integer on its own -- by the magic-number addition fma(w, f, 1.5 * 2^23), a full-rate FMA
-// instead of a quarter-rate F2I -- and integer addition commutes.  |W F 2^k| < 2^22 by the choice of k.
+// S2, the two other forms the north_star names ("gather-by-cell over Morton-sorted nodes or
+// warp-aggregated atomics, whichever the counters favour"; the paper's own
+// fluid3d_force_distribute_kernel is gather-shaped, L356-362).  All nodes with the same base cell
+// b = floor(X) - 1 (a "bin") spread into the SAME 4 x 4 x 4 cells.
+//   AGGREGATE (warp-aggregated atomics, spread_warp_kernel): a warp takes 32 consecutive nodes, one
+//     per lane (along the hidden Morton order they are neighbours on the surface: about 4 share a
+//     bin), groups them by bin with match.any, and then serves the groups one after the other:
+//     lane = (ox, oy, oz mod 2) owns the two cells (ox, oy, oz) and (ox, oy, oz + 2) of the bin's
+//     stencil, reads the group's node records as shared-memory broadcasts, sums W F over the group
+//     IN REGISTERS (in lane order: deterministic) and issues one shared-memory atomic per (group,
+//     cell, component) instead of one per (node, cell, component).  No block-wide sort, no barrier
+//     inside the node loop.
+//   GATHER (no atomics at all, spread_gather_kernel): the nodes of a chunk are counting-sorted by bin
+//     in shared memory; one thread per tile cell sums W F over the nodes of the (up to) 4 x 4 x 4
+//     bins whose stencil contains the cell, and adds the total to its own tile cell.  Each product
+//     W F 2^k is rounded to an integer on its own -- by the magic-number addition
+//     fma(w, f, 1.5 * 2^23), a full-rate FMA instead of a quarter-rate F2I -- so the result does not
+//     depend on the order inside a bin, which the counting sort does not fix.
+// Both accumulate into the same 32-bit fixed-point tile as the scatter form.
 // ---------------------------------------------------------------------------------------------
 constexpr int BIN_CHUNK = IB_THREADS;              // nodes sorted per pass: one per thread
 constexpr float FIX_MAGIC = 12582912.0f;           // 1.5 * 2^23
@@ -597,12 +669,11 @@ __device__ __forceinline__ void block_exclusive_scan(int* __restrict__ a, const 
     __syncthreads();
 }
 
-template <bool GATHER>
-__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_binned_kernel(
+__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_gather_kernel(
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
-    const int cap) {
+    const int cap, int* __restrict__ range_box, const int box_cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
     __shared__ int warp_tot[IB_THREADS / 32];
@@ -610,26 +681,30 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_binned_k
     int* new_segs = tile + 3 * cap;                                    // [SPREAD_SEG_LIST]
     int* bin_start = new_segs + SPREAD_SEG_LIST;                       // [cap + 4] counts, then first slot of each bin
     float4* rec = reinterpret_cast<float4*>(bin_start + ((cap + 4) & ~3));   // [3][BIN_CHUNK] sorted node records
+    unsigned* binrow = reinterpret_cast<unsigned*>(rec + 3 * BIN_CHUNK);     // [cap / 4] occupied base cells, x-mask per tile row
+    unsigned* rowmask = binrow + cap / 4;                              // [cap / 4] touched cells, x-mask per tile row
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true);
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
-    if (!(fmax > 0.f)) return;                                         // nothing to spread
     if (T.enabled == 0 || !(fmax < 3.0e38f)) {
         spread_direct(X, Y, Z, F, n0, n1, g, seg_mask, seg_list, seg_count, p);
         return;
     }
     // |tile value| <= n_nodes max W max|F| 2^k < 2^30 and every product |W F 2^k| <= max|F| 2^k / 8 < 2^22
-    const int k = max(-100, min(100, min(29 - ilogbf(0.125f * (float)(n1 - n0) * fmax), 21 - ilogbf(0.125f * fmax))));
+    // (a range without force still runs: its cells are listed for the interpolation)
+    const int k = fmax > 0.f ? max(-100, min(100, min(29 - ilogbf(0.125f * (float)(n1 - n0) * fmax), 21 - ilogbf(0.125f * fmax)))) : 0;
     const float scale = ldexpf(1.0f, k), inv_scale = ldexpf(1.0f, -k);
     const int p0 = T.p0, pp = T.pp, nword = pp * T.e[2];
     for (int t = tid; t < nword; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
+    const bool by_rows = T.e[0] <= 32;
+    if (by_rows)
+        for (int t = tid; t < T.e[1] * T.e[2]; t += IB_THREADS) binrow[t] = 0u;
     const int nb0 = T.e[0] - 3, nb1 = T.e[1] - 3, nb2 = T.e[2] - 3, nbins = nb0 * nb1 * nb2;
     const bool clipped = T.clipped != 0;
     const int n_chunks = (n1 - n0 + BIN_CHUNK - 1) / BIN_CHUNK;
-    const int lane = tid & 31, warp = tid >> 5;
     for (int c = 0; c < n_chunks; ++c) {
         const int c0 = n0 + (int)((long)(n1 - n0) * c / n_chunks), c1 = n0 + (int)((long)(n1 - n0) * (c + 1) / n_chunks);
         for (int b = tid; b <= nbins; b += IB_THREADS) bin_start[b] = 0;
@@ -651,6 +726,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_binned_k
             sincospif(0.5f * (float)(z - fz), &r1.x, &r1.y);
             r1.z = Fm.x * scale; r1.w = Fm.y * scale; r2.x = Fm.z * scale;
             r2.y = __int_as_float(bx);
+            if (by_rows) touch_base(binrow, T, bx, by, bz);             // binrow was zeroed before the barrier above
         }
         __syncthreads();
         block_exclusive_scan(bin_start, nbins, warp_tot);
@@ -659,56 +735,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_binned_k
             rec[slot] = r0; rec[BIN_CHUNK + slot] = r1; rec[2 * BIN_CHUNK + slot] = r2;
         }
         __syncthreads();
-        if (!GATHER) {
-            // ---- one warp per occupied bin (32 bins examined at a time)
-            const int ox = lane & 3, oy = (lane >> 2) & 3, h = lane >> 4;
-            const float ax = (ox == 0 || ox == 3) ? -0.25f : 0.25f, ay = (oy == 0 || oy == 3) ? -0.25f : 0.25f;
-            const float az = h ? 0.25f : -0.25f;                       // oz = h: (0: 1/4 - s/4, 1: 1/4 + c/4); oz = h + 2: opposite sign
-            for (int b0 = warp * 32; b0 < nbins; b0 += IB_THREADS) {
-                const int bl = b0 + lane;
-                const int my_s = bl < nbins ? bin_start[bl] : 0, my_e = bl < nbins ? bin_start[bl + 1] : 0;
-                unsigned occupied = __ballot_sync(0xffffffffu, my_e > my_s);
-                while (occupied) {
-                    const int src = __ffs(occupied) - 1;
-                    occupied &= occupied - 1;
-                    const int js = __shfl_sync(0xffffffffu, my_s, src), je = __shfl_sync(0xffffffffu, my_e, src);
-                    const int b = b0 + src;
-                    const int bx = b % nb0, br = b / nb0;
-                    const int by = br % nb1, bz = br / nb1;
-                    int a0x = 0, a0y = 0, a0z = 0, a1x = 0, a1y = 0, a1z = 0;
-                    for (int j = js; j < je; ++j) {
-                        const float4 q0 = rec[j], q1 = rec[BIN_CHUNK + j];
-                        const float fzc = rec[2 * BIN_CHUNK + j].x;
-                        const float wx = fmaf(ax, (ox & 1) ? q0.y : q0.x, 0.25f);
-                        const float wy = fmaf(ay, (oy & 1) ? q0.w : q0.z, 0.25f);
-                        const float tz = h ? q1.y : q1.x;
-                        const float wlo = fmaf(az, tz, 0.25f), whi = fmaf(-az, tz, 0.25f);
-                        const float wxy = wx * wy;
-                        const float gx = wxy * q1.z, gy = wxy * q1.w, gz = wxy * fzc;
-                        a0x += __float_as_int(fmaf(wlo, gx, FIX_MAGIC));
-                        a0y += __float_as_int(fmaf(wlo, gy, FIX_MAGIC));
-                        a0z += __float_as_int(fmaf(wlo, gz, FIX_MAGIC));
-                        a1x += __float_as_int(fmaf(whi, gx, FIX_MAGIC));
-                        a1y += __float_as_int(fmaf(whi, gy, FIX_MAGIC));
-                        a1z += __float_as_int(fmaf(whi, gz, FIX_MAGIC));
-                    }
-                    const int bias = (je - js) * FIX_MAGIC_BITS;           // wraps; so did the sums
-                    const int tx = bx + ox, ty = by + oy, tz0 = bz + h, tz1 = bz + h + 2;
-                    if (clipped && (tx < T.lo[0] || tx >= T.hi[0] || ty < T.lo[1] || ty >= T.hi[1])) continue;
-                    const int t0 = tz0 * pp + ty * p0 + tx, t1 = t0 + 2 * pp;
-                    if (!clipped || (tz0 >= T.lo[2] && tz0 < T.hi[2])) {
-                        atomicAdd(tile + t0, a0x - bias);
-                        atomicAdd(tile + cap + t0, a0y - bias);
-                        atomicAdd(tile + 2 * cap + t0, a0z - bias);
-                    }
-                    if (!clipped || (tz1 >= T.lo[2] && tz1 < T.hi[2])) {
-                        atomicAdd(tile + t1, a1x - bias);
-                        atomicAdd(tile + cap + t1, a1y - bias);
-                        atomicAdd(tile + 2 * cap + t1, a1z - bias);
-                    }
-                }
-            }
-        } else {
+        {
             // ---- one thread per tile cell: the bins (bx, by, bz) with cell - bin in {0..3}^3; the x-run
             // of bins of one (by, bz) row is one run of sorted nodes
             const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
@@ -740,7 +767,116 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_binned_k
         }
         __syncthreads();                                               // bins and records consumed
     }
-    spread_flush(T, tile, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
+    if (by_rows) {
+        dilate_rows(binrow, rowmask, T);
+        __syncthreads();
+    }
+    spread_flush(T, tile, rowmask, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
+}
+
+__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_kernel(
+    const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
+    const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
+    unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
+    const int cap, int* __restrict__ range_box, const int box_cap) {
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ MeshTile T;
+    int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point, padded pitches
+    int* new_segs = tile + 3 * cap;                                    // [SPREAD_SEG_LIST]
+    float4* rec = reinterpret_cast<float4*>(new_segs + SPREAD_SEG_LIST);   // [warp][3][32] node records
+    unsigned* binrow = reinterpret_cast<unsigned*>(rec + 3 * IB_THREADS);    // [cap / 4] occupied base cells, x-mask per tile row
+    unsigned* rowmask = binrow + cap / 4;                              // [cap / 4] touched cells, x-mask per tile row
+    const int2 range = __ldg(ranges + blockIdx.x);
+    const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
+    const float fmax = __uint_as_float(T.fmax_bits);
+    if (T.enabled == 0 || !(fmax < 3.0e38f)) {
+        spread_direct(X, Y, Z, F, n0, n1, g, seg_mask, seg_list, seg_count, p);
+        return;
+    }
+    // |tile value| <= n_nodes max W max|F| 2^k < 2^30 (a range without force still runs: its cells are listed)
+    const int k = fmax > 0.f ? max(-100, min(100, 29 - ilogbf(0.125f * (float)(n1 - n0) * fmax))) : 0;
+    const float scale = ldexpf(1.0f, k), inv_scale = ldexpf(1.0f, -k);
+    const int p0 = T.p0, pp = T.pp, nword = pp * T.e[2];
+    for (int t = tid; t < nword; t += IB_THREADS) {
+        tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
+    }
+    const bool by_rows = T.e[0] <= 32;
+    if (by_rows)
+        for (int t = tid; t < T.e[1] * T.e[2]; t += IB_THREADS) binrow[t] = 0u;
+    const bool clipped = T.clipped != 0;
+    __syncthreads();
+    const int lane = tid & 31, warp = tid >> 5;
+    float4* wrec = rec + warp * 96;
+    const int ox = lane & 3, oy = (lane >> 2) & 3, h = lane >> 4;
+    const bool xc = ox & 1, yc = oy & 1;                               // this lane's weights use cos (odd offset) or sin
+    const float ax = (ox == 0 || ox == 3) ? -0.25f : 0.25f, ay = (oy == 0 || oy == 3) ? -0.25f : 0.25f;
+    const float az = h ? 0.25f : -0.25f;     // oz = h: (0: 1/4 - s/4, 1: 1/4 + c/4); oz = h + 2: the opposite sign
+    for (int base = n0 + warp * 32; base < n1; base += IB_THREADS) {
+        // ---- one node per lane: its record and its bin (tile coordinates of the stencil's first cell, < 1024)
+        const int m = base + lane;
+        const bool have = m < n1;
+        int key = -1;
+        if (have) {
+            const double x = X[m], y = Y[m], z = Z[m];
+            const float4 Fm = __ldg(F + m);
+            const double fx = floor(x), fy = floor(y), fz = floor(z);
+            key = ((int)fx - 1 - T.o[0]) | (((int)fy - 1 - T.o[1]) << 10) | (((int)fz - 1 - T.o[2]) << 20);
+            float4 r0, r1;
+            sincospif(0.5f * (float)(x - fx), &r0.x, &r0.y);
+            sincospif(0.5f * (float)(y - fy), &r0.z, &r0.w);
+            sincospif(0.5f * (float)(z - fz), &r1.x, &r1.y);
+            r1.z = Fm.x * scale; r1.w = Fm.y * scale;
+            wrec[lane] = r0; wrec[32 + lane] = r1; wrec[64 + lane] = make_float4(Fm.z * scale, 0.f, 0.f, 0.f);
+        }
+        __syncwarp();
+        const unsigned peers = __match_any_sync(FULL, key);
+        unsigned todo = __ballot_sync(FULL, have && (__ffs(peers) - 1) == lane);   // the first lane of every group
+        while (todo) {
+            const int src = __ffs(todo) - 1;
+            todo &= todo - 1;
+            unsigned members = __shfl_sync(FULL, peers, src);
+            const int kk = __shfl_sync(FULL, key, src);
+            const int bx = kk & 1023, by = (kk >> 10) & 1023, bz = kk >> 20;
+            float a0x = 0.f, a0y = 0.f, a0z = 0.f, a1x = 0.f, a1y = 0.f, a1z = 0.f;
+            while (members) {                                          // in lane order: a fixed summation order
+                const int j = __ffs(members) - 1;
+                members &= members - 1;
+                const float4 q0 = wrec[j], q1 = wrec[32 + j];
+                const float fzc = wrec[64 + j].x;
+                const float wx = fmaf(ax, xc ? q0.y : q0.x, 0.25f);
+                const float wy = fmaf(ay, yc ? q0.w : q0.z, 0.25f);
+                const float tz = h ? q1.y : q1.x;
+                const float wlo = fmaf(az, tz, 0.25f), whi = fmaf(-az, tz, 0.25f);
+                const float wxy = wx * wy;
+                const float gx = wxy * q1.z, gy = wxy * q1.w, gz = wxy * fzc;
+                a0x = fmaf(wlo, gx, a0x); a0y = fmaf(wlo, gy, a0y); a0z = fmaf(wlo, gz, a0z);
+                a1x = fmaf(whi, gx, a1x); a1y = fmaf(whi, gy, a1y); a1z = fmaf(whi, gz, a1z);
+            }
+            const int tx = bx + ox, ty = by + oy, tz0 = bz + h, tz1 = bz + h + 2;
+            if (by_rows && lane == src) touch_base(binrow, T, bx, by, bz);
+            if (clipped && (tx < T.lo[0] || tx >= T.hi[0] || ty < T.lo[1] || ty >= T.hi[1])) continue;
+            const int t0 = tz0 * pp + ty * p0 + tx, t1 = t0 + 2 * pp;
+            if (!clipped || (tz0 >= T.lo[2] && tz0 < T.hi[2])) {
+                atomicAdd(tile + t0, __float2int_rn(a0x));
+                atomicAdd(tile + cap + t0, __float2int_rn(a0y));
+                atomicAdd(tile + 2 * cap + t0, __float2int_rn(a0z));
+            }
+            if (!clipped || (tz1 >= T.lo[2] && tz1 < T.hi[2])) {
+                atomicAdd(tile + t1, __float2int_rn(a1x));
+                atomicAdd(tile + cap + t1, __float2int_rn(a1y));
+                atomicAdd(tile + 2 * cap + t1, __float2int_rn(a1z));
+            }
+        }
+        __syncwarp();                                                  // records consumed
+    }
+    __syncthreads();
+    if (by_rows) {
+        dilate_rows(binrow, rowmask, T);
+        __syncthreads();
+    }
+    spread_flush(T, tile, rowmask, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
 // zero the cells of the segments the previous spread touched (its list), and drop their activity
@@ -977,6 +1113,139 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
     }
 }
 
+// S4 + S5 right after ib_spread for the same positions (the coupled loop).  Every cell of every
+// node's stencil is then in a listed segment, so its (v, rho) is in the velocity field
+// segment_macros_kernel just wrote, and the bounding box of the range is the one the spread
+// stored.  The block copies the box out of the field into its shared-memory tile -- whole rows,
+// coalesced, L2 hits; cells of the box that no stencil contains hold older finite values that no
+// node reads -- and the nodes gather from the tile.  No bounding-box pass, no marks, no
+// compaction, no pull: the general kernel above spent 78 warp instructions per node on those
+// around a 10-instruction gather (profiles/r02b).  The positions of the range are staged in
+// shared memory (one coalesced load, in flight while the tile fills), so the gather sweeps run
+// without a global-load stall and every read of a position precedes every write.
+// A range whose box does not fit the tile (or PLB_INTERP=direct) gathers straight from the field.
+constexpr int INTERP_STAGE = 1024;     // positions of the first nodes of a range are staged in shared memory
+
+__device__ __forceinline__ void interpolate_node(double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z,
+                                                 float4* __restrict__ U, const float4* __restrict__ tile,
+                                                 const float4* __restrict__ vfield, const MeshTile& T, const bool tiled,
+                                                 const double x, const int m, const bool valid, const int sub,
+                                                 const int o0, const int o1, const int o2, int* __restrict__ counters,
+                                                 const LbmParams& p) {
+    const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
+    float ux = 0.f, uy = 0.f, uz = 0.f;
+    if (!valid) {
+    } else if (tiled) {
+        if (T.clipped) gather_column<true>(tile, T, st, st.bx + sub, ux, uy, uz);
+        else           gather_column<false>(tile, T, st, st.bx + sub, ux, uy, uz);
+    } else {
+        const int qx = wrap_index(st.bx + sub, p.nx, p.wall[0]);
+        if (qx >= 0) {
+            int row[4];                                               // qx + nx * qy, or -1
+#pragma unroll
+            for (int oy = 0; oy < 4; ++oy) {
+                const int qy = wrap_index(st.by + oy, p.ny, p.wall[1]);
+                row[oy] = qy < 0 ? -1 : qx + p.nx * qy;
+            }
+            const int sz = p.nx * p.ny;
+#pragma unroll
+            for (int oz = 0; oz < 4; ++oz) {
+                const int qz = wrap_index(st.bz + oz, p.nz, p.wall[2]);
+                if (qz < 0) continue;
+#pragma unroll
+                for (int oy = 0; oy < 4; ++oy) {
+                    if (row[oy] < 0) continue;
+                    const float W = st.wy[oy] * st.wz[oz];
+                    const float4 v = __ldg(vfield + (row[oy] + sz * qz));
+                    ux = fmaf(W, v.x, ux);
+                    uy = fmaf(W, v.y, uy);
+                    uz = fmaf(W, v.z, uz);
+                }
+            }
+        }
+    }
+    ux *= st.wx; uy *= st.wx; uz *= st.wx;
+#pragma unroll
+    for (int o = NODE_LANES / 2; o > 0; o >>= 1) {
+        ux += __shfl_xor_sync(0xffffffffu, ux, o);
+        uy += __shfl_xor_sync(0xffffffffu, uy, o);
+        uz += __shfl_xor_sync(0xffffffffu, uz, o);
+    }
+    // the lane of axis a advances coordinate a (it holds the old value: no second read)
+    const float ua = sub == 1 ? uy : (sub == 2 ? uz : ux);
+    if (valid && sub < 3) {
+        const double xn = x + (double)ua;
+        (sub == 1 ? Y : (sub == 2 ? Z : X))[m] = xn;
+        // halfway bounce-back walls lie at -1/2 and n - 1/2, on-site velocity walls at 0 and n - 1
+        const int na = sub == 1 ? p.ny : (sub == 2 ? p.nz : p.nx);
+        const double ma = p.wall[sub] == PLB_WALL_HH ? 0.0 : 0.5;
+        if (p.wall[sub] && (xn < -ma || xn > (double)(na - 1) + ma)) atomicOr(counters + 1, STATUS_NODE_LEFT);
+    }
+    if (valid && sub == 3) U[m] = make_float4(ux, uy, uz, 0.f);
+}
+
+__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_listed_kernel(
+    double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z, float4* __restrict__ U,
+    const int2* __restrict__ ranges, const float4* __restrict__ vfield, const int* __restrict__ range_box,
+    const int box_cap, int* __restrict__ counters, const LbmParams p, const int cap, const bool use_tile) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ MeshTile T;
+    float4* tile = reinterpret_cast<float4*>(smem_raw);                // [cap] (vx, vy, vz, rho)
+    const int2 range = __ldg(ranges + blockIdx.x);
+    const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
+    const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
+    double* pos = reinterpret_cast<double*>(tile + cap);               // [3][INTERP_STAGE]
+    const int n_staged = min(n1 - n0, INTERP_STAGE);
+    for (int i = tid; i < n_staged; i += IB_THREADS) {
+        pos[i] = X[n0 + i]; pos[INTERP_STAGE + i] = Y[n0 + i]; pos[2 * INTERP_STAGE + i] = Z[n0 + i];
+    }
+    if (!use_tile) {
+        if (tid == 0) T.enabled = 0;
+        __syncthreads();
+    } else if ((int)blockIdx.x < box_cap) {
+        if (tid == 0) {
+            const int4 b0 = __ldg(reinterpret_cast<const int4*>(range_box) + 2 * blockIdx.x);
+            const int4 b1 = __ldg(reinterpret_cast<const int4*>(range_box) + 2 * blockIdx.x + 1);
+            T.mn[0] = b0.x; T.mn[1] = b0.y; T.mn[2] = b0.z;
+            T.mx[0] = b1.x; T.mx[1] = b1.y; T.mx[2] = b1.z;
+            tile_geometry(T, b0.w != 0, p, cap, false);
+        }
+        __syncthreads();
+    } else {
+        tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, false);
+    }
+    const bool tiled = T.enabled != 0;
+    const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
+    if (tiled) {
+        const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+        if (T.interior) {
+            const int sy = p.nx, sz = p.nx * p.ny;
+            const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
+            for (int t = tid; t < ncell; t += IB_THREADS) {
+                const int x = t % e0, r = t / e0;
+                const int y = r % e1, z = r / e1;
+                tile[t] = __ldg(vfield + (origin + x + sy * y + sz * z));
+            }
+        } else {
+            for (int t = tid; t < ncell; t += IB_THREADS) {
+                const int x = t % e0, r = t / e0;
+                const int y = r % e1, z = r / e1;
+                if (x < T.lo[0] || x >= T.hi[0] || y < T.lo[1] || y >= T.hi[1] || z < T.lo[2] || z >= T.hi[2]) continue;
+                const Cell c = tile_cell(T, t, p);
+                tile[t] = __ldg(vfield + (c.i + p.nx * (c.j + p.ny * c.k)));
+            }
+        }
+    }
+    __syncthreads();                                                   // positions staged (and the tile filled)
+    for (int mb = n0; mb < n1; mb += IB_GROUPS) {
+        const int m = mb + group;
+        const bool valid = m < n1;
+        double x = 0.0;                                                // (lanes without a node only run the shuffles)
+        if (valid) x = m - n0 < INTERP_STAGE ? pos[min(sub, 2) * INTERP_STAGE + (m - n0)] : node_coord(X, Y, Z, m, sub);
+        interpolate_node(X, Y, Z, U, tile, vfield, T, tiled, x, m, valid, sub, o0, o1, o2, counters, p);
+    }
+}
+
 // positions: device SoA <-> AoS staging buffer (so host transfers are one contiguous copy)
 // (also stored order <-> caller's order)
 __global__ void __launch_bounds__(256) nodes_transpose_kernel(double* __restrict__ X, double* __restrict__ Y,
@@ -1031,9 +1300,10 @@ int launch_clear_spread(Ctx* c, float4* g) {
     return cuda_check(cudaGetLastError(), "clear_spread_kernel");
 }
 
-static size_t spread_smem(int cap) { return (size_t)cap * 12 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)SPREAD_CHUNK * 48; }
+static size_t spread_smem(int cap) { return (size_t)cap * 14 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)SPREAD_CHUNK * 48; }
+static size_t warp_smem(int cap) { return (size_t)cap * 14 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)IB_THREADS * 48; }
 static size_t binned_smem(int cap) {
-    return (size_t)cap * 12 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)((cap + 4) & ~3) * 4 + (size_t)BIN_CHUNK * 48;
+    return (size_t)cap * 14 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)((cap + 4) & ~3) * 4 + (size_t)BIN_CHUNK * 48;
 }
 static size_t interp_smem(int cap) { return (size_t)cap * 16 + (((size_t)cap * 2 + 15) & ~(size_t)15); }
 
@@ -1054,8 +1324,8 @@ int ib_max_tile_cap() {
     return (int)(cap < 65535 ? cap : 65535);
 }
 
-// words per component of the padded spread tile: two blocks of 110 KB per SM
-int ib_max_spread_cap() { return (int)((90 * 1024) / 12); }
+// words per component of the padded spread tile: two blocks of 113 KB per SM (14 B per word + 20 KB)
+int ib_max_spread_cap() { return 6656; }
 
 // Which form of the spread runs: the caller's choice (ib_set_spread_mode), else by how densely the
 // tiles are sampled -- measured on the B200 (profiles/): the scatter form wins on sparsely sampled
@@ -1065,6 +1335,11 @@ int spread_mode_of(const Ctx* c) {
     if (c->spread_mode != PLB_SPREAD_AUTO) return c->spread_mode;
     return c->tile_density >= 0.6 ? PLB_SPREAD_AGGREGATE : PLB_SPREAD_SCATTER;
 }
+
+// Which form of the interpolation runs after a current spread: the listed-cells kernel through its
+// tile (default), straight from the field, or the general kernel (PLB_INTERP = "tile" / "direct" /
+// "general": measurement knob).
+int interp_form_of(const Ctx* c) { return c->interp_form == PLB_INTERP_AUTO ? PLB_INTERP_TILE : c->interp_form; }
 
 int launch_spread(Ctx* c, float4* g) {
     if (c->n_nodes == 0) return PLB_OK;
@@ -1078,19 +1353,19 @@ int launch_spread(Ctx* c, float4* g) {
         rc = ensure_smem(spread_mesh_kernel, smem, granted_scatter, "cudaFuncSetAttribute(spread_mesh_kernel)");
         if (rc) return rc;
         spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap);
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap);
     } else if (mode == PLB_SPREAD_AGGREGATE) {
-        const size_t smem = binned_smem(cap);
-        rc = ensure_smem(spread_binned_kernel<false>, smem, granted_aggregate, "cudaFuncSetAttribute(spread_binned_kernel<false>)");
+        const size_t smem = warp_smem(cap);
+        rc = ensure_smem(spread_warp_kernel, smem, granted_aggregate, "cudaFuncSetAttribute(spread_warp_kernel)");
         if (rc) return rc;
-        spread_binned_kernel<false><<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap);
+        spread_warp_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap);
     } else {
         const size_t smem = binned_smem(cap);
-        rc = ensure_smem(spread_binned_kernel<true>, smem, granted_gather, "cudaFuncSetAttribute(spread_binned_kernel<true>)");
+        rc = ensure_smem(spread_gather_kernel, smem, granted_gather, "cudaFuncSetAttribute(spread_gather_kernel)");
         if (rc) return rc;
-        spread_binned_kernel<true><<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap);
+        spread_gather_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap);
     }
     c->launches++;
     return cuda_check(cudaGetLastError(), "spread kernel");
@@ -1111,11 +1386,24 @@ int launch_interpolate_advance(Ctx* c) {
                                                            c->vfield, c->prm);
         c->launches++;
     }
-    interpolate_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-        c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->f[c->cur], g, c->vfield, c->seg_mask, c->counters, c->prm,
-        c->tile_cap);
+    // Right after ib_spread for these positions every stencil cell is listed and the boxes of the
+    // ranges are stored: the listed-cells kernel.  Every other case (passive advection, moved
+    // nodes) takes the general kernel, which also computes what the list does not cover.
+    if (c->spread_current && interp_form_of(c) != PLB_INTERP_GENERAL) {
+        static size_t granted_listed = 0;
+        const size_t smem_l = (size_t)c->tile_cap * 16 + (size_t)3 * INTERP_STAGE * sizeof(double);
+        const int rc2 = ensure_smem(interpolate_listed_kernel, smem_l, granted_listed, "cudaFuncSetAttribute(interpolate_listed_kernel)");
+        if (rc2) return rc2;
+        interpolate_listed_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem_l, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->vfield, c->range_box, c->box_cap, c->counters, c->prm,
+            c->tile_cap, interp_form_of(c) != PLB_INTERP_DIRECT);
+    } else {
+        interpolate_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
+            c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->f[c->cur], g, c->vfield, c->seg_mask, c->counters, c->prm,
+            c->tile_cap);
+    }
     c->launches++;
-    return cuda_check(cudaGetLastError(), "interpolate_mesh_kernel");
+    return cuda_check(cudaGetLastError(), "interpolation kernel");
 }
 
 int launch_nodes_transpose(Ctx* c, bool to_aos) {

@@ -12,8 +12,11 @@ constexpr int Q = 19;
 // Activity segments: 8 consecutive cells (one 128-byte line of the float4 forcing field, one
 // 32-byte sector of a population row).  Bit (s & 31) of seg_mask[s >> 5] is set while segment s
 // holds spread force.
-constexpr int SEG = 8;
-constexpr int SEG_SHIFT = 3;
+#ifndef PLB_SEG_SHIFT
+#define PLB_SEG_SHIFT 3
+#endif
+constexpr int SEG_SHIFT = PLB_SEG_SHIFT;
+constexpr int SEG = 1 << SEG_SHIFT;
 
 // D3Q19 velocity set in the paper's numbering (Eq. 21, Eq. 23-30; index = paper's i - 1).
 __host__ __device__ constexpr int CX(int d) {
@@ -65,6 +68,7 @@ __host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e
 }
 
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
+enum InterpForm { PLB_INTERP_AUTO = 0, PLB_INTERP_TILE = 1, PLB_INTERP_DIRECT = 2, PLB_INTERP_GENERAL = 3 };
 
 // consecutive meshes that share one spring table: nodes [node_first, node_first + n_meshes * nn)
 struct SpringGroup {
@@ -163,8 +167,12 @@ struct Ctx {
     std::vector<char> mesh_constrained;
     int2* ranges;              // node ranges [first, last) served by one thread block of the IB kernels
     long n_ranges;
+    int* range_box;            // per range: min and max of floor(X) as the last spread saw them (8 ints), first box_cap ranges
+    int box_cap;
     int tile_cap;              // cells of the shared-memory lattice tile of the interpolation kernel
     int spread_cap;            // words per component of the (padded, bank-conflict-free) spread tile
+    int interp_form;           // PLB_INTERP_*: AUTO, or the form forced through the PLB_INTERP environment variable
+    int range_nodes;           // > 0: nodes per IB thread block forced through PLB_RANGE_NODES
     int spread_mode;           // PLB_SPREAD_*: which form of the spread kernel runs (AUTO: by tile_density)
     double tile_nodes, tile_cells;   // sums over the ranges at ib_add_meshes time: nodes, cells of their tiles
     double tile_density;       // tile_nodes / tile_cells
@@ -203,6 +211,7 @@ void reference_area_volume(const double* xyz, int n_tris, const int* tris, float
 int launch_clear_spread(Ctx* c, float4* g);
 int launch_spread(Ctx* c, float4* g);
 int spread_mode_of(const Ctx* c);
+int interp_form_of(const Ctx* c);
 int launch_interpolate_advance(Ctx* c);
 int ib_max_tile_cap();
 int ib_max_spread_cap();

@@ -288,6 +288,48 @@ def test_interpolate_advance_matches_oracle(kind):
     assert np.abs(rho_g.cpu().numpy() - rho_o).max() <= 6e-7
 
 
+@pytest.mark.parametrize("form", ["tile", "direct", "general"])
+@pytest.mark.parametrize("mode", SPREAD_FORMS)
+def test_interpolation_forms_cover_forceless_and_weak_nodes(form, mode, monkeypatch):
+    """after ib_spread every cell inside some node's stencil is listed, whatever its force: a mesh
+    with NO force, one whose forces are 1e-12 of the neighbouring mesh's (they round to zero in
+    the tile's fixed point) and nodes sitting exactly on lattice points (zero weights) all get the
+    oracle's velocity from either form of the interpolation (PLB_INTERP: measurement knob)"""
+    monkeypatch.setenv("PLB_INTERP", form)
+    n = (40, 24, 36)
+    kind = (0, 1, 0)
+    cells = n[0] * n[1] * n[2]
+    v2, _, _ = wl.icosphere(2)
+    meshes = [v2 * (4.0, 4.0, 1.0) + (20.3, 12.1, 18.7),
+              v2 * (4.0, 1.0, 4.0) + (39.6, 11.0, 9.2),            # across the periodic x seam
+              v2 * (1.0, 4.0, 4.0) + (11.1, 3.6, 27.9),            # against the y wall (clipped stencils)
+              np.round(v2 * (4.0, 4.0, 1.0) + (30.0, 14.0, 30.0))]  # nodes on lattice points
+    sim = plb.Simulation(*n, 0.8, kind, max_nodes=4 * len(v2), max_edges=1)
+    ora = orc.Oracle(*n, 0.8, kind)
+    edges = np.zeros((0, 2), dtype=np.int32)
+    for x in meshes:
+        sim.add_mesh(x, edges, None, 0.0)
+        ora.add_mesh(x, edges, None, 0.0)
+    sim.set_spread_mode(mode)
+    rng = np.random.default_rng(101)
+    F = 1e-2 * rng.standard_normal((sim.n_nodes, 3))
+    F[:len(v2)] = 0.0                                              # mesh 0: no force at all
+    F[len(v2):len(v2) + len(v2) // 2] *= 1e-12                      # half of mesh 1: far below the tile's quantum
+    rho, u = wl.random_fields(103, cells)
+    sim.set_equilibrium(dev(rho), dev(u))
+    ora.set_equilibrium(rho, u)
+    for s_ in (sim, ora):
+        s_.write_forces(F)
+    sim.spread(); sim.step(sim.forcing); sim.interpolate_advance()
+    g = ora.spread(); ora.step(g); ora.interpolate_advance()
+    sim.status()
+    U_g, U_o = sim.read_node_velocities().astype(np.float64), ora.read_node_velocities()
+    assert np.abs(U_o).max() > 1e-3
+    assert np.abs(U_g - U_o).max() <= 1e-6
+    assert np.abs(sim.read_nodes() - ora.read_nodes()).max() <= 1e-6
+    sim.close(); ora.close()
+
+
 def test_P13_passive_advection_across_the_seam():
     """GPU twin of the oracle pin P13: lbm_step(NULL) -> ib_interpolate_advance with NO spread in
     between (Eq. 33 alone).  A pre-stressed mesh in a uniform periodic flow translates rigidly by u0
