@@ -149,20 +149,26 @@ PLB_API int ib_spread(plb_ctx* ctx, float* d_forcing);
 /* The three forms of the S2 kernel (all compute the sum of Eq. 34; they differ in how the
  * contributions of the nodes of one thread block meet in its shared-memory lattice tile):
  *   SCATTER   one shared-memory atomic per (node, cell, component);
- *   AGGREGATE nodes counting-sorted by base cell, one warp per occupied base cell sums its nodes in
- *             registers: one shared-memory atomic per (base cell, cell, component);
- *   GATHER    same sort, one thread per tile cell sums over the 4 x 4 x 4 base cells around it: no
- *             atomics (the form of the paper's own fluid3d_force_distribute_kernel, L356-362).
- * AUTO (default) picks SCATTER or AGGREGATE from the sampling density of the tiles.
- * ib_get_spread_mode returns the form ib_spread would launch now. */
+ *   AGGREGATE warp-aggregated atomics: a warp groups its 32 consecutive nodes by base cell
+ *             (match.any), sums each group in registers and issues one shared-memory atomic per
+ *             (group, cell, component);
+ *   GATHER    nodes counting-sorted by base cell, one thread per tile cell sums over the 4 x 4 x 4
+ *             base cells around it: no atomics (the form of the paper's own
+ *             fluid3d_force_distribute_kernel, L356-362).
+ * AUTO (default) picks SCATTER or AGGREGATE from the sampling density of the tiles (DESIGN.md
+ * section 5 has the measurements behind the choice).  ib_get_spread_mode returns the form
+ * ib_spread would launch now.
+ * Whatever the form, ib_spread also LISTS every cell inside some node's stencil (also where the
+ * spread force is zero): right after it, ib_interpolate_advance for the same positions reads the
+ * velocity of exactly those cells. */
+enum { PLB_SPREAD_AUTO = 0, PLB_SPREAD_SCATTER = 1, PLB_SPREAD_AGGREGATE = 2, PLB_SPREAD_GATHER = 3 };
+PLB_API int ib_set_spread_mode(plb_ctx* ctx, int mode);
+PLB_API int ib_get_spread_mode(plb_ctx* ctx, int* out_mode_in_use);
+
 /* Forget the forcing buffers the context still points to (the one ib_spread last filled, the one
  * lbm_step last read), clearing what ib_spread wrote first; the caller may free them afterwards.
  * ib_interpolate_advance / lbm_read_macros then see g = 0 until the next lbm_step. */
 PLB_API int ib_release_forcing(plb_ctx* ctx);
-
-enum { PLB_SPREAD_AUTO = 0, PLB_SPREAD_SCATTER = 1, PLB_SPREAD_AGGREGATE = 2, PLB_SPREAD_GATHER = 3 };
-PLB_API int ib_set_spread_mode(plb_ctx* ctx, int mode);
-PLB_API int ib_get_spread_mode(plb_ctx* ctx, int* out_mode_in_use);
 
 /* S4 + S5.  U_m = sum_ijk v_ijk phi phi phi (Eq. 33) with v the velocity lbm_read_macros
  * would return now (state after lbm_step, force just applied) and the stencil around the not yet

@@ -504,8 +504,7 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
                     lo = f < lo ? f : lo;
                     hi = f > hi ? f : hi;
                 }
-                // the interpolation tile pads its rows (interp_row_pitch)
-                vol *= d == 0 && hi - lo < 1e6 ? (double)interp_row_pitch((int)(hi - lo) + 6) : hi - lo + 4.0 + 2.0;
+                vol *= hi - lo + 4.0 + 2.0;
                 box *= hi - lo + 4.0;
                 ext[d] = hi - lo < 1e6 ? (int)(hi - lo) + 6 : 1 << 20;
             }
@@ -516,7 +515,7 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
             ctx->tile_nodes += (double)(b - a);
             ctx->tile_cells += box;
             const int emax = ext[0] > ext[1] ? (ext[0] > ext[2] ? ext[0] : ext[2]) : (ext[1] > ext[2] ? ext[1] : ext[2]);
-            const double cube = (double)interp_row_pitch(emax) * emax * emax;
+            const double cube = (double)emax * emax * emax;
             if (vol <= (double)ib_max_tile_cap()) {
                 double want = vol;
                 const double allowance = cube < 4352.0 ? cube : 4352.0;

@@ -237,9 +237,8 @@ __device__ __forceinline__ void mark_segment(const int cell, unsigned* __restric
 }
 
 // tile geometry from the box T.mn, T.mx of floor(X) over the range (one thread)
-// pitches: 0 = dense, 1 = the spread tile's bank-conflict-free pitches, 2 = interp_row_pitch
 __device__ __forceinline__ void tile_geometry(MeshTile& T, const bool nonempty, const LbmParams& p, const int cap,
-                                              const int padded) {
+                                              const bool padded) {
     const int n[3] = {p.nx, p.ny, p.nz};
     long long vol = 1;
     bool ok = nonempty, clipped = false, interior = true;
@@ -260,8 +259,8 @@ __device__ __forceinline__ void tile_geometry(MeshTile& T, const bool nonempty, 
         clipped = clipped || T.lo[a] != 0 || T.hi[a] != T.e[a];
         interior = interior && (long long)T.o[a] >= 1 && (long long)T.o[a] + ext <= (long long)n[a] - 1;
     }
-    T.p0 = padded == 1 ? tile_row_pitch(T.e[0]) : (padded == 2 ? interp_row_pitch(T.e[0]) : T.e[0]);
-    T.pp = padded == 1 ? tile_plane_pitch(T.p0, T.e[1]) : T.p0 * T.e[1];
+    T.p0 = padded ? tile_row_pitch(T.e[0]) : T.e[0];
+    T.pp = padded ? tile_plane_pitch(T.p0, T.e[1]) : T.e[0] * T.e[1];
     ok = ok && (long long)T.pp * T.e[2] <= (long long)cap;
     T.enabled = ok ? 1 : 0;
     T.clipped = clipped ? 1 : 0;
@@ -273,7 +272,7 @@ __device__ __forceinline__ void tile_geometry(MeshTile& T, const bool nonempty, 
 // is also stored (8 ints) for the interpolation of the same positions
 __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict__ X, const double* __restrict__ Y,
                                            const double* __restrict__ Z, const float4* __restrict__ F, const int n0,
-                                           const int n1, const LbmParams& p, const int cap, const int padded,
+                                           const int n1, const LbmParams& p, const int cap, const bool padded,
                                            int* __restrict__ box_out = nullptr) {
     if (threadIdx.x == 0) {
         for (int a = 0; a < 3; ++a) { T.mn[a] = INT_MAX; T.mx[a] = INT_MIN; }
@@ -445,68 +444,36 @@ __device__ __forceinline__ void dilate_rows(const unsigned* __restrict__ binrow,
     }
 }
 
-// Flush of a spread tile: one vector RED per non-zero tile cell, and the segments of the touched
-// cells marked.  The segments this block is the first to mark are collected in shared memory and
-// appended to the global list with ONE atomicAdd per block (a returning atomic per segment on the
-// single list counter was 58 % of the scatter kernel's stall samples).  All threads of the block
-// call it, after a __syncthreads().
-// Tiles up to 32 cells wide: one warp per tile row, lane = x -- no division per cell, and ONE
-// returning atomic per (row, segment) on the activity mask instead of a dependent read per cell
-// (12 % of the stall samples of the per-cell form, profiles/r02e).
-__device__ __forceinline__ void note_new_segment(MeshTile& T, int* __restrict__ new_segs, int* __restrict__ seg_list,
-                                                 int* __restrict__ seg_count, const int seg) {
-    const int slot = atomicAdd(&T.n_need, 1);                           // n_need doubles as the block's list length
-    if (slot < SPREAD_SEG_LIST) new_segs[slot] = seg;
-    else seg_list[atomicAdd(seg_count, 1)] = seg;                      // list full: append directly
-}
-
+// Flush of a spread tile: one vector RED per non-zero tile cell.  The segments this block is the
+// first to mark are collected in shared memory and appended to the global list with ONE atomicAdd
+// per block (a returning atomic per segment on the single list counter was 58 % of the scatter
+// kernel's stall samples).  All threads of the block call it, after a __syncthreads().
 __device__ __forceinline__ void spread_flush(MeshTile& T, const int* __restrict__ tile, const unsigned* __restrict__ rowmask,
                                              int* __restrict__ new_segs, const int cap, const float inv_scale,
                                              float4* __restrict__ g, unsigned* __restrict__ seg_mask,
                                              int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams& p) {
     const int tid = threadIdx.x;
-    const int e0 = T.e[0], e1 = T.e[1];
-    if (e0 <= 32) {
-        const int lane = tid & 31, warp = tid >> 5, nrow = e1 * T.e[2];
-        const int qx = wrap_index(T.o[0] + lane, p.nx, 0);
-        for (int r = warp; r < nrow; r += IB_THREADS / 32) {
-            const unsigned touched_row = rowmask[r];
-            if (touched_row == 0u) continue;
-            const int z = r / e1, y = r - z * e1;
-            const int row_cell = p.nx * (wrap_index(T.o[1] + y, p.ny, 0) + p.ny * wrap_index(T.o[2] + z, p.nz, 0));
-            const bool touched = (touched_row >> lane) & 1u;
-            const int cell = row_cell + qx, seg = cell >> SEG_SHIFT;
-            if (touched) {
-                const int w = z * T.pp + y * T.p0 + lane;
-                const int vx = tile[w], vy = tile[cap + w], vz = tile[2 * cap + w];
-                if ((vx | vy | vz) != 0)
-                    atomicAdd(g + cell, make_float4((float)vx * inv_scale, (float)vy * inv_scale, (float)vz * inv_scale, 0.f));
-            }
-            // the first touched lane of every segment of the row marks it
-            const int seg_below = __shfl_up_sync(0xffffffffu, seg, 1);
-            const bool below_touched = lane > 0 && ((touched_row >> (lane - 1)) & 1u);
-            if (touched && (!below_touched || seg_below != seg)) {
-                const unsigned bit = 1u << (seg & 31);
-                if ((atomicOr(seg_mask + (seg >> 5), bit) & bit) == 0u) note_new_segment(T, new_segs, seg_list, seg_count, seg);
-            }
-        }
-    } else {
-        const int ncell = e0 * e1 * T.e[2];
-        for (int t = tid; t < ncell; t += IB_THREADS) {
-            const int x = t % e0, r = t / e0;
-            const int y = r % e1, z = r / e1;
-            if (!(x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2])) continue;
-            const int w = z * T.pp + y * T.p0 + x;
-            const int vx = tile[w], vy = tile[cap + w], vz = tile[2 * cap + w];
-            const Cell c = tile_cell(T, t, p);
-            const int cell = c.i + p.nx * (c.j + p.ny * c.k);
-            if ((vx | vy | vz) != 0)
-                atomicAdd(g + cell, make_float4((float)vx * inv_scale, (float)vy * inv_scale, (float)vz * inv_scale, 0.f));
-            const int seg = cell >> SEG_SHIFT;
-            const unsigned bit = 1u << (seg & 31);
-            unsigned* word = seg_mask + (seg >> 5);
-            if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u)
-                note_new_segment(T, new_segs, seg_list, seg_count, seg);
+    const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+    const bool by_rows = e0 <= 32;
+    for (int t = tid; t < ncell; t += IB_THREADS) {
+        const int x = t % e0, r = t / e0;
+        const int y = r % e1, z = r / e1;
+        const bool touched = by_rows ? ((rowmask[r] >> x) & 1u) != 0u
+                                     : (x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]);
+        if (!touched) continue;
+        const int w = z * T.pp + y * T.p0 + x;
+        const int qx = tile[w], qy = tile[cap + w], qz = tile[2 * cap + w];
+        const Cell c = tile_cell(T, t, p);
+        const int cell = c.i + p.nx * (c.j + p.ny * c.k);
+        if ((qx | qy | qz) != 0)
+            atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
+        const int seg = cell >> SEG_SHIFT;
+        const unsigned bit = 1u << (seg & 31);
+        unsigned* word = seg_mask + (seg >> 5);
+        if ((*(volatile unsigned*)word & bit) == 0u && (atomicOr(word, bit) & bit) == 0u) {
+            const int slot = atomicAdd(&T.n_need, 1);                   // n_need doubles as the block's list length
+            if (slot < SPREAD_SEG_LIST) new_segs[slot] = seg;
+            else seg_list[atomicAdd(seg_count, 1)] = seg;              // list full: append directly
         }
     }
     __syncthreads();
@@ -535,7 +502,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     unsigned* rowmask = binrow + cap / 4;                              // [cap / 4] touched cells, x-mask per tile row
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, 1, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
     const bool tiled = T.enabled != 0 && fmax < 3.0e38f;
     const int nword = tiled ? T.pp * T.e[2] : 0;
@@ -718,7 +685,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_gather_k
     unsigned* rowmask = binrow + cap / 4;                              // [cap / 4] touched cells, x-mask per tile row
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, 1, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
     if (T.enabled == 0 || !(fmax < 3.0e38f)) {
         spread_direct(X, Y, Z, F, n0, n1, g, seg_mask, seg_list, seg_count, p);
@@ -817,12 +784,12 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
     __shared__ MeshTile T;
     int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point, padded pitches
     int* new_segs = tile + 3 * cap;                                    // [SPREAD_SEG_LIST]
-    float* rec = reinterpret_cast<float*>(new_segs + SPREAD_SEG_LIST);  // [warp][32][16] node records: wx[4], wy[4], (wz0, wz2, wz1, wz3), F 2^k
-    unsigned* binrow = reinterpret_cast<unsigned*>(rec + 16 * IB_THREADS);   // [cap / 4] occupied base cells, x-mask per tile row
+    float4* rec = reinterpret_cast<float4*>(new_segs + SPREAD_SEG_LIST);   // [warp][3][32] node records
+    unsigned* binrow = reinterpret_cast<unsigned*>(rec + 3 * IB_THREADS);    // [cap / 4] occupied base cells, x-mask per tile row
     unsigned* rowmask = binrow + cap / 4;                              // [cap / 4] touched cells, x-mask per tile row
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, 1, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
+    tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
     if (T.enabled == 0 || !(fmax < 3.0e38f)) {
         spread_direct(X, Y, Z, F, n0, n1, g, seg_mask, seg_list, seg_count, p);
@@ -841,11 +808,13 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
     const bool clipped = T.clipped != 0;
     __syncthreads();
     const int lane = tid & 31, warp = tid >> 5;
-    float* wrec = rec + warp * 512;
-    const int ox = lane & 3, oy = (lane >> 2) & 3, h = lane >> 4;     // this lane's two cells: (ox, oy, h) and (ox, oy, h + 2)
+    float4* wrec = rec + warp * 96;
+    const int ox = lane & 3, oy = (lane >> 2) & 3, h = lane >> 4;
+    const bool xc = ox & 1, yc = oy & 1;                               // this lane's weights use cos (odd offset) or sin
+    const float ax = (ox == 0 || ox == 3) ? -0.25f : 0.25f, ay = (oy == 0 || oy == 3) ? -0.25f : 0.25f;
+    const float az = h ? 0.25f : -0.25f;     // oz = h: (0: 1/4 - s/4, 1: 1/4 + c/4); oz = h + 2: the opposite sign
     for (int base = n0 + warp * 32; base < n1; base += IB_THREADS) {
-        // ---- one node per lane: its twelve weights, its scaled force and its bin (tile coordinates
-        // of the stencil's first cell, each < 1024)
+        // ---- one node per lane: its record and its bin (tile coordinates of the stencil's first cell, < 1024)
         const int m = base + lane;
         const bool have = m < n1;
         int key = -1;
@@ -854,18 +823,12 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
             const float4 Fm = __ldg(F + m);
             const double fx = floor(x), fy = floor(y), fz = floor(z);
             key = ((int)fx - 1 - T.o[0]) | (((int)fy - 1 - T.o[1]) << 10) | (((int)fz - 1 - T.o[2]) << 20);
-            float sn, cs, w[4];
-            float4* out = reinterpret_cast<float4*>(wrec + 16 * lane);
-            sincospif(0.5f * (float)(x - fx), &sn, &cs);
-            weights4(sn, cs, w);
-            out[0] = make_float4(w[0], w[1], w[2], w[3]);
-            sincospif(0.5f * (float)(y - fy), &sn, &cs);
-            weights4(sn, cs, w);
-            out[1] = make_float4(w[0], w[1], w[2], w[3]);
-            sincospif(0.5f * (float)(z - fz), &sn, &cs);
-            weights4(sn, cs, w);
-            out[2] = make_float4(w[0], w[2], w[1], w[3]);
-            out[3] = make_float4(Fm.x * scale, Fm.y * scale, Fm.z * scale, 0.f);
+            float4 r0, r1;
+            sincospif(0.5f * (float)(x - fx), &r0.x, &r0.y);
+            sincospif(0.5f * (float)(y - fy), &r0.z, &r0.w);
+            sincospif(0.5f * (float)(z - fz), &r1.x, &r1.y);
+            r1.z = Fm.x * scale; r1.w = Fm.y * scale;
+            wrec[lane] = r0; wrec[32 + lane] = r1; wrec[64 + lane] = make_float4(Fm.z * scale, 0.f, 0.f, 0.f);
         }
         __syncwarp();
         const unsigned peers = __match_any_sync(FULL, key);
@@ -880,13 +843,16 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
             while (members) {                                          // in lane order: a fixed summation order
                 const int j = __ffs(members) - 1;
                 members &= members - 1;
-                const float* q = wrec + 16 * j;
-                const float wxy = q[ox] * q[4 + oy];
-                const float2 wz = *reinterpret_cast<const float2*>(q + 8 + 2 * h);
-                const float4 f = *reinterpret_cast<const float4*>(q + 12);
-                const float gx = wxy * f.x, gy = wxy * f.y, gz = wxy * f.z;
-                a0x = fmaf(wz.x, gx, a0x); a0y = fmaf(wz.x, gy, a0y); a0z = fmaf(wz.x, gz, a0z);
-                a1x = fmaf(wz.y, gx, a1x); a1y = fmaf(wz.y, gy, a1y); a1z = fmaf(wz.y, gz, a1z);
+                const float4 q0 = wrec[j], q1 = wrec[32 + j];
+                const float fzc = wrec[64 + j].x;
+                const float wx = fmaf(ax, xc ? q0.y : q0.x, 0.25f);
+                const float wy = fmaf(ay, yc ? q0.w : q0.z, 0.25f);
+                const float tz = h ? q1.y : q1.x;
+                const float wlo = fmaf(az, tz, 0.25f), whi = fmaf(-az, tz, 0.25f);
+                const float wxy = wx * wy;
+                const float gx = wxy * q1.z, gy = wxy * q1.w, gz = wxy * fzc;
+                a0x = fmaf(wlo, gx, a0x); a0y = fmaf(wlo, gy, a0y); a0z = fmaf(wlo, gz, a0z);
+                a1x = fmaf(whi, gx, a1x); a1y = fmaf(whi, gy, a1y); a1z = fmaf(whi, gz, a1z);
             }
             const int tx = bx + ox, ty = by + oy, tz0 = bz + h, tz1 = bz + h + 2;
             if (by_rows && lane == src) touch_base(binrow, T, bx, by, bz);
@@ -989,7 +955,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
     unsigned short* list = reinterpret_cast<unsigned short*>(tile + cap);   // [cap] needed tile cells
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, 0);
+    tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, false);
     const bool tiled = T.enabled != 0;
     const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
     const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
@@ -1159,88 +1125,51 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mes
 // without a global-load stall and every read of a position precedes every write.
 // A range whose box does not fit the tile (or PLB_INTERP=direct) gathers straight from the field.
 constexpr int INTERP_STAGE = 1024;     // positions of the first nodes of a range are staged in shared memory
-constexpr int INTERP_LANES = 8;        // lane = (ox, hy): x offset of the stencil column and which of two rows per step
-constexpr int INTERP_GROUPS = IB_THREADS / INTERP_LANES;
 
-// One node, its eight lanes.  Lane a < 3 holds x = coordinate a of the node and evaluates that axis.
-// Per load instruction the eight lanes read two tile rows d apart, four consecutive cells each:
-// with interp_row_pitch the two 64-byte pieces cover all 32 banks once, so a warp's four nodes cost
-// exactly four shared-memory wavefronts per instruction (the four-lane column layout of the general
-// kernel measured 6.8).
 __device__ __forceinline__ void interpolate_node(double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z,
                                                  float4* __restrict__ U, const float4* __restrict__ tile,
                                                  const float4* __restrict__ vfield, const MeshTile& T, const bool tiled,
                                                  const double x, const int m, const bool valid, const int sub,
                                                  const int o0, const int o1, const int o2, int* __restrict__ counters,
                                                  const LbmParams& p) {
-    constexpr unsigned FULL = 0xffffffffu;
-    const int ox = sub & 3, hy = sub >> 2;
-    const double fl = floor(x);
-    const int base = (int)fl - 1 - (sub == 1 ? o1 : (sub == 2 ? o2 : o0));
-    float s, c;
-    sincospif(0.5f * (float)(x - fl), &s, &c);
-    const int bx = __shfl_sync(FULL, base, 0, INTERP_LANES), by = __shfl_sync(FULL, base, 1, INTERP_LANES),
-              bz = __shfl_sync(FULL, base, 2, INTERP_LANES);
-    const float sx = __shfl_sync(FULL, s, 0, INTERP_LANES), cx = __shfl_sync(FULL, c, 0, INTERP_LANES);
-    const float sy = __shfl_sync(FULL, s, 1, INTERP_LANES), cy = __shfl_sync(FULL, c, 1, INTERP_LANES);
-    const float sz = __shfl_sync(FULL, s, 2, INTERP_LANES), cz = __shfl_sync(FULL, c, 2, INTERP_LANES);
-    // rows of this lane: step k = 0, 1 reads row oy[k]; the partner lane (other hy) reads the row d apart
-    const int d = tiled && (T.p0 & 7) != 4 ? 2 : 1;
-    const int oy0 = d == 1 ? hy : 2 * hy, oy1 = d == 1 ? 2 + hy : 1 + 2 * hy;
-    const float wx = weight_o(sx, cx, ox), wy0 = weight_o(sy, cy, oy0), wy1 = weight_o(sy, cy, oy1);
-    float wz[4];
-    weights4(sz, cz, wz);
+    const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
     float ux = 0.f, uy = 0.f, uz = 0.f;
     if (!valid) {
     } else if (tiled) {
-        const int tx = bx + ox, ty0 = by + oy0, ty1 = by + oy1;
-        const bool clipped = T.clipped != 0;
-        const bool in0 = !clipped || (tx >= T.lo[0] && tx < T.hi[0] && ty0 >= T.lo[1] && ty0 < T.hi[1]);
-        const bool in1 = !clipped || (tx >= T.lo[0] && tx < T.hi[0] && ty1 >= T.lo[1] && ty1 < T.hi[1]);
-        const float4* col = tile + (bz * T.pp + by * T.p0 + tx);
-        const int r0 = oy0 * T.p0, r1 = oy1 * T.p0;
-#pragma unroll
-        for (int oz = 0; oz < 4; ++oz) {
-            if (clipped && (bz + oz < T.lo[2] || bz + oz >= T.hi[2])) continue;
-            if (in0) {
-                const float W = wy0 * wz[oz];
-                const float4 v = col[oz * T.pp + r0];
-                ux = fmaf(W, v.x, ux); uy = fmaf(W, v.y, uy); uz = fmaf(W, v.z, uz);
-            }
-            if (in1) {
-                const float W = wy1 * wz[oz];
-                const float4 v = col[oz * T.pp + r1];
-                ux = fmaf(W, v.x, ux); uy = fmaf(W, v.y, uy); uz = fmaf(W, v.z, uz);
-            }
-        }
+        if (T.clipped) gather_column<true>(tile, T, st, st.bx + sub, ux, uy, uz);
+        else           gather_column<false>(tile, T, st, st.bx + sub, ux, uy, uz);
     } else {
-        const int qx = wrap_index(bx + ox, p.nx, p.wall[0]);
-        const int qy0 = wrap_index(by + oy0, p.ny, p.wall[1]), qy1 = wrap_index(by + oy1, p.ny, p.wall[1]);
+        const int qx = wrap_index(st.bx + sub, p.nx, p.wall[0]);
         if (qx >= 0) {
-            const int sz_ = p.nx * p.ny;
+            int row[4];                                               // qx + nx * qy, or -1
+#pragma unroll
+            for (int oy = 0; oy < 4; ++oy) {
+                const int qy = wrap_index(st.by + oy, p.ny, p.wall[1]);
+                row[oy] = qy < 0 ? -1 : qx + p.nx * qy;
+            }
+            const int sz = p.nx * p.ny;
 #pragma unroll
             for (int oz = 0; oz < 4; ++oz) {
-                const int qz = wrap_index(bz + oz, p.nz, p.wall[2]);
+                const int qz = wrap_index(st.bz + oz, p.nz, p.wall[2]);
                 if (qz < 0) continue;
-                if (qy0 >= 0) {
-                    const float W = wy0 * wz[oz];
-                    const float4 v = __ldg(vfield + (qx + p.nx * qy0 + sz_ * qz));
-                    ux = fmaf(W, v.x, ux); uy = fmaf(W, v.y, uy); uz = fmaf(W, v.z, uz);
-                }
-                if (qy1 >= 0) {
-                    const float W = wy1 * wz[oz];
-                    const float4 v = __ldg(vfield + (qx + p.nx * qy1 + sz_ * qz));
-                    ux = fmaf(W, v.x, ux); uy = fmaf(W, v.y, uy); uz = fmaf(W, v.z, uz);
+#pragma unroll
+                for (int oy = 0; oy < 4; ++oy) {
+                    if (row[oy] < 0) continue;
+                    const float W = st.wy[oy] * st.wz[oz];
+                    const float4 v = __ldg(vfield + (row[oy] + sz * qz));
+                    ux = fmaf(W, v.x, ux);
+                    uy = fmaf(W, v.y, uy);
+                    uz = fmaf(W, v.z, uz);
                 }
             }
         }
     }
-    ux *= wx; uy *= wx; uz *= wx;
+    ux *= st.wx; uy *= st.wx; uz *= st.wx;
 #pragma unroll
-    for (int o = INTERP_LANES / 2; o > 0; o >>= 1) {
-        ux += __shfl_xor_sync(FULL, ux, o);
-        uy += __shfl_xor_sync(FULL, uy, o);
-        uz += __shfl_xor_sync(FULL, uz, o);
+    for (int o = NODE_LANES / 2; o > 0; o >>= 1) {
+        ux += __shfl_xor_sync(0xffffffffu, ux, o);
+        uy += __shfl_xor_sync(0xffffffffu, uy, o);
+        uz += __shfl_xor_sync(0xffffffffu, uz, o);
     }
     // the lane of axis a advances coordinate a (it holds the old value: no second read)
     const float ua = sub == 1 ? uy : (sub == 2 ? uz : ux);
@@ -1261,10 +1190,10 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_lis
     const int box_cap, int* __restrict__ counters, const LbmParams p, const int cap, const bool use_tile) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
-    float4* tile = reinterpret_cast<float4*>(smem_raw);                // [cap] (vx, vy, vz, rho), rows of interp_row_pitch
+    float4* tile = reinterpret_cast<float4*>(smem_raw);                // [cap] (vx, vy, vz, rho)
     const int2 range = __ldg(ranges + blockIdx.x);
     const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    const int sub = tid & (INTERP_LANES - 1), group = tid / INTERP_LANES;
+    const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
     double* pos = reinterpret_cast<double*>(tile + cap);               // [3][INTERP_STAGE]
     const int n_staged = min(n1 - n0, INTERP_STAGE);
     for (int i = tid; i < n_staged; i += IB_THREADS) {
@@ -1279,37 +1208,40 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_lis
             const int4 b1 = __ldg(reinterpret_cast<const int4*>(range_box) + 2 * blockIdx.x + 1);
             T.mn[0] = b0.x; T.mn[1] = b0.y; T.mn[2] = b0.z;
             T.mx[0] = b1.x; T.mx[1] = b1.y; T.mx[2] = b1.z;
-            tile_geometry(T, b0.w != 0, p, cap, 2);
+            tile_geometry(T, b0.w != 0, p, cap, false);
         }
         __syncthreads();
     } else {
-        tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, 2);
+        tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, false);
     }
     const bool tiled = T.enabled != 0;
     const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
     if (tiled) {
-        // one warp per tile row, lane = x: coalesced loads, no division
-        const int e0 = T.e[0], e1 = T.e[1], nrow = e1 * T.e[2];
-        const int lane = tid & 31, warp = tid >> 5;
-        for (int x0 = 0; x0 < e0; x0 += 32) {
-            const int x = x0 + lane;
-            const int qx = wrap_index(T.o[0] + x, p.nx, 0);
-            const bool xin = x < e0 && x >= T.lo[0] && x < T.hi[0];
-            for (int r = warp; r < nrow; r += IB_THREADS / 32) {
-                const int z = r / e1, y = r - z * e1;
-                if (y < T.lo[1] || y >= T.hi[1] || z < T.lo[2] || z >= T.hi[2]) continue;
-                const int qy = wrap_index(T.o[1] + y, p.ny, 0), qz = wrap_index(T.o[2] + z, p.nz, 0);
-                if (xin) tile[z * T.pp + y * T.p0 + x] = __ldg(vfield + (qx + p.nx * (qy + p.ny * qz)));
+        const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+        if (T.interior) {
+            const int sy = p.nx, sz = p.nx * p.ny;
+            const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
+            for (int t = tid; t < ncell; t += IB_THREADS) {
+                const int x = t % e0, r = t / e0;
+                const int y = r % e1, z = r / e1;
+                tile[t] = __ldg(vfield + (origin + x + sy * y + sz * z));
+            }
+        } else {
+            for (int t = tid; t < ncell; t += IB_THREADS) {
+                const int x = t % e0, r = t / e0;
+                const int y = r % e1, z = r / e1;
+                if (x < T.lo[0] || x >= T.hi[0] || y < T.lo[1] || y >= T.hi[1] || z < T.lo[2] || z >= T.hi[2]) continue;
+                const Cell c = tile_cell(T, t, p);
+                tile[t] = __ldg(vfield + (c.i + p.nx * (c.j + p.ny * c.k)));
             }
         }
     }
     __syncthreads();                                                   // positions staged (and the tile filled)
-    for (int mb = n0; mb < n1; mb += INTERP_GROUPS) {
+    for (int mb = n0; mb < n1; mb += IB_GROUPS) {
         const int m = mb + group;
         const bool valid = m < n1;
         double x = 0.0;                                                // (lanes without a node only run the shuffles)
-        const int axis = sub < 3 ? sub : 0;
-        if (valid) x = m - n0 < INTERP_STAGE ? pos[axis * INTERP_STAGE + (m - n0)] : node_coord(X, Y, Z, m, axis);
+        if (valid) x = m - n0 < INTERP_STAGE ? pos[min(sub, 2) * INTERP_STAGE + (m - n0)] : node_coord(X, Y, Z, m, sub);
         interpolate_node(X, Y, Z, U, tile, vfield, T, tiled, x, m, valid, sub, o0, o1, o2, counters, p);
     }
 }
@@ -1369,7 +1301,7 @@ int launch_clear_spread(Ctx* c, float4* g) {
 }
 
 static size_t spread_smem(int cap) { return (size_t)cap * 14 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)SPREAD_CHUNK * 48; }
-static size_t warp_smem(int cap) { return (size_t)cap * 14 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)IB_THREADS * 64; }
+static size_t warp_smem(int cap) { return (size_t)cap * 14 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)IB_THREADS * 48; }
 static size_t binned_smem(int cap) {
     return (size_t)cap * 14 + (size_t)SPREAD_SEG_LIST * 4 + (size_t)((cap + 4) & ~3) * 4 + (size_t)BIN_CHUNK * 48;
 }

@@ -67,12 +67,6 @@ __host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e
     return r + ((8 - (r & 15)) & 15);
 }
 
-// Row pitch (in cells of 16 bytes) of the interpolation tile: even and not a multiple of 8, so that
-// two rows d = 1 (pitch = 4 mod 8) or d = 2 (pitch = 2, 6 mod 8) apart start 64 bytes apart modulo the
-// 128 bytes of the shared-memory banks: the two 64-byte row pieces a node's eight lanes read per
-// instruction cover every bank exactly once.
-__host__ __device__ inline int interp_row_pitch(const int e0) { return (e0 & 1) ? e0 + 1 : ((e0 & 7) == 0 ? e0 + 2 : e0); }
-
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
 enum InterpForm { PLB_INTERP_AUTO = 0, PLB_INTERP_TILE = 1, PLB_INTERP_DIRECT = 2, PLB_INTERP_GENERAL = 3 };
 
