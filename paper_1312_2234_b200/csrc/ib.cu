@@ -1328,9 +1328,10 @@ int ib_max_tile_cap() {
 int ib_max_spread_cap() { return 6656; }
 
 // Which form of the spread runs: the caller's choice (ib_set_spread_mode), else by how densely the
-// tiles are sampled -- measured on the B200 (profiles/): the scatter form wins on sparsely sampled
-// tiles (config 4: 0.4 nodes per tile cell, 1.5 per occupied bin), the warp-aggregated form on
-// densely sampled ones (config 5: 0.9 per tile cell, 6 per occupied bin).
+// tiles are sampled -- measured on the B200 (profiles/r02h_*): the scatter form
+// wins on sparsely sampled tiles (config 4: 0.4 nodes per tile cell; 0.106 ms against 0.19 ms), the
+// warp-aggregated form on densely sampled ones (config 5: 0.9 per tile cell, about 4 nodes per
+// warp-group; 1.38 ms against 1.68 ms).
 int spread_mode_of(const Ctx* c) {
     if (c->spread_mode != PLB_SPREAD_AUTO) return c->spread_mode;
     return c->tile_density >= 0.6 ? PLB_SPREAD_AGGREGATE : PLB_SPREAD_SCATTER;
