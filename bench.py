@@ -418,7 +418,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (lbm_step_kernel: 152 B per cell per launch)
     peak, peak_src = hbm_peak()
     achieved = BYTES_PER_CELL * w.cells / (lbm_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "lbm_step_vec_kernel<MODE,4,128,4> (lbm_step)", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "lbm_step_vec_kernel<MODE,4,128,4,WALLS> (lbm_step)", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": ncu_traffic(args.config),
                 "traffic_source": "static: profiles/lbm_dram_traffic.txt (one ncu --set full capture of this kernel; "
                                   "not measured in this run)",

@@ -279,6 +279,10 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->mesh_node_off.push_back(0);
     c->mesh_edge_off.push_back(0);
     carve(c, (char*)d_workspace, cells, n_segs, max_nodes, max_edges);
+    if (const char* e = getenv("PLB_BOX_CAP")) {                        // test knob: ranges whose box the spread stores
+        const int v = atoi(e);
+        if (v >= 0 && v < c->box_cap) c->box_cap = v;
+    }
 
     LbmParams& p = c->prm;
     p.nx = grid->nx; p.ny = grid->ny; p.nz = grid->nz; p.cells = (int)cells;
