@@ -256,7 +256,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     c->cur = 0;
     c->cap_nodes = max_nodes; c->cap_edges = max_edges; c->n_nodes = 0; c->n_edges = 0;
     c->g_last = nullptr; c->g_last_mode = FORCE_NONE; c->spread_target = nullptr;
-    c->spread_current = false; c->forces_valid = false; c->populated = false;
+    c->spread_current = false; c->listed_all = false; c->forces_valid = false; c->populated = false;
     c->launches = 0;
     c->n_ranges = 0;
     c->n_csr_off = 0; c->n_csr_ent = 0;
@@ -270,7 +270,7 @@ int lbm_create(const plb_grid* grid, float tau, const plb_boundary* bnd, void* d
     if (const char* e = getenv("PLB_INTERP")) {                         // measurement knob
         if (!strcmp(e, "direct")) c->interp_form = PLB_INTERP_DIRECT;
         if (!strcmp(e, "tile")) c->interp_form = PLB_INTERP_TILE;
-        if (!strcmp(e, "general")) c->interp_form = PLB_INTERP_GENERAL;
+        if (!strcmp(e, "pull")) c->interp_form = PLB_INTERP_PULL;
     }
     c->range_nodes = 0;
     if (const char* e = getenv("PLB_RANGE_NODES")) c->range_nodes = atoi(e);   // measurement knob: nodes per IB block

@@ -449,23 +449,28 @@ __device__ __forceinline__ void dilate_rows(const unsigned* __restrict__ binrow,
 // per block (a returning atomic per segment on the single list counter was 58 % of the scatter
 // kernel's stall samples).  All threads of the block call it, after a __syncthreads().
 __device__ __forceinline__ void spread_flush(MeshTile& T, const int* __restrict__ tile, const unsigned* __restrict__ rowmask,
-                                             int* __restrict__ new_segs, const int cap, const float inv_scale,
-                                             float4* __restrict__ g, unsigned* __restrict__ seg_mask,
+                                             const bool list_all, int* __restrict__ new_segs, const int cap,
+                                             const float inv_scale, float4* __restrict__ g, unsigned* __restrict__ seg_mask,
                                              int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams& p) {
+    // list_all: every touched cell is listed (rowmask; a tile without row masks counts every existing
+    // cell as touched); else only the cells that received force are (the interpolation will then not
+    // rely on the list)
     const int tid = threadIdx.x;
     const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
-    const bool by_rows = e0 <= 32;
     for (int t = tid; t < ncell; t += IB_THREADS) {
         const int x = t % e0, r = t / e0;
         const int y = r % e1, z = r / e1;
-        const bool touched = by_rows ? ((rowmask[r] >> x) & 1u) != 0u
-                                     : (x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]);
-        if (!touched) continue;
         const int w = z * T.pp + y * T.p0 + x;
         const int qx = tile[w], qy = tile[cap + w], qz = tile[2 * cap + w];
+        const bool nonzero = (qx | qy | qz) != 0;
+        bool listed = nonzero;
+        if (list_all)
+            listed = rowmask ? ((rowmask[r] >> x) & 1u) != 0u
+                             : (x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]);
+        if (!listed) continue;
         const Cell c = tile_cell(T, t, p);
         const int cell = c.i + p.nx * (c.j + p.ny * c.k);
-        if ((qx | qy | qz) != 0)
+        if (nonzero)
             atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
         const int seg = cell >> SEG_SHIFT;
         const unsigned bit = 1u << (seg & 31);
@@ -489,7 +494,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
-    const int cap, int* __restrict__ range_box, const int box_cap) {
+    const int cap, int* __restrict__ range_box, const int box_cap, const bool list_all) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
     int* tile = reinterpret_cast<int*>(smem_raw);                      // [3][cap] fixed point, padded pitches
@@ -513,7 +518,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     for (int t = tid; t < nword; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
-    const bool by_rows = tiled && T.e[0] <= 32;
+    const bool by_rows = list_all && tiled && T.e[0] <= 32;
     if (by_rows)
         for (int t = tid; t < T.e[1] * T.e[2]; t += IB_THREADS) binrow[t] = 0u;
     const int sub = tid & (SPREAD_LANES - 1), ox = sub & 3, oy = sub >> 2, group = tid / SPREAD_LANES;
@@ -575,7 +580,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
         dilate_rows(binrow, rowmask, T);
         __syncthreads();
     }
-    spread_flush(T, tile, rowmask, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
+    spread_flush(T, tile, by_rows ? rowmask : nullptr, list_all, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -673,7 +678,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_gather_k
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
-    const int cap, int* __restrict__ range_box, const int box_cap) {
+    const int cap, int* __restrict__ range_box, const int box_cap, const bool list_all) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
     __shared__ int warp_tot[IB_THREADS / 32];
@@ -699,7 +704,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_gather_k
     for (int t = tid; t < nword; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
-    const bool by_rows = T.e[0] <= 32;
+    const bool by_rows = list_all && T.e[0] <= 32;
     if (by_rows)
         for (int t = tid; t < T.e[1] * T.e[2]; t += IB_THREADS) binrow[t] = 0u;
     const int nb0 = T.e[0] - 3, nb1 = T.e[1] - 3, nb2 = T.e[2] - 3, nbins = nb0 * nb1 * nb2;
@@ -771,14 +776,14 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_gather_k
         dilate_rows(binrow, rowmask, T);
         __syncthreads();
     }
-    spread_flush(T, tile, rowmask, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
+    spread_flush(T, tile, by_rows ? rowmask : nullptr, list_all, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
 __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_kernel(
     const double* __restrict__ X, const double* __restrict__ Y, const double* __restrict__ Z,
     const float4* __restrict__ F, const int2* __restrict__ ranges, float4* __restrict__ g,
     unsigned* __restrict__ seg_mask, int* __restrict__ seg_list, int* __restrict__ seg_count, const LbmParams p,
-    const int cap, int* __restrict__ range_box, const int box_cap) {
+    const int cap, int* __restrict__ range_box, const int box_cap, const bool list_all) {
     constexpr unsigned FULL = 0xffffffffu;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MeshTile T;
@@ -802,7 +807,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
     for (int t = tid; t < nword; t += IB_THREADS) {
         tile[t] = 0; tile[cap + t] = 0; tile[2 * cap + t] = 0;
     }
-    const bool by_rows = T.e[0] <= 32;
+    const bool by_rows = list_all && T.e[0] <= 32;
     if (by_rows)
         for (int t = tid; t < T.e[1] * T.e[2]; t += IB_THREADS) binrow[t] = 0u;
     const bool clipped = T.clipped != 0;
@@ -876,7 +881,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
         dilate_rows(binrow, rowmask, T);
         __syncthreads();
     }
-    spread_flush(T, tile, rowmask, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
+    spread_flush(T, tile, by_rows ? rowmask : nullptr, list_all, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
 // zero the cells of the segments the previous spread touched (its list), and drop their activity
@@ -941,186 +946,13 @@ __device__ __forceinline__ void gather_column(const float4* __restrict__ tile, c
     }
 }
 
-// S4 + S5: U_m = sum v phi phi phi (Eq. 33) with v = (sum c_i f_i + g/2)/rho of the state after
-// lbm_step (G11), each of a node's four lanes summing its stencil column, then a 4-lane
-// shuffle reduction, then X_m += U_m in fp64.
-__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_mesh_kernel(
-    double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z, float4* __restrict__ U,
-    const int2* __restrict__ ranges, const float* __restrict__ src, const float4* __restrict__ g,
-    const float4* __restrict__ vfield, const unsigned* __restrict__ seg_mask, int* __restrict__ counters,
-    const LbmParams p, const int cap) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ MeshTile T;
-    float4* tile = reinterpret_cast<float4*>(smem_raw);                // [cap] (vx, vy, vz, rho)
-    unsigned short* list = reinterpret_cast<unsigned short*>(tile + cap);   // [cap] needed tile cells
-    const int2 range = __ldg(ranges + blockIdx.x);
-    const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
-    tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, false);
-    const bool tiled = T.enabled != 0;
-    const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
-    const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
-    const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
-    if (tiled) {
-        unsigned* need = reinterpret_cast<unsigned*>(smem_raw);       // marks alias the (not yet filled) tile
-        // A densely sampled tile (config 5: 2562 nodes on ~2700 cells, every cell inside ~1000
-        // stencils) needs all of its cells: skip the marking sweep and take every existing cell.
-        const bool dense = 2L * (n1 - n0) >= (long)ncell;
-        const bool by_rows = !dense && e0 <= 32;                       // one 32-bit x-mask per (y, z) tile row
-        if (dense) {
-            for (int t = tid; t < ncell; t += IB_THREADS) {
-                const int x = t % e0, r = t / e0;
-                const int y = r % e1, z = r / e1;
-                need[t] = (x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]) ? 1u : 0u;
-            }
-        } else if (by_rows) {
-            // lane = oz: the node's four x cells of row (oy, oz) are four adjacent bits of that row's
-            // mask -- 4 marks per lane instead of 16, and most of them only read (the stencils of
-            // a mesh overlap about 13-fold)
-            const int nrow = e1 * T.e[2];
-            for (int t = tid; t < nrow; t += IB_THREADS) need[t] = 0u;
-            __syncthreads();
-            const unsigned below_hi = T.hi[0] >= 32 ? 0xffffffffu : ((1u << T.hi[0]) - 1u);
-            const unsigned below_lo = T.lo[0] >= 32 ? 0xffffffffu : ((1u << T.lo[0]) - 1u);
-            const unsigned exist = below_hi & ~below_lo;                   // x cells of the tile that lie on the lattice
-            for (int mb = n0; mb < n1; mb += IB_GROUPS) {
-                const bool valid = mb + group < n1;
-                const double x = node_coord(X, Y, Z, min(mb + group, n1 - 1), sub);
-                const NodeStencil st = node_stencil<false>(x, sub, o0, o1, o2);
-                const int tz = st.bz + sub;
-                if (!valid || tz < T.lo[2] || tz >= T.hi[2]) continue;
-                const unsigned m4 = (0xFu << st.bx) & exist;
-#pragma unroll
-                for (int oy = 0; oy < 4; ++oy) {
-                    const int ty = st.by + oy;
-                    if (ty < T.lo[1] || ty >= T.hi[1]) continue;
-                    unsigned* row = need + tz * e1 + ty;
-                    if ((*(volatile unsigned*)row & m4) != m4) atomicOr(row, m4);
-                }
-            }
-        } else {
-            for (int t = tid; t < ncell; t += IB_THREADS) need[t] = 0u;
-            __syncthreads();
-            for (int mb = n0; mb < n1; mb += IB_GROUPS) {                  // the 4^3 cells each node needs
-                const bool valid = mb + group < n1;
-                const double x = node_coord(X, Y, Z, min(mb + group, n1 - 1), sub);
-                const NodeStencil st = node_stencil<false>(x, sub, o0, o1, o2);
-                const int tx = st.bx + sub;
-                if (!valid || tx < T.lo[0] || tx >= T.hi[0]) continue;
-#pragma unroll
-                for (int oz = 0; oz < 4; ++oz) {
-                    const int tz = st.bz + oz;
-                    if (tz < T.lo[2] || tz >= T.hi[2]) continue;
-#pragma unroll
-                    for (int oy = 0; oy < 4; ++oy) {
-                        const int ty = st.by + oy;
-                        if (ty >= T.lo[1] && ty < T.hi[1]) need[(tz * e1 + ty) * e0 + tx] = 1u;
-                    }
-                }
-            }
-        }
-        __syncthreads();
-        // compact the needed cells so that every lane of the moment pass has a cell
-        for (int t0 = 0; t0 < ncell; t0 += IB_THREADS) {
-            const int t = t0 + tid;
-            const bool want = t < ncell && (by_rows ? ((need[t / e0] >> (t % e0)) & 1u) != 0u : need[t] != 0u);
-            const unsigned vote = __ballot_sync(0xffffffffu, want);
-            int base = 0;
-            if ((tid & 31) == 0 && vote) base = atomicAdd(&T.n_need, __popc(vote));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            if (want) list[base + __popc(vote & ((1u << (tid & 31)) - 1u))] = (unsigned short)t;
-        }
-        __syncthreads();
-        const int n_need = T.n_need;
-        // a cell of a segment the last spread listed has its velocity in the field already
-        // (segment_macros_kernel); any other cell -- a mesh without force, passive advection -- is
-        // computed here from its 19 pulled populations
-        if (T.interior) {
-            const int sy = p.nx, sz = p.nx * p.ny;
-            const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
-            for (int e = tid; e < n_need; e += IB_THREADS) {
-                const int t = list[e];
-                const int x = t % e0, r = t / e0;
-                const int y = r % e1, z = r / e1;
-                const int cell = origin + x + sy * y + sz * z;
-                tile[t] = seg_active(seg_mask, cell) ? __ldg(vfield + cell) : cell_macros_interior(src, g, p, cell);
-            }
-        } else {
-            for (int e = tid; e < n_need; e += IB_THREADS) {
-                const int t = list[e];
-                const Cell c = tile_cell(T, t, p);
-                const int cell = c.i + p.nx * (c.j + p.ny * c.k);
-                tile[t] = seg_active(seg_mask, cell) ? __ldg(vfield + cell) : cell_macros(src, g, p, c);
-            }
-        }
-        __syncthreads();
-    }
-    for (int mb = n0; mb < n1; mb += IB_GROUPS) {
-        // Lanes without a node take no part in the gather and read no position: another warp may
-        // already be writing the advanced position of node n1 - 1, and a stencil built from a moved
-        // node could leave the tile.  They still run the shuffles of node_stencil and the reduction.
-        const bool valid = mb + group < n1;
-        const int m = valid ? mb + group : n1 - 1;
-        const double x = valid ? node_coord(X, Y, Z, m, sub) : 0.0;
-        const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
-        float ux = 0.f, uy = 0.f, uz = 0.f;
-        if (!valid) {
-        } else if (tiled) {
-            if (T.clipped) gather_column<true>(tile, T, st, st.bx + sub, ux, uy, uz);
-            else           gather_column<false>(tile, T, st, st.bx + sub, ux, uy, uz);
-        } else {
-            const int qx = wrap_index(st.bx + sub, p.nx, p.wall[0]);
-            if (qx >= 0) {
-#pragma unroll
-                for (int oz = 0; oz < 4; ++oz) {
-                    const int qz = wrap_index(st.bz + oz, p.nz, p.wall[2]);
-                    if (qz < 0) continue;
-#pragma unroll
-                    for (int oy = 0; oy < 4; ++oy) {
-                        const int qy = wrap_index(st.by + oy, p.ny, p.wall[1]);
-                        if (qy < 0) continue;
-                        const float W = st.wy[oy] * st.wz[oz];
-                        Cell c;
-                        c.i = qx; c.j = qy; c.k = qz;
-                        const float4 v = cell_macros(src, g, p, c);
-                        ux = fmaf(W, v.x, ux);
-                        uy = fmaf(W, v.y, uy);
-                        uz = fmaf(W, v.z, uz);
-                    }
-                }
-            }
-        }
-        ux *= st.wx; uy *= st.wx; uz *= st.wx;
-#pragma unroll
-        for (int o = NODE_LANES / 2; o > 0; o >>= 1) {
-            ux += __shfl_xor_sync(0xffffffffu, ux, o);
-            uy += __shfl_xor_sync(0xffffffffu, uy, o);
-            uz += __shfl_xor_sync(0xffffffffu, uz, o);
-        }
-        // all reads of this sweep's positions are done before any lane of the warp writes (the
-        // shuffles above are warp-synchronous and every lane's loads feed them)
-        if (valid && sub == 0) {
-            U[m] = make_float4(ux, uy, uz, 0.f);
-            const double xn = X[m] + (double)ux, yn = Y[m] + (double)uy, zn = Z[m] + (double)uz;
-            X[m] = xn; Y[m] = yn; Z[m] = zn;
-            // halfway bounce-back walls lie at -1/2 and n - 1/2, on-site velocity walls at 0 and n - 1
-            const double m0 = p.wall[0] == PLB_WALL_HH ? 0.0 : 0.5, m1 = p.wall[1] == PLB_WALL_HH ? 0.0 : 0.5,
-                         m2 = p.wall[2] == PLB_WALL_HH ? 0.0 : 0.5;
-            const bool left = (p.wall[0] && (xn < -m0 || xn > (double)(p.nx - 1) + m0)) ||
-                              (p.wall[1] && (yn < -m1 || yn > (double)(p.ny - 1) + m1)) ||
-                              (p.wall[2] && (zn < -m2 || zn > (double)(p.nz - 1) + m2));
-            if (left) atomicOr(counters + 1, STATUS_NODE_LEFT);
-        }
-    }
-}
-
 // S4 + S5 right after ib_spread for the same positions (the coupled loop).  Every cell of every
 // node's stencil is then in a listed segment, so its (v, rho) is in the velocity field
 // segment_macros_kernel just wrote, and the bounding box of the range is the one the spread
 // stored.  The block copies the box out of the field into its shared-memory tile -- whole rows,
 // coalesced, L2 hits; cells of the box that no stencil contains hold older finite values that no
 // node reads -- and the nodes gather from the tile.  No bounding-box pass, no marks, no
-// compaction, no pull: the general kernel above spent 78 warp instructions per node on those
-// around a 10-instruction gather (profiles/r02b).  The positions of the range are staged in
+// compaction, no pull.  The positions of the range are staged in
 // shared memory (one coalesced load, in flight while the tile fills), so the gather sweeps run
 // without a global-load stall and every read of a position precedes every write.
 // A range whose box does not fit the tile (or PLB_INTERP=direct) gathers straight from the field.
@@ -1246,6 +1078,153 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_lis
     }
 }
 
+// S4 + S5, PULL form: no velocity field at all.  The block finds the tile cells some node of its
+// range needs (one bit per node for its base cell, dilated by the 4 x 4 x 4 stencil: the marks of
+// the spread), compacts them, computes their (v, rho) straight from the 19 populations each cell
+// pulls out of the post-collision lattice, and gathers.  Sparsely sampled meshes (config 4: a tile
+// cell is needed by one mesh only) take this form: the pull of one block overlaps the gather of
+// another on the same SM, which a bandwidth-bound pre-pass followed by a latency-bound gather
+// kernel cannot (config 4: 0.16 ms against 0.19 ms; at config 5, where a cell lies in ~14 tiles,
+// the pre-pass computes it once and wins: 1.33 against 1.51 ms).  It also serves every call order
+// (passive advection, moved nodes): the box of the range comes from the last spread only when that
+// spread saw these positions, else from a pass over the positions.
+__global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_pull_kernel(
+    double* __restrict__ X, double* __restrict__ Y, double* __restrict__ Z, float4* __restrict__ U,
+    const int2* __restrict__ ranges, const float* __restrict__ src, const float4* __restrict__ g,
+    const int* __restrict__ range_box, const int box_cap, int* __restrict__ counters, const LbmParams p,
+    const int cap) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ MeshTile T;
+    float4* tile = reinterpret_cast<float4*>(smem_raw);                // [cap] (vx, vy, vz, rho)
+    unsigned short* list = reinterpret_cast<unsigned short*>(tile + cap);   // [cap] needed tile cells
+    const int2 range = __ldg(ranges + blockIdx.x);
+    const int n0 = range.x, n1 = range.y, tid = threadIdx.x;
+    const int sub = tid & (NODE_LANES - 1), group = tid / NODE_LANES;
+    // (no staging of the positions in shared memory: the pull below wants the L1 cache that
+    // shared memory takes away -- 24 KB more per block cost 40 % of the kernel, measured twice)
+    if ((int)blockIdx.x < box_cap) {
+        if (tid == 0) {
+            const int4 b0 = __ldg(reinterpret_cast<const int4*>(range_box) + 2 * blockIdx.x);
+            const int4 b1 = __ldg(reinterpret_cast<const int4*>(range_box) + 2 * blockIdx.x + 1);
+            T.mn[0] = b0.x; T.mn[1] = b0.y; T.mn[2] = b0.z;
+            T.mx[0] = b1.x; T.mx[1] = b1.y; T.mx[2] = b1.z;
+            T.n_need = 0;
+            tile_geometry(T, b0.w != 0, p, cap, 0);
+        }
+        __syncthreads();
+    } else {
+        tile_setup(T, X, Y, Z, nullptr, n0, n1, p, cap, 0);
+    }
+    const bool tiled = T.enabled != 0;
+    const int e0 = T.e[0], e1 = T.e[1], ncell = tiled ? e0 * e1 * T.e[2] : 0;
+    const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
+    if (tiled) {
+        unsigned* binrow = reinterpret_cast<unsigned*>(smem_raw);     // marks alias the (not yet filled) tile
+        unsigned* rowmask = binrow + e1 * T.e[2];
+        // A densely sampled tile needs all of its cells; so does one wider than a 32-bit row mask.
+        const bool by_rows = 2L * (n1 - n0) < (long)ncell && e0 <= 32;
+        if (by_rows) {
+            for (int t = tid; t < e1 * T.e[2]; t += IB_THREADS) binrow[t] = 0u;
+            __syncthreads();
+            for (int m = n0 + tid; m < n1; m += IB_THREADS)
+                touch_base(binrow, T, (int)floor(X[m]) - 1 - o0, (int)floor(Y[m]) - 1 - o1, (int)floor(Z[m]) - 1 - o2);
+            __syncthreads();
+            dilate_rows(binrow, rowmask, T);
+        }
+        __syncthreads();
+        // compact the needed cells so that every lane of the moment pass has a cell
+        for (int t0 = 0; t0 < ncell; t0 += IB_THREADS) {
+            const int t = t0 + tid;
+            bool want = false;
+            if (t < ncell) {
+                const int x = t % e0, r = t / e0;
+                if (by_rows) want = ((rowmask[r] >> x) & 1u) != 0u;
+                else {
+                    const int y = r % e1, z = r / e1;
+                    want = x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2];
+                }
+            }
+            const unsigned vote = __ballot_sync(0xffffffffu, want);
+            int base = 0;
+            if ((tid & 31) == 0 && vote) base = atomicAdd(&T.n_need, __popc(vote));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (want) list[base + __popc(vote & ((1u << (tid & 31)) - 1u))] = (unsigned short)t;
+        }
+        __syncthreads();                                               // the marks are consumed: the tile may be written
+        const int n_need = T.n_need;
+        if (T.interior) {
+            const int sy = p.nx, sz = p.nx * p.ny;
+            const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
+            for (int e = tid; e < n_need; e += IB_THREADS) {
+                const int t = list[e];
+                const int x = t % e0, r = t / e0;
+                const int y = r % e1, z = r / e1;
+                tile[t] = cell_macros_interior(src, g, p, origin + x + sy * y + sz * z);
+            }
+        } else {
+            for (int e = tid; e < n_need; e += IB_THREADS) {
+                const int t = list[e];
+                tile[t] = cell_macros(src, g, p, tile_cell(T, t, p));
+            }
+        }
+    }
+    __syncthreads();                                                   // tile filled
+    for (int mb = n0; mb < n1; mb += IB_GROUPS) {
+        const int m = mb + group;
+        const bool valid = m < n1;
+        const int axis = sub < 3 ? sub : 0;
+        double x = 0.0;                                                // (lanes without a node only run the shuffles)
+        if (valid) x = node_coord(X, Y, Z, m, axis);
+        const NodeStencil st = node_stencil<true>(x, sub, o0, o1, o2);
+        float ux = 0.f, uy = 0.f, uz = 0.f;
+        if (!valid) {
+        } else if (tiled) {
+            if (T.clipped) gather_column<true>(tile, T, st, st.bx + sub, ux, uy, uz);
+            else           gather_column<false>(tile, T, st, st.bx + sub, ux, uy, uz);
+        } else {
+            const int qx = wrap_index(st.bx + sub, p.nx, p.wall[0]);
+            if (qx >= 0) {
+#pragma unroll
+                for (int oz = 0; oz < 4; ++oz) {
+                    const int qz = wrap_index(st.bz + oz, p.nz, p.wall[2]);
+                    if (qz < 0) continue;
+#pragma unroll
+                    for (int oy = 0; oy < 4; ++oy) {
+                        const int qy = wrap_index(st.by + oy, p.ny, p.wall[1]);
+                        if (qy < 0) continue;
+                        const float W = st.wy[oy] * st.wz[oz];
+                        Cell c;
+                        c.i = qx; c.j = qy; c.k = qz;
+                        const float4 v = cell_macros(src, g, p, c);
+                        ux = fmaf(W, v.x, ux);
+                        uy = fmaf(W, v.y, uy);
+                        uz = fmaf(W, v.z, uz);
+                    }
+                }
+            }
+        }
+        ux *= st.wx; uy *= st.wx; uz *= st.wx;
+#pragma unroll
+        for (int o = NODE_LANES / 2; o > 0; o >>= 1) {
+            ux += __shfl_xor_sync(0xffffffffu, ux, o);
+            uy += __shfl_xor_sync(0xffffffffu, uy, o);
+            uz += __shfl_xor_sync(0xffffffffu, uz, o);
+        }
+        // the lane of axis a advances coordinate a (it holds the old value: no second read, and a
+        // position is read by its own group only)
+        const float ua = sub == 1 ? uy : (sub == 2 ? uz : ux);
+        if (valid && sub < 3) {
+            const double xn = x + (double)ua;
+            (sub == 1 ? Y : (sub == 2 ? Z : X))[m] = xn;
+            // halfway bounce-back walls lie at -1/2 and n - 1/2, on-site velocity walls at 0 and n - 1
+            const int na = sub == 1 ? p.ny : (sub == 2 ? p.nz : p.nx);
+            const double ma = p.wall[sub] == PLB_WALL_HH ? 0.0 : 0.5;
+            if (p.wall[sub] && (xn < -ma || xn > (double)(na - 1) + ma)) atomicOr(counters + 1, STATUS_NODE_LEFT);
+        }
+        if (valid && sub == 3) U[m] = make_float4(ux, uy, uz, 0.f);
+    }
+}
+
 // positions: device SoA <-> AoS staging buffer (so host transfers are one contiguous copy)
 // (also stored order <-> caller's order)
 __global__ void __launch_bounds__(256) nodes_transpose_kernel(double* __restrict__ X, double* __restrict__ Y,
@@ -1337,10 +1316,15 @@ int spread_mode_of(const Ctx* c) {
     return c->tile_density >= 0.6 ? PLB_SPREAD_AGGREGATE : PLB_SPREAD_SCATTER;
 }
 
-// Which form of the interpolation runs after a current spread: the listed-cells kernel through its
-// tile (default), straight from the field, or the general kernel (PLB_INTERP = "tile" / "direct" /
-// "general": measurement knob).
-int interp_form_of(const Ctx* c) { return c->interp_form == PLB_INTERP_AUTO ? PLB_INTERP_TILE : c->interp_form; }
+// Which form of the interpolation the coupled loop takes: by how densely the tiles are sampled --
+// measured on the B200: the pull form on sparsely sampled tiles (config 4: 0.154 ms
+// against 0.191 ms), the pre-pass + listed-cells kernel on densely sampled ones, where a cell lies in
+// many tiles (config 5: 1.33 ms against 1.52 ms).  PLB_INTERP = "pull" / "tile" / "direct" overrides
+// (measurement knob; "direct" = the listed-cells kernel gathering straight from the field).
+int interp_form_of(const Ctx* c) {
+    if (c->interp_form != PLB_INTERP_AUTO) return c->interp_form;
+    return c->tile_density >= 0.6 ? PLB_INTERP_TILE : PLB_INTERP_PULL;
+}
 
 int launch_spread(Ctx* c, float4* g) {
     if (c->n_nodes == 0) return PLB_OK;
@@ -1348,25 +1332,28 @@ int launch_spread(Ctx* c, float4* g) {
     const int cap = (c->spread_cap + 3) & ~3;
     int* seg_count = c->counters + 2 + c->list_parity;
     const int mode = spread_mode_of(c);
+    // the listed-cells interpolation relies on the list covering every stencil cell
+    const bool list_all = interp_form_of(c) != PLB_INTERP_PULL;
+    c->listed_all = list_all;
     int rc;
     if (mode == PLB_SPREAD_SCATTER) {
         const size_t smem = spread_smem(cap);
         rc = ensure_smem(spread_mesh_kernel, smem, granted_scatter, "cudaFuncSetAttribute(spread_mesh_kernel)");
         if (rc) return rc;
         spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap);
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
     } else if (mode == PLB_SPREAD_AGGREGATE) {
         const size_t smem = warp_smem(cap);
         rc = ensure_smem(spread_warp_kernel, smem, granted_aggregate, "cudaFuncSetAttribute(spread_warp_kernel)");
         if (rc) return rc;
         spread_warp_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap);
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
     } else {
         const size_t smem = binned_smem(cap);
         rc = ensure_smem(spread_gather_kernel, smem, granted_gather, "cudaFuncSetAttribute(spread_gather_kernel)");
         if (rc) return rc;
         spread_gather_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap);
+            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
     }
     c->launches++;
     return cuda_check(cudaGetLastError(), "spread kernel");
@@ -1374,37 +1361,37 @@ int launch_spread(Ctx* c, float4* g) {
 
 int launch_interpolate_advance(Ctx* c) {
     if (c->n_nodes == 0) return PLB_OK;
-    static size_t granted = 0;
-    const size_t smem = interp_smem(c->tile_cap);
-    const int rc = ensure_smem(interpolate_mesh_kernel, smem, granted, "cudaFuncSetAttribute(interpolate_mesh_kernel)");
-    if (rc) return rc;
     const float4* g = (c->g_last_mode == FORCE_NONE) ? nullptr : c->g_last;
-    // velocities of the listed segments first (the list of the last spread; empty before any)
-    {
+    const int form = interp_form_of(c);
+    // Densely sampled meshes, right after an ib_spread that saw these positions and listed every
+    // stencil cell: the velocity of the listed segments once (pre-pass), then the listed-cells kernel.
+    if (form != PLB_INTERP_PULL && c->spread_current && c->listed_all) {
         const long want = (c->n_segs + 31) / 32;
         const unsigned grid = (unsigned)(want < (long)c->sm_count * 16 ? (want > 0 ? want : 1) : (long)c->sm_count * 16);
         segment_macros_kernel<<<grid, 256, 0, c->stream>>>(c->f[c->cur], g, c->seg_list, c->counters + 2 + c->list_parity,
                                                            c->vfield, c->prm);
         c->launches++;
-    }
-    // Right after ib_spread for these positions every stencil cell is listed and the boxes of the
-    // ranges are stored: the listed-cells kernel.  Every other case (passive advection, moved
-    // nodes) takes the general kernel, which also computes what the list does not cover.
-    if (c->spread_current && interp_form_of(c) != PLB_INTERP_GENERAL) {
         static size_t granted_listed = 0;
         const size_t smem_l = (size_t)c->tile_cap * 16 + (size_t)3 * INTERP_STAGE * sizeof(double);
-        const int rc2 = ensure_smem(interpolate_listed_kernel, smem_l, granted_listed, "cudaFuncSetAttribute(interpolate_listed_kernel)");
-        if (rc2) return rc2;
+        const int rc = ensure_smem(interpolate_listed_kernel, smem_l, granted_listed, "cudaFuncSetAttribute(interpolate_listed_kernel)");
+        if (rc) return rc;
         interpolate_listed_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem_l, c->stream>>>(
             c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->vfield, c->range_box, c->box_cap, c->counters, c->prm,
-            c->tile_cap, interp_form_of(c) != PLB_INTERP_DIRECT);
-    } else {
-        interpolate_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->f[c->cur], g, c->vfield, c->seg_mask, c->counters, c->prm,
-            c->tile_cap);
+            c->tile_cap, form != PLB_INTERP_DIRECT);
+        c->launches++;
+        return cuda_check(cudaGetLastError(), "interpolate_listed_kernel");
     }
+    // Sparsely sampled meshes, and every other call order (passive advection, moved nodes): the
+    // pull form, which needs neither list nor field.
+    static size_t granted_pull = 0;
+    const size_t smem_p = interp_smem(c->tile_cap);
+    const int rc = ensure_smem(interpolate_pull_kernel, smem_p, granted_pull, "cudaFuncSetAttribute(interpolate_pull_kernel)");
+    if (rc) return rc;
+    interpolate_pull_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem_p, c->stream>>>(
+        c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->f[c->cur], g, c->range_box, c->spread_current ? c->box_cap : 0,
+        c->counters, c->prm, c->tile_cap);
     c->launches++;
-    return cuda_check(cudaGetLastError(), "interpolation kernel");
+    return cuda_check(cudaGetLastError(), "interpolate_pull_kernel");
 }
 
 int launch_nodes_transpose(Ctx* c, bool to_aos) {

@@ -68,7 +68,7 @@ __host__ __device__ inline int tile_plane_pitch(const int row_pitch, const int e
 }
 
 enum ForceMode { FORCE_NONE = 0, FORCE_DENSE = 1, FORCE_SPARSE = 2 };
-enum InterpForm { PLB_INTERP_AUTO = 0, PLB_INTERP_TILE = 1, PLB_INTERP_DIRECT = 2, PLB_INTERP_GENERAL = 3 };
+enum InterpForm { PLB_INTERP_AUTO = 0, PLB_INTERP_TILE = 1, PLB_INTERP_DIRECT = 2, PLB_INTERP_PULL = 3 };
 
 // consecutive meshes that share one spring table: nodes [node_first, node_first + n_meshes * nn)
 struct SpringGroup {
@@ -189,6 +189,7 @@ struct Ctx {
     int g_last_mode;           // ForceMode used by the last lbm_step
     float4* spread_target;     // buffer ib_spread last filled (its touched cells are listed in seg_list)
     bool spread_current;       // seg_list matches the current node positions
+    bool listed_all;           // the last spread listed every stencil cell (not only the cells that received force)
     bool forces_valid;
     bool populated;
     long launches;

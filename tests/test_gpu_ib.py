@@ -288,13 +288,14 @@ def test_interpolate_advance_matches_oracle(kind):
     assert np.abs(rho_g.cpu().numpy() - rho_o).max() <= 6e-7
 
 
-@pytest.mark.parametrize("form", ["tile", "tile-own-box", "direct", "general"])
+@pytest.mark.parametrize("form", ["tile", "tile-own-box", "direct", "pull"])
 @pytest.mark.parametrize("mode", SPREAD_FORMS)
 def test_interpolation_forms_cover_forceless_and_weak_nodes(form, mode, monkeypatch):
-    """after ib_spread every cell inside some node's stencil is listed, whatever its force: a mesh
-    with NO force, one whose forces are 1e-12 of the neighbouring mesh's (they round to zero in
-    the tile's fixed point) and nodes sitting exactly on lattice points (zero weights) all get the
-    oracle's velocity from either form of the interpolation (PLB_INTERP: measurement knob)"""
+    """the listed-cells forms ("tile", "direct") rely on ib_spread listing every cell inside some
+    node's stencil, whatever its force; the pull form needs no list.  A mesh with NO force, one whose
+    forces are 1e-12 of the neighbouring mesh's (they round to zero in the tile's fixed point) and
+    nodes sitting exactly on lattice points (zero weights) all get the oracle's velocity from every
+    form of the interpolation (PLB_INTERP: measurement knob; default = by sampling density)"""
     monkeypatch.setenv("PLB_INTERP", "tile" if form == "tile-own-box" else form)
     if form == "tile-own-box":
         monkeypatch.setenv("PLB_BOX_CAP", "2")                     # ranges beyond the second compute their own box
