@@ -531,6 +531,10 @@ int ib_add_meshes(plb_ctx* ctx, int n_meshes, int n_nodes, const double* h_xyz, 
             }
         }
     }
+    if (const char* e = getenv("PLB_TILE_CAP")) {                       // measurement knob: cells of the interpolation tile
+        const int v = atoi(e);
+        if (v >= 64 && v <= ib_max_tile_cap()) cap = v;
+    }
     ctx->tile_cap = cap;
     ctx->spread_cap = scap;
     ctx->tile_density = ctx->tile_cells > 0.0 ? ctx->tile_nodes / ctx->tile_cells : 0.0;

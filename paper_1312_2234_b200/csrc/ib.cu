@@ -1308,7 +1308,7 @@ int ib_max_spread_cap() { return 6656; }
 
 // Which form of the spread runs: the caller's choice (ib_set_spread_mode), else by how densely the
 // tiles are sampled -- measured on the B200 (profiles/r02h_*): the scatter form
-// wins on sparsely sampled tiles (config 4: 0.4 nodes per tile cell; 0.106 ms against 0.19 ms), the
+// wins on sparsely sampled tiles (config 4: 0.26 nodes per tile cell; 0.098 ms against 0.19 ms), the
 // warp-aggregated form on densely sampled ones (config 5: 0.9 per tile cell, about 4 nodes per
 // warp-group; 1.38 ms against 1.68 ms).
 int spread_mode_of(const Ctx* c) {
