@@ -181,9 +181,10 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// S2 and S4/S5 run one thread block per NODE RANGE (a mesh, or a slice of a very large mesh).
-// A platelet is a compact object: the 4x4x4 supports of its nodes overlap heavily (about 13
-// contributions per touched cell at config 4, 1000 at config 5), so the block accumulates /
+// S2 and S4/S5 run one thread block per NODE RANGE: a mesh, or a run of consecutive stored nodes of
+// a mesh (a surface patch, thanks to the hidden Morton order) when there are few meshes or a mesh is
+// very large.  A platelet is a compact object: the 4x4x4 supports of its nodes overlap heavily (about
+// 13 contributions per touched cell at config 4, 1000 at config 5), so the block accumulates /
 // gathers through a TILE of the lattice held in shared memory -- the bounding box of the
 // supports of its nodes -- and touches global memory once per tile cell:
 //   spread:       zero tile -> nodes scatter into the tile -> the non-zero tile cells go to the
@@ -191,8 +192,10 @@ __device__ __forceinline__ int wrap_index(int q, const int n, const int wall) {
 //                 point with a per-block power-of-two scale (native shared-memory integer
 //                 atomics; the fp32 ones are compare-and-swap loops): order-independent, and
 //                 with a resolution of n_nodes/8 * 2^-30 of the largest nodal force component;
-//   interpolate:  mark the tile cells some node needs -> compact them -> their v straight from
-//                 the 19 pulled populations (no velocity field in HBM) -> nodes gather from the tile.
+//   interpolate:  (pull form) mark the tile cells some node needs -> compact them -> their v
+//                 straight from the 19 pulled populations (no velocity field in HBM) -> nodes gather
+//                 from the tile; (listed-cells form, densely sampled meshes) the velocity of every
+//                 listed cell once, in a pre-pass -> tile copied from that field -> gather.
 // A range whose bounding box does not fit the tile (a non-compact "mesh") takes the direct path:
 // global REDs per (node, cell) and on-the-fly cell moments.  Both paths compute the same sums.
 // Lane layouts (each measured against the alternatives on the B200):
@@ -555,6 +558,8 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
                     if (clipped && (bz + oz < T.lo[2] || bz + oz >= T.hi[2])) continue;
                     const float wz = weight_o(sz, cz, oz);
                     const int t = t0 + oz * pp;
+                    // (F2I is not the limiter: the magic-number FMA of the gather form in its place
+                    // changed nothing -- 0.0977 vs 0.0980 ms at config 4, 1.677 vs 1.692 ms at config 5)
                     atomicAdd(tile + t, __float2int_rn(wz * fx));
                     atomicAdd(tile + cap + t, __float2int_rn(wz * fy));
                     atomicAdd(tile + 2 * cap + t, __float2int_rn(wz * fz));
@@ -1307,7 +1312,7 @@ int ib_max_tile_cap() {
 int ib_max_spread_cap() { return 6656; }
 
 // Which form of the spread runs: the caller's choice (ib_set_spread_mode), else by how densely the
-// tiles are sampled -- measured on the B200 (profiles/r02h_*): the scatter form
+// tiles are sampled -- measured on the B200 (profiles/r02p_*): the scatter form
 // wins on sparsely sampled tiles (config 4: 0.26 nodes per tile cell; 0.098 ms against 0.19 ms), the
 // warp-aggregated form on densely sampled ones (config 5: 0.9 per tile cell, about 4 nodes per
 // warp-group; 1.38 ms against 1.68 ms).
