@@ -687,13 +687,15 @@ int ib_spread(plb_ctx* ctx, float* d_forcing) {
         return PLB_ERR_ORDER;
     }
     // clear what the previous spread wrote (into whichever buffer it used) and drop its segment list
-    if (ctx->spread_target) {
+    const bool cleared = ctx->spread_target != nullptr;
+    if (cleared) {
         const int rc = launch_clear_spread(ctx, ctx->spread_target);
         if (rc) return rc;
     }
     ctx->spread_target = (float4*)d_forcing;
     ctx->spread_current = true;
-    return launch_spread(ctx, (float4*)d_forcing);
+    // the spread kernel overlaps the clear up to its flush (programmatic dependent launch, ib.cu)
+    return launch_spread(ctx, (float4*)d_forcing, cleared);
 }
 
 int ib_release_forcing(plb_ctx* ctx) {

@@ -227,6 +227,14 @@ struct MeshTile {
     int n_need;          // interpolate: number of tile cells some node needs; spread: segments newly marked
 };
 
+// Programmatic dependent launch (sm_90+): ib_spread launches clear_spread_kernel and then the spread
+// kernel.  The clear lets its dependent start at once (launch_dependents), and the spread kernel
+// runs everything that does not touch what the clear writes -- bounding box, tile zeroing, the
+// whole scatter into shared memory -- before it waits for the clear to have completed (wait),
+// just ahead of its flush into the forcing field, the activity mask and the segment list.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // set the activity bit of the 8-cell segment of a cell; the thread that sets it first also appends
 // the segment to the list the next ib_spread clears from
 __device__ __forceinline__ void mark_segment(const int cell, unsigned* __restrict__ seg_mask, int* __restrict__ seg_list,
@@ -513,6 +521,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
     tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
     const bool tiled = T.enabled != 0 && fmax < 3.0e38f;
+    if (!tiled) pdl_wait();                                            // the direct path writes the field as it goes
     const int nword = tiled ? T.pp * T.e[2] : 0;
     // |tile value| <= n_nodes * max W * max|F| = bound; scale = 2^k with bound * scale < 2^30
     // (a range without force still runs: its cells are listed for the interpolation)
@@ -585,6 +594,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_mesh_ker
         dilate_rows(binrow, rowmask, T);
         __syncthreads();
     }
+    pdl_wait();
     spread_flush(T, tile, by_rows ? rowmask : nullptr, list_all, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
@@ -698,6 +708,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_gather_k
     tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
     if (T.enabled == 0 || !(fmax < 3.0e38f)) {
+        pdl_wait();
         spread_direct(X, Y, Z, F, n0, n1, g, seg_mask, seg_list, seg_count, p);
         return;
     }
@@ -781,6 +792,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_gather_k
         dilate_rows(binrow, rowmask, T);
         __syncthreads();
     }
+    pdl_wait();
     spread_flush(T, tile, by_rows ? rowmask : nullptr, list_all, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
@@ -802,6 +814,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
     tile_setup(T, X, Y, Z, F, n0, n1, p, cap, true, (int)blockIdx.x < box_cap ? range_box + 8 * blockIdx.x : nullptr);
     const float fmax = __uint_as_float(T.fmax_bits);
     if (T.enabled == 0 || !(fmax < 3.0e38f)) {
+        pdl_wait();
         spread_direct(X, Y, Z, F, n0, n1, g, seg_mask, seg_list, seg_count, p);
         return;
     }
@@ -886,6 +899,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
         dilate_rows(binrow, rowmask, T);
         __syncthreads();
     }
+    pdl_wait();
     spread_flush(T, tile, by_rows ? rowmask : nullptr, list_all, new_segs, cap, inv_scale, g, seg_mask, seg_list, seg_count, p);
 }
 
@@ -895,6 +909,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) spread_warp_ker
 __global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ g, unsigned* __restrict__ seg_mask,
                                                            const int* __restrict__ seg_list, const int* __restrict__ count_done,
                                                            int* __restrict__ count_next, const int cells) {
+    pdl_launch_dependents();                                           // the spread kernel may start its prologue
     const int n = *count_done;
     const int lane8 = threadIdx.x & (SEG - 1);
     const int stride = gridDim.x * (256 / SEG);
@@ -1331,7 +1346,21 @@ int interp_form_of(const Ctx* c) {
     return c->tile_density >= 0.6 ? PLB_INTERP_TILE : PLB_INTERP_PULL;
 }
 
-int launch_spread(Ctx* c, float4* g) {
+// launch with the programmatic-stream-serialization attribute: the kernel may start before the
+// preceding kernel of the stream has completed and synchronises with it by griddepcontrol.wait
+template <typename... KArgs, typename... Args>
+static void launch_overlapped(void (*kernel)(KArgs...), const unsigned grid, const unsigned block, const size_t smem,
+                              cudaStream_t stream, const bool overlap, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = overlap ? 1 : 0;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
+int launch_spread(Ctx* c, float4* g, bool after_clear) {
     if (c->n_nodes == 0) return PLB_OK;
     static size_t granted_scatter = 0, granted_aggregate = 0, granted_gather = 0;
     const int cap = (c->spread_cap + 3) & ~3;
@@ -1345,20 +1374,20 @@ int launch_spread(Ctx* c, float4* g) {
         const size_t smem = spread_smem(cap);
         rc = ensure_smem(spread_mesh_kernel, smem, granted_scatter, "cudaFuncSetAttribute(spread_mesh_kernel)");
         if (rc) return rc;
-        spread_mesh_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
+        launch_overlapped(spread_mesh_kernel, (unsigned)c->n_ranges, IB_THREADS, smem, c->stream, after_clear,
+                          c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
     } else if (mode == PLB_SPREAD_AGGREGATE) {
         const size_t smem = warp_smem(cap);
         rc = ensure_smem(spread_warp_kernel, smem, granted_aggregate, "cudaFuncSetAttribute(spread_warp_kernel)");
         if (rc) return rc;
-        spread_warp_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
+        launch_overlapped(spread_warp_kernel, (unsigned)c->n_ranges, IB_THREADS, smem, c->stream, after_clear,
+                          c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
     } else {
         const size_t smem = binned_smem(cap);
         rc = ensure_smem(spread_gather_kernel, smem, granted_gather, "cudaFuncSetAttribute(spread_gather_kernel)");
         if (rc) return rc;
-        spread_gather_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
+        launch_overlapped(spread_gather_kernel, (unsigned)c->n_ranges, IB_THREADS, smem, c->stream, after_clear,
+                          c->X[0], c->X[1], c->X[2], c->F, c->ranges, g, c->seg_mask, c->seg_list, seg_count, c->prm, cap, c->range_box, c->box_cap, list_all);
     }
     c->launches++;
     return cuda_check(cudaGetLastError(), "spread kernel");

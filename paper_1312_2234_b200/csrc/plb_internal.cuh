@@ -210,7 +210,7 @@ int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigne
 // host-side geometry of the unstressed shape (set-up, not on the timed path)
 void reference_area_volume(const double* xyz, int n_tris, const int* tris, float* S0, double* S0_tot, double* V0);
 int launch_clear_spread(Ctx* c, float4* g);
-int launch_spread(Ctx* c, float4* g);
+int launch_spread(Ctx* c, float4* g, bool after_clear);
 int spread_mode_of(const Ctx* c);
 int interp_form_of(const Ctx* c);
 int launch_interpolate_advance(Ctx* c);
