@@ -932,6 +932,7 @@ __global__ void __launch_bounds__(256) clear_spread_kernel(float4* __restrict__ 
 __global__ void __launch_bounds__(256, 4) segment_macros_kernel(const float* __restrict__ src, const float4* __restrict__ g,
                                                              const int* __restrict__ seg_list, const int* __restrict__ seg_count,
                                                              float4* __restrict__ vfield, const LbmParams p) {
+    pdl_launch_dependents();                                           // the listed-cells kernel may stage its positions
     const int n = *seg_count;
     const int lane8 = threadIdx.x & (SEG - 1);
     const int stride = gridDim.x * (256 / SEG);
@@ -1068,6 +1069,7 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_lis
     }
     const bool tiled = T.enabled != 0;
     const int o0 = tiled ? T.o[0] : 0, o1 = tiled ? T.o[1] : 0, o2 = tiled ? T.o[2] : 0;
+    pdl_wait();                                                        // the pre-pass has written the velocity field
     if (tiled) {
         const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
         if (T.interior) {
@@ -1409,9 +1411,11 @@ int launch_interpolate_advance(Ctx* c) {
         const size_t smem_l = (size_t)c->tile_cap * 16 + (size_t)3 * INTERP_STAGE * sizeof(double);
         const int rc = ensure_smem(interpolate_listed_kernel, smem_l, granted_listed, "cudaFuncSetAttribute(interpolate_listed_kernel)");
         if (rc) return rc;
-        interpolate_listed_kernel<<<(unsigned)c->n_ranges, IB_THREADS, smem_l, c->stream>>>(
-            c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->vfield, c->range_box, c->box_cap, c->counters, c->prm,
-            c->tile_cap, form != PLB_INTERP_DIRECT);
+        // a programmatic dependent launch behind the pre-pass: box, geometry and the staging of the
+        // positions overlap it, the kernel waits just ahead of its first read of the field
+        launch_overlapped(interpolate_listed_kernel, (unsigned)c->n_ranges, IB_THREADS, smem_l, c->stream, true,
+                          c->X[0], c->X[1], c->X[2], c->U, c->ranges, c->vfield, c->range_box, c->box_cap, c->counters, c->prm,
+                          c->tile_cap, form != PLB_INTERP_DIRECT);
         c->launches++;
         return cuda_check(cudaGetLastError(), "interpolate_listed_kernel");
     }
