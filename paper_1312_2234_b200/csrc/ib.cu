@@ -324,10 +324,24 @@ __device__ __forceinline__ void tile_setup(MeshTile& T, const double* __restrict
     __syncthreads();
 }
 
-// global lattice cell of tile cell t (only called for cells inside [lo, hi) on wall axes)
-__device__ __forceinline__ Cell tile_cell(const MeshTile& T, const int t, const LbmParams& p) {
-    const int x = t % T.e[0], r = t / T.e[0];
-    const int y = r % T.e[1], z = r / T.e[1];
+// tile cell index t -> (x, y, z) without integer division: t < 2^16 and 4 <= e0, e1 < 2^16, so
+// floor(t / e) = umulhi(t, floor(2^32 / e) + 1) exactly (the error term t (m e - 2^32) / 2^32 stays
+// below t e / 2^32 < 1).  The generic 32-bit division costs about 20 instructions, twice per cell.
+struct TileSplit {
+    unsigned m0, m1;
+    int e0, e1;
+    __device__ __forceinline__ explicit TileSplit(const MeshTile& T)
+        : m0(0xffffffffu / (unsigned)T.e[0] + 1u), m1(0xffffffffu / (unsigned)T.e[1] + 1u), e0(T.e[0]), e1(T.e[1]) {}
+    __device__ __forceinline__ void operator()(const int t, int& x, int& y, int& z) const {
+        const int r = (int)__umulhi((unsigned)t, m0);
+        x = t - r * e0;
+        z = (int)__umulhi((unsigned)r, m1);
+        y = r - z * e1;
+    }
+};
+
+// global lattice cell of tile cell (x, y, z) (only called for cells inside [lo, hi) on wall axes)
+__device__ __forceinline__ Cell tile_cell(const MeshTile& T, const int x, const int y, const int z, const LbmParams& p) {
     Cell c;
     c.i = wrap_index(T.o[0] + x, p.nx, 0);
     c.j = wrap_index(T.o[1] + y, p.ny, 0);
@@ -467,19 +481,20 @@ __device__ __forceinline__ void spread_flush(MeshTile& T, const int* __restrict_
     // cell as touched); else only the cells that received force are (the interpolation will then not
     // rely on the list)
     const int tid = threadIdx.x;
-    const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+    const int e1 = T.e[1], ncell = T.e[0] * e1 * T.e[2];
+    const TileSplit split(T);
     for (int t = tid; t < ncell; t += IB_THREADS) {
-        const int x = t % e0, r = t / e0;
-        const int y = r % e1, z = r / e1;
+        int x, y, z;
+        split(t, x, y, z);
         const int w = z * T.pp + y * T.p0 + x;
         const int qx = tile[w], qy = tile[cap + w], qz = tile[2 * cap + w];
         const bool nonzero = (qx | qy | qz) != 0;
         bool listed = nonzero;
         if (list_all)
-            listed = rowmask ? ((rowmask[r] >> x) & 1u) != 0u
+            listed = rowmask ? ((rowmask[z * e1 + y] >> x) & 1u) != 0u
                              : (x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2]);
         if (!listed) continue;
-        const Cell c = tile_cell(T, t, p);
+        const Cell c = tile_cell(T, x, y, z, p);
         const int cell = c.i + p.nx * (c.j + p.ny * c.k);
         if (nonzero)
             atomicAdd(g + cell, make_float4((float)qx * inv_scale, (float)qy * inv_scale, (float)qz * inv_scale, 0.f));
@@ -1072,20 +1087,21 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_lis
     pdl_wait();                                                        // the pre-pass has written the velocity field
     if (tiled) {
         const int e0 = T.e[0], e1 = T.e[1], ncell = e0 * e1 * T.e[2];
+        const TileSplit split(T);
         if (T.interior) {
             const int sy = p.nx, sz = p.nx * p.ny;
             const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
             for (int t = tid; t < ncell; t += IB_THREADS) {
-                const int x = t % e0, r = t / e0;
-                const int y = r % e1, z = r / e1;
+                int x, y, z;
+                split(t, x, y, z);
                 tile[t] = __ldg(vfield + (origin + x + sy * y + sz * z));
             }
         } else {
             for (int t = tid; t < ncell; t += IB_THREADS) {
-                const int x = t % e0, r = t / e0;
-                const int y = r % e1, z = r / e1;
+                int x, y, z;
+                split(t, x, y, z);
                 if (x < T.lo[0] || x >= T.hi[0] || y < T.lo[1] || y >= T.hi[1] || z < T.lo[2] || z >= T.hi[2]) continue;
-                const Cell c = tile_cell(T, t, p);
+                const Cell c = tile_cell(T, x, y, z, p);
                 tile[t] = __ldg(vfield + (c.i + p.nx * (c.j + p.ny * c.k)));
             }
         }
@@ -1155,16 +1171,15 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_pul
         }
         __syncthreads();
         // compact the needed cells so that every lane of the moment pass has a cell
+        const TileSplit split(T);
         for (int t0 = 0; t0 < ncell; t0 += IB_THREADS) {
             const int t = t0 + tid;
             bool want = false;
             if (t < ncell) {
-                const int x = t % e0, r = t / e0;
-                if (by_rows) want = ((rowmask[r] >> x) & 1u) != 0u;
-                else {
-                    const int y = r % e1, z = r / e1;
-                    want = x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2];
-                }
+                int x, y, z;
+                split(t, x, y, z);
+                if (by_rows) want = ((rowmask[z * e1 + y] >> x) & 1u) != 0u;
+                else want = x >= T.lo[0] && x < T.hi[0] && y >= T.lo[1] && y < T.hi[1] && z >= T.lo[2] && z < T.hi[2];
             }
             const unsigned vote = __ballot_sync(0xffffffffu, want);
             int base = 0;
@@ -1179,14 +1194,16 @@ __global__ void __launch_bounds__(IB_THREADS, 1024 / IB_THREADS) interpolate_pul
             const int origin = T.o[0] + sy * T.o[1] + sz * T.o[2];
             for (int e = tid; e < n_need; e += IB_THREADS) {
                 const int t = list[e];
-                const int x = t % e0, r = t / e0;
-                const int y = r % e1, z = r / e1;
+                int x, y, z;
+                split(t, x, y, z);
                 tile[t] = cell_macros_interior(src, g, p, origin + x + sy * y + sz * z);
             }
         } else {
             for (int e = tid; e < n_need; e += IB_THREADS) {
                 const int t = list[e];
-                tile[t] = cell_macros(src, g, p, tile_cell(T, t, p));
+                int x, y, z;
+                split(t, x, y, z);
+                tile[t] = cell_macros(src, g, p, tile_cell(T, x, y, z, p));
             }
         }
     }
