@@ -385,6 +385,34 @@ def test_release_forcing_forgets_the_buffers():
     sim.close(); ora.close()
 
 
+@pytest.mark.parametrize("mode", SPREAD_FORMS)
+def test_spread_alternating_buffers_many_times(mode):
+    """ib_spread clears what the previous call wrote -- into whichever buffer that was -- while the
+    spread kernel already runs (it is a programmatic dependent launch behind the clear and waits
+    just ahead of its flush): 40 spreads alternating between two buffers, the nodes moved in
+    between, must each leave the oracle's field in one buffer and exact zeros in the other"""
+    w = wl.config3(nx=64, ny=32, nz=64, n_meshes=3, steps=1)
+    sim, ora = pu.build_pair(w)
+    sim.set_spread_mode(mode)
+    A, B = sim.forcing, torch.zeros_like(sim.forcing)
+    X0 = w.mesh_xyz.reshape(-1, 3)
+    rng = np.random.default_rng(113)
+    for it in range(40):
+        X = X0 + rng.uniform(-1.5, 1.5, size=(1, 3)) + 0.05 * rng.standard_normal(X0.shape)
+        sim.write_nodes(X); ora.write_nodes(X)
+        sim.compute_membrane_forces(); ora.compute_membrane_forces()
+        tgt, other = (A, B) if it % 2 == 0 else (B, A)
+        sim.spread(tgt)
+        g_o = ora.spread()
+        assert float(other.abs().max()) == 0.0
+        g_g = tgt.view(-1, 4)[:, :3].t().cpu().numpy().astype(np.float64)
+        # the gather form rounds every single product W F to 2^-22 of max|F|/8 (ib.cu), ~13 of them per
+        # cell: a few 1e-6 of the field's maximum; the other forms round once per (node, cell) at 2^-30
+        tol = 6e-6 if mode == "gather" else 2e-6
+        assert np.abs(g_g - g_o.reshape(3, -1)).max() <= tol * max(np.abs(g_o).max(), 1e-30)
+    sim.close(); ora.close()
+
+
 def test_node_leaving_channel_is_reported():
     n = (8, 8, 8)
     u = np.zeros((3, 512)); u[1] = 0.2                    # fluid moving towards the wall
