@@ -239,6 +239,19 @@ PLB_API int lbm_write_populations(plb_ctx* ctx, const float* d_f);
  * population or a density sum_i f_i (Eq. 17) that is not positive (0 = healthy); synchronises the
  * stream */
 PLB_API int lbm_check_finite(plb_ctx* ctx, long* out_bad_cells);
+/* The same count (Eq. 17: density = sum_i f_i; SURVEY.md section 5 debug aid) for
+ * callers that can neither allocate nor synchronise at the point of the call (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): the scratch of the reduction is a
+ * file-scope device array inside the library -- 256 KiB, held by every GPU that loads libplb.so until
+ * the process exits -- and the call allocates nothing, copies nothing and does not wait.
+ *   d_out_bad_cells : DEVICE pointer to one int (caller-owned); written asynchronously on the
+ *                     context's stream with the number of bad cells (deterministic, no atomics).
+ * Grids of more than PLB_STATIC_MAX_CELLS cells are refused with PLB_ERR_WORKSPACE; PLB_ERR_ORDER
+ * before the populations were set; PLB_ERR_ARG for a null pointer.  All calls on one device share
+ * the scratch array: calls that overlap on the GPU (other streams, other contexts) RACE on it;
+ * calls on one stream are safe back to back. */
+#define PLB_STATIC_MAX_CELLS 16777216L
+PLB_API int lbm_check_finite_static(plb_ctx* ctx, int* d_out_bad_cells);
 /* synchronise the stream; returns PLB_ERR_NODE_LEFT / PLB_ERR_CUDA if raised since creation */
 PLB_API int plb_status(plb_ctx* ctx);
 /* number of kernels this context has launched so far (for gpu_launches accounting) */

@@ -52,6 +52,7 @@ SYMBOLS = {
     "ib_read_bonds": (_i, [_vp, _vp]),
     "ib_write_bonds": (_i, [_vp, _vp]),
     "lbm_check_finite": (_i, [_vp, C.POINTER(_l)]),
+    "lbm_check_finite_static": (_i, [_vp, _vp]),
     "plb_status": (_i, [_vp]),
     "plb_launch_count": (_i, [_vp, C.POINTER(_l)]),
     "plb_philox4x32_10": (_i, [_vp, _l, _vp, _vp, _vp]),
@@ -305,6 +306,11 @@ def lbm_check_finite(h) -> int:
     out = _l(0)
     _check(lib().lbm_check_finite(h, C.byref(out)), "lbm_check_finite")
     return out.value
+
+
+def lbm_check_finite_static(h, d_out):
+    """d_out: a device int32 tensor of one element (written asynchronously on the context's stream)"""
+    _check(lib().lbm_check_finite_static(h, None if d_out is None else d_out.data_ptr()), "lbm_check_finite_static")
 
 
 def plb_status(h):

@@ -994,6 +994,15 @@ int lbm_check_finite(plb_ctx* ctx, long* out_bad_cells) {
     return rc;
 }
 
+int lbm_check_finite_static(plb_ctx* ctx, int* d_out_bad_cells) {
+    REQUIRE_CTX(ctx);
+    if (!d_out_bad_cells || !ctx->populated) {
+        set_error("lbm_check_finite_static: null output or populations not set");
+        return d_out_bad_cells ? PLB_ERR_ORDER : PLB_ERR_ARG;
+    }
+    return launch_check_finite_static(ctx, d_out_bad_cells);
+}
+
 int plb_status(plb_ctx* ctx) {
     REQUIRE_CTX(ctx);
     return sync_status(ctx);

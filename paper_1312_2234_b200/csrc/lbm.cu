@@ -8,6 +8,7 @@
 //                                                          bounce-back + Ladd term, rho_w = 1)
 // so one fused kernel does pull-stream -> moments -> BGK + Guo forcing -> aligned store.
 // The w_d shift keeps |stored value| ~ 1e-2 so that fp32 holds |d rho| <= 1e-6.
+#include <mutex>
 #include "plb_internal.cuh"
 #include "lbm_device.cuh"
 
@@ -436,6 +437,115 @@ __global__ void __launch_bounds__(256) check_finite_kernel(const float* __restri
     float drho, jx, jy, jz;
     moments<1, 0>(h, drho, jx, jy, jz);
     if (!finite || !(1.0f + drho > 0.f)) atomicAdd(bad, 1);
+}
+
+// ---------------------------------------------------------------------------------------------
+// lbm_check_finite_static: the same count with NO caller- or library-allocated scratch.  Some
+// callers cannot provide or allocate scratch at the point of the call (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc), and the count of
+// check_finite_kernel needs a device counter.  Here the scratch is a file-scope device array of
+// a stated maximum size: PLB_STATIC_SCRATCH_INTS ints = 256 KiB, held by every GPU that loads the
+// library until the process exits.  One slot per thread block of 256 cells, so grids of up to
+// PLB_STATIC_MAX_CELLS (plb.h) = 65,536 x 256 = 16,777,216 cells (256^3: configs 2 and 5) are served;
+// larger grids are refused.
+//   kernel 1: block b counts its bad cells and WRITES partial[b] (no atomics, no clear needed:
+//             every slot that is read was written by the same call first);
+//   kernel 2: one block sums partial[0 .. n_blocks) in a fixed order and writes *d_out.
+// Every call on a device shares the array, which keeps the last call's contents: calls that
+// overlap on the GPU (two streams, two contexts on one device) race on it.
+// In HOST code the array's name is only a stand-in for the symbol, not a device address: the
+// address kernel 1 receives comes from cudaGetSymbolAddress, asked once per device with that
+// device current.  Device code of this file names the array directly (kernel 2).
+// ---------------------------------------------------------------------------------------------
+constexpr int PLB_STATIC_SCRATCH_INTS = 65536;
+constexpr long STATIC_MAX_CELLS = (long)PLB_STATIC_SCRATCH_INTS * 256;
+static_assert(STATIC_MAX_CELLS == PLB_STATIC_MAX_CELLS, "plb.h states the limit of lbm_check_finite_static");
+static __device__ __align__(256) int g_static_scratch[PLB_STATIC_SCRATCH_INTS];
+
+__global__ void __launch_bounds__(256) check_finite_partial_kernel(const float* __restrict__ src, int* __restrict__ partial,
+                                                                   const LbmParams p) {
+    __shared__ int warp_count[8];
+    const int idx = blockIdx.x * 256 + threadIdx.x;
+    bool bad = false;
+    if (idx < p.cells) {
+        float h[Q][1];
+        pull19<1, 0>(src, p, cell_of(idx, p), idx, h);
+        bool finite = true;
+#pragma unroll
+        for (int d = 0; d < Q; ++d) finite = finite && isfinite(h[d][0]);
+        float drho, jx, jy, jz;
+        moments<1, 0>(h, drho, jx, jy, jz);
+        bad = !finite || !(1.0f + drho > 0.f);
+    }
+    const int n = __popc(__ballot_sync(0xffffffffu, bad));
+    if ((threadIdx.x & 31) == 0) warp_count[threadIdx.x >> 5] = n;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) tot += warp_count[w];
+        partial[blockIdx.x] = tot;
+    }
+}
+
+__global__ void __launch_bounds__(1024) check_finite_total_kernel(const int n_blocks, int* __restrict__ out) {
+    __shared__ int warp_sum[32];
+    int s = 0;
+    for (int b = threadIdx.x; b < n_blocks; b += 1024) s += g_static_scratch[b];   // device code names the array
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        int t = warp_sum[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+        if (threadIdx.x == 0) *out = t;
+    }
+}
+
+// device address of g_static_scratch on the CURRENT device (cudaGetSymbolAddress once per device)
+static int static_scratch_address(int** out) {
+    constexpr int MAX_DEVICES = 64;
+    static int* address[MAX_DEVICES] = {nullptr};
+    static std::mutex lock;
+    int dev = 0;
+    int rc = cuda_check(cudaGetDevice(&dev), "cudaGetDevice");
+    if (rc) return rc;
+    if (dev < 0 || dev >= MAX_DEVICES) {
+        set_error("lbm_check_finite_static: device ordinal %d out of range", dev);
+        return PLB_ERR_ARG;
+    }
+    std::lock_guard<std::mutex> guard(lock);
+    if (!address[dev]) {
+        int* ptr = nullptr;
+        rc = cuda_check(cudaGetSymbolAddress((void**)&ptr, g_static_scratch), "cudaGetSymbolAddress(g_static_scratch)");
+        if (rc) return rc;
+        if (!ptr) {
+            set_error("lbm_check_finite_static: cudaGetSymbolAddress returned a null address");
+            return PLB_ERR_CUDA;
+        }
+        address[dev] = ptr;
+    }
+    *out = address[dev];
+    return PLB_OK;
+}
+
+// asynchronous on c->stream; no allocation, no host synchronisation
+int launch_check_finite_static(Ctx* c, int* d_out) {
+    if ((long)c->prm.cells > STATIC_MAX_CELLS) {
+        set_error("lbm_check_finite_static: grid of %d cells exceeds the static scratch (%ld cells at most)", c->prm.cells,
+                  STATIC_MAX_CELLS);
+        return PLB_ERR_WORKSPACE;
+    }
+    int* partial = nullptr;
+    const int rc = static_scratch_address(&partial);
+    if (rc) return rc;
+    const int n_blocks = (c->prm.cells + 255) / 256;
+    check_finite_partial_kernel<<<n_blocks, 256, 0, c->stream>>>(c->f[c->cur], partial, c->prm);
+    check_finite_total_kernel<<<1, 1024, 0, c->stream>>>(n_blocks, d_out);
+    c->launches += 2;
+    return cuda_check(cudaGetLastError(), "check_finite_partial_kernel / check_finite_total_kernel");
 }
 
 // ---------------------------------------------------------------------------------------------

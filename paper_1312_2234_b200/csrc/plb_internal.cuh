@@ -205,6 +205,7 @@ int launch_lbm_step(Ctx* c, const float4* g, int mode);
 int launch_read_macros(Ctx* c, float* d_rho, float* d_u);
 int launch_read_populations(Ctx* c, float* d_f);
 int launch_check_finite(Ctx* c, int* d_bad);
+int launch_check_finite_static(Ctx* c, int* d_out);
 int launch_write_populations(Ctx* c, const float* d_f);
 int launch_membrane_forces(Ctx* c, float sigma, unsigned long long seed, unsigned long long step);
 // host-side geometry of the unstressed shape (set-up, not on the timed path)
