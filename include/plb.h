@@ -17,7 +17,8 @@
  *   - The FORCING field is AoS: float4 per cell = (g_x, g_y, g_z, 0), 16-byte aligned, so that
  *     the spread can use 128-bit vector atomics.
  *   - The library never allocates device memory: the caller passes one workspace of
- *     lbm_workspace_bytes() bytes (256-byte aligned) to lbm_create, which carves it.
+ *     lbm_workspace_bytes() bytes (256-byte aligned) to lbm_create, which carves it.  (One call,
+ *     lbm_check_finite_static, keeps its scratch in a 256 KiB device array inside the library.)
  *   - Calls that take only device pointers are asynchronous on the context's stream.  Calls that
  *     take host pointers synchronise that stream before returning.
  *   - Every call returns 0 on success or a negative code (below); plb_last_error() gives a
@@ -74,7 +75,8 @@ enum {
 PLB_API const char* plb_last_error(void);
 
 /* Bytes of workspace lbm_create needs for this grid and mesh capacity (two fp32 lattices, the
- * activity-segment mask and list, node, edge and triangle arrays). */
+ * activity-segment mask and list, the (v, rho) field of the listed segments, node arrays, the
+ * per-topology spring tables, node ranges and their boxes, triangle arrays). */
 PLB_API int lbm_workspace_bytes(const plb_grid* grid, long max_nodes, long max_edges, size_t* out_bytes);
 
 /* Create a context.  tau > 1/2 is the BGK relaxation time (Eq. 16).  d_workspace must stay

@@ -7,7 +7,9 @@
   steps on a sub-block cut from the seeded inputs alone (parity_utils.Block) and size-independent
   properties (mass, total spread force = total node force, springs sum to zero) are checked.
 * C2 is in test_gpu_lbm.py (reduced whole run + full-size slab oracle).
-* PLB_FULL=1 adds the full-length, full-size C3 run against the oracle (minutes of CPU time).
+* PLB_FULL=1 adds the full-length, full-size, whole-domain runs of C3 (2000 steps), C4 (500) and
+  C5 (200) against the oracle (2, 12 and 25 minutes on the GPU box's 16 host cores; results in
+  profiles/r02_full_parity.md).
 
 Tolerances are the north_star's: |dv| <= 1e-4 u_wall, |drho| <= 1e-6, |dX| <= 1e-4."""
 import os
