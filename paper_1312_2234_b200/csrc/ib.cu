@@ -1,8 +1,9 @@
 // ib.cu -- immersed-boundary and membrane kernels (Eq. 2-3, section 3.4.2 Eq. 31-36).
 //
 // Node data: positions SoA fp64 (unwrapped), forces / node velocities float4 AoS.
-// The forcing field is float4 per cell so that the spread is one 128-bit vector atomic per
-// (node, cell) pair (red.global.add.v4.f32, sm_90+).
+// The forcing field is float4 per cell so that the spread ends in one 128-bit vector atomic per
+// touched tile cell (red.global.add.v4.f32, sm_90+).  The nodes of a mesh are stored along the
+// Morton curve of the mesh's initial shape (api.cu); `orig` maps a stored node to the caller's index.
 #include <climits>
 #include "plb_internal.cuh"
 #include "lbm_device.cuh"
